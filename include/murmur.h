@@ -1,0 +1,214 @@
+/* murmur.h - C ABI of the B200-native MURMUR intra-chunk hot path.
+ *
+ * Paper: "MURMUR: An Efficient Inference System for Long-Form ASR" (arxiv/paper_2606_01483);
+ * citations below are PAPER.md:<line> of the text mounted at /root/reference/PAPER.md.
+ *
+ * What the library computes, once per decode step and per layer:
+ *   murmur_kv_append   - the newest token's K,V rows enter the KV cache C
+ *   murmur_kv_evict    - the sliding-window eviction policy is applied: Alg. 1 on output
+ *                        tokens, Eq. 2 / Alg. 2 on speech tokens
+ *                        (PAPER.md:119-146), system prompts always kept;
+ *                        dead pages are freed and the compacted page tables rebuilt
+ *                        ("cache management")
+ *   murmur_decode_attn - Eq. 1 softmax attention of one query token per
+ *                        sequence over what remains, grouped-query, fp32 softmax
+ *
+ * Sequence layout: [prefix system prompt P][speech S][system prompt M][text t].
+ * Positions are 0-based and absolute; t counts the output tokens in the cache INCLUDING the
+ * newest one.  Retained ("attended") set at step t, region-relative indices r (speech), u (out):
+ *     l(t)        = min(max(0, t - delay), max(0, S - w_speech))
+ *     keep speech : r < n_sink_speech  or  l <= r < l + w_speech
+ *     keep output : u < n_sink_out     or  u >= t - w_out
+ *     keep prefix / mid always.
+ * Tokens behind the trailing edge of their window (and not sinks) are dead for good; speech
+ * tokens ahead of the window stay resident but are not attended.  See DESIGN.md "Readings".
+ *
+ * Memory model
+ *   - The library never allocates device memory.  k_pool, v_pool and workspace are DEVICE
+ *     buffers owned by the caller (e.g. torch tensors); they must outlive the handle and be
+ *     256-byte aligned.  Sizes: murmur_pool_bytes() each for K and V, murmur_workspace_bytes().
+ *   - Pool layout is PRIVATE (pre-swizzled for the attention kernel): read rows back only
+ *     through murmur_kv_gather.
+ *   - One physical page id addresses the same logical block in every layer and in K and V.
+ *   - Arguments marked HOST are host pointers and are consumed before the call returns;
+ *     arguments marked DEVICE are device pointers borrowed until the stream work completes.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  All calls on one
+ *     handle must be issued from one host thread at a time and on one stream (or on streams
+ *     the caller orders).
+ *
+ * Errors: every call returns a murmur_status_t; nothing throws, aborts or prints.  Argument
+ * and state errors (including page exhaustion, which the host-side mirror of the integer
+ * state can always prove) are detected before any launch and leave all state unchanged.
+ * The device additionally keeps an error word (murmur_get_last_error) as a cross-check.
+ *
+ * Order per decode step: append -> evict -> decode_attn (the query of output token t attends
+ * a set containing token t itself: Alg. 1's K includes j).  evict twice at the
+ * same t is a no-op.
+ */
+#ifndef MURMUR_H_
+#define MURMUR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(_WIN32)
+#define MURMUR_API
+#else
+#define MURMUR_API __attribute__((visibility("default")))
+#endif
+
+typedef struct murmur_cache murmur_cache_t; /* opaque host object */
+
+typedef enum {
+  MURMUR_OK = 0,
+  MURMUR_ERR_INVALID_ARG = 1, /* NULL pointer, out-of-range id, bad size, duplicate sequence in a call */
+  MURMUR_ERR_STATE = 2,       /* sequence not active / already active / empty / max_blocks exceeded */
+  MURMUR_ERR_OOM_PAGES = 3,   /* the call as a whole needs more pages than are free; nothing changed */
+  MURMUR_ERR_CUDA = 4,        /* a CUDA runtime call failed */
+  MURMUR_ERR_UNSUPPORTED = 5  /* geometry outside what the kernels are built for */
+} murmur_status_t;
+
+#define MURMUR_WINDOW_OFF 0x7fffffff /* window >= any length: that region is never evicted */
+#define MURMUR_MAX_SEQS_PER_LAUNCH 128 /* larger calls are split internally, in order */
+
+/* Geometry + caller-owned buffers.
+ * Supported: head_dim == 128; n_q_heads % n_kv_heads == 0 with group size <= 8; page_size a power
+ * of two in [1, 64] (the tensor-core attention path needs page_size >= 16; smaller pages use the
+ * generic path); bf16 K/V/Q/O. */
+typedef struct {
+  int32_t n_layers, n_q_heads, n_kv_heads, head_dim; /* 28, 28, 4, 128 */
+  int32_t page_size;                                 /* tokens per page */
+  int32_t max_seqs;                                  /* sequence ids are 0 .. max_seqs-1 */
+  int32_t max_blocks_per_seq;                        /* logical blocks (pages) a sequence may ever span */
+  int64_t n_pages;                                   /* physical pages in each pool */
+  void* k_pool;                                      /* DEVICE, murmur_pool_bytes() bytes */
+  void* v_pool;                                      /* DEVICE, murmur_pool_bytes() bytes */
+  void* workspace;                                   /* DEVICE, >= murmur_workspace_bytes() bytes */
+  size_t workspace_bytes;
+} murmur_cache_desc_t;
+
+/* Per-sequence policy (paper names): w of Alg. 2, d of Alg. 2, n_sink of Eq. 2, w of Alg. 1,
+ * n_sink of Alg. 1.  All >= 0.  MURMUR_WINDOW_OFF for a window disables that eviction. */
+typedef struct {
+  int32_t w_speech, delay, n_sink_speech, w_out, n_sink_out;
+} murmur_policy_t;
+
+/* Counters kept by the host object (what was launched through this handle). */
+typedef struct {
+  int64_t kernel_launches; /* CUDA kernels launched by this handle since creation / last reset */
+  int64_t append_calls, evict_calls, attn_calls;
+  int64_t free_pages;      /* host mirror of the free-stack height */
+  int32_t attn_grid;       /* CTAs of the last attention launch */
+  int32_t attn_smem_bytes; /* dynamic shared memory of the last attention launch */
+  int32_t attn_variant;    /* variant used by the last attention launch (MURMUR_ATTN_*) */
+  int32_t sm_count;
+} murmur_stats_t;
+
+/* Options for murmur_set_option. */
+#define MURMUR_OPT_ATTN_VARIANT 1 /* value: MURMUR_ATTN_AUTO / _GENERIC / _MMA */
+#define MURMUR_OPT_ATTN_GRID 2    /* value: CTAs for the persistent attention kernel; 0 = one per SM */
+#define MURMUR_ATTN_AUTO 0    /* tensor-core split-K kernel when page_size >= 16, else generic */
+#define MURMUR_ATTN_GENERIC 1 /* one CTA per (layer, sequence, KV head), FFMA, no smem staging */
+#define MURMUR_ATTN_MMA 2     /* persistent split-K kernel: bulk-copy staging + mma.sync bf16 */
+
+/* ---- sizing ------------------------------------------------------------------------------ */
+/* Bytes of ONE pool (K or V): n_layers * n_pages * n_kv_heads * page_size * head_dim * 2. */
+MURMUR_API size_t murmur_pool_bytes(const murmur_cache_desc_t* desc);
+/* Bytes of workspace the handle needs (page tables, free stack, split-K partials, staging).
+ * Returns 0 if desc is NULL or unsupported. */
+MURMUR_API size_t murmur_workspace_bytes(const murmur_cache_desc_t* desc);
+
+/* ---- lifecycle --------------------------------------------------------------------------- */
+/* Creates the handle and initialises the workspace on `stream` (free stack = all pages, pops
+ * return page 0,1,2,...).  Pool contents are not touched.  *out is set only on MURMUR_OK. */
+MURMUR_API murmur_status_t murmur_cache_create(const murmur_cache_desc_t* desc, murmur_cache_t** out, void* stream);
+/* Frees the host object only (device buffers belong to the caller). NULL is a no-op. */
+MURMUR_API murmur_status_t murmur_cache_destroy(murmur_cache_t* cache);
+
+/* Declares sequence `seq` with its region sizes and policy; it starts empty.  The first
+ * n_prefix + n_speech + n_mid tokens appended are the prefill, later ones are output tokens. */
+MURMUR_API murmur_status_t murmur_seq_begin(murmur_cache_t* cache, int32_t seq, int32_t n_prefix, int32_t n_speech,
+                                            int32_t n_mid, const murmur_policy_t* policy, void* stream);
+/* Ends the sequence; its live pages are pushed on the free stack in ascending block order. */
+MURMUR_API murmur_status_t murmur_seq_end(murmur_cache_t* cache, int32_t seq, void* stream);
+
+/* ---- the hot path ------------------------------------------------------------------------ */
+/* Appends n_tokens[i] tokens to sequence seq_ids[i].
+ *   seq_ids, n_tokens : HOST int32[n_seqs]; ids distinct and active; n_tokens[i] >= 0.
+ *   k_new, v_new      : DEVICE bf16 [layer_end-layer_begin][sum n_tokens][n_kv_heads][head_dim],
+ *                       tokens of a sequence contiguous, sequences in call order.
+ *   layer_begin == 0 reserves the slots (allocating pages in call order, new blocks ascending;
+ *   all-or-nothing) and advances the sequence lengths; a call with layer_begin > 0 only writes
+ *   rows for the LAST n_tokens[i] reserved positions (engines that produce layer l's K/V at
+ *   layer l call it once per layer range).  Bulk prefill and 1-token decode use the same call. */
+MURMUR_API murmur_status_t murmur_kv_append(murmur_cache_t* cache, const int32_t* seq_ids, const int32_t* n_tokens,
+                                            int32_t n_seqs, const void* k_new, const void* v_new,
+                                            int32_t layer_begin, int32_t layer_end, void* stream);
+
+/* Applies each sequence's policy at its current t: frees blocks whose every
+ * position is dead (sequences in call order, blocks ascending), rebuilds the compacted live-page
+ * list, the run descriptors (maximal intervals of the retained set) and the attention work
+ * list.  No K/V bytes move.  seq_ids: HOST int32[n_seqs], distinct, active. */
+MURMUR_API murmur_status_t murmur_kv_evict(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs, void* stream);
+
+/* Eq. 1: out[l][i][h] = sum_x alpha_x v_x over the retained set of seq_ids[i]
+ * as of its last murmur_kv_evict, alpha = softmax(q . k_x * sm_scale), KV head of query head h
+ * is h / (n_q_heads / n_kv_heads).
+ *   q, out : DEVICE bf16 [layer_end-layer_begin][n_seqs][n_q_heads][head_dim]
+ *   lse    : DEVICE fp32 [layer_end-layer_begin][n_seqs][n_q_heads] natural-log-sum-exp of the
+ *            scaled scores, or NULL
+ * Every listed sequence must have a non-empty retained set and have been evicted since its last
+ * append (else MURMUR_ERR_STATE). */
+MURMUR_API murmur_status_t murmur_decode_attn(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                              const void* q, void* out, float* lse, int32_t layer_begin,
+                                              int32_t layer_end, float sm_scale, void* stream);
+
+/* One whole decode step from HOST buffers (the end-to-end entry): copies k_new, v_new, q
+ * (HOST, pinned or pageable, layouts as above with 1 token per sequence and all layers) to
+ * device staging, runs append -> evict -> decode_attn, copies out (HOST bf16
+ * [n_layers][n_seqs][n_q_heads][head_dim]) back, all on `stream`; returns after enqueueing
+ * (synchronise the stream before reading out_host).  n_seqs <= MURMUR_MAX_SEQS_PER_LAUNCH. */
+MURMUR_API murmur_status_t murmur_decode_step_host(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                                   const void* k_new_host, const void* v_new_host,
+                                                   const void* q_host, void* out_host, float sm_scale, void* stream);
+
+/* ---- introspection (tests; each call synchronises the stream it is given) ------------------ */
+/* state_out[0..5] = length, t, n_live_blocks, n_runs, n_attn_tiles, n_retained (device values). */
+MURMUR_API murmur_status_t murmur_seq_get_state(murmur_cache_t* cache, int32_t seq, int32_t* state_out, void* stream);
+/* Sorted absolute positions of the retained set (expanded on the device from the run descriptors). */
+MURMUR_API murmur_status_t murmur_kv_get_retained(murmur_cache_t* cache, int32_t seq, int32_t* pos_out, int32_t cap,
+                                                  int32_t* n_out, void* stream);
+/* Compacted page table: physical ids and logical block numbers of the live blocks, ascending. */
+MURMUR_API murmur_status_t murmur_kv_get_page_list(murmur_cache_t* cache, int32_t seq, int32_t* pages_out,
+                                                   int32_t* blocks_out, int32_t cap, int32_t* n_out, void* stream);
+/* Run descriptors: runs_out[3*k+0..2] = first_pos, n_tok, index of the run's first block in the page list. */
+MURMUR_API murmur_status_t murmur_kv_get_runs(murmur_cache_t* cache, int32_t seq, int32_t* runs_out, int32_t cap_runs,
+                                              int32_t* n_out, void* stream);
+/* Free stack, bottom to top (the next pop returns the last element). */
+MURMUR_API murmur_status_t murmur_kv_get_free_stack(murmur_cache_t* cache, int32_t* pages_out, int64_t cap,
+                                                    int64_t* n_out, void* stream);
+/* Gathers the K and V rows of n positions (HOST int32[n], all resident) of one sequence into
+ * k_out, v_out: DEVICE bf16 [layer_end-layer_begin][n][n_kv_heads][head_dim], natural order. */
+MURMUR_API murmur_status_t murmur_kv_gather(murmur_cache_t* cache, int32_t seq, const int32_t* positions, int32_t n,
+                                            int32_t layer_begin, int32_t layer_end, void* k_out, void* v_out,
+                                            void* stream);
+/* Device error word: 0 or the first MURMUR_ERR_* a kernel detected since creation. */
+MURMUR_API murmur_status_t murmur_get_last_error(murmur_cache_t* cache, int32_t* device_err_out, void* stream);
+
+/* ---- options / stats --------------------------------------------------------------------- */
+MURMUR_API murmur_status_t murmur_set_option(murmur_cache_t* cache, int32_t option, int32_t value);
+MURMUR_API murmur_status_t murmur_get_stats(murmur_cache_t* cache, murmur_stats_t* out);
+MURMUR_API murmur_status_t murmur_reset_stats(murmur_cache_t* cache);
+MURMUR_API const char* murmur_status_str(murmur_status_t s);
+/* Text of the CUDA error behind the last MURMUR_ERR_CUDA returned through this handle. */
+MURMUR_API const char* murmur_last_cuda_error(murmur_cache_t* cache);
+MURMUR_API const char* murmur_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MURMUR_H_ */

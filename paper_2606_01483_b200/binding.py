@@ -1,0 +1,277 @@
+"""Thin ctypes binding over the C ABI of include/murmur.h.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of libmurmur.so.
+PyTorch is used for device memory (pools, workspace, Q/O tensors) and the current stream.
+There is no CPU fallback: if the library cannot be loaded, importing ``lib()`` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+MURMUR_WINDOW_OFF = 0x7FFFFFFF
+MURMUR_OPT_ATTN_VARIANT = 1
+MURMUR_OPT_ATTN_GRID = 2
+MURMUR_ATTN_AUTO, MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA = 0, 1, 2
+
+STATUS_NAMES = {0: "MURMUR_OK", 1: "MURMUR_ERR_INVALID_ARG", 2: "MURMUR_ERR_STATE", 3: "MURMUR_ERR_OOM_PAGES",
+                4: "MURMUR_ERR_CUDA", 5: "MURMUR_ERR_UNSUPPORTED"}
+
+# every symbol include/murmur.h declares (checked by tests/test_abi.py)
+EXPORTED_SYMBOLS = [
+    "murmur_pool_bytes", "murmur_workspace_bytes", "murmur_cache_create", "murmur_cache_destroy",
+    "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
+    "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
+    "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
+    "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
+    "murmur_last_cuda_error", "murmur_version",
+]
+
+
+class CacheDesc(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32),
+                ("head_dim", C.c_int32), ("page_size", C.c_int32), ("max_seqs", C.c_int32),
+                ("max_blocks_per_seq", C.c_int32), ("n_pages", C.c_int64), ("k_pool", C.c_void_p),
+                ("v_pool", C.c_void_p), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+class Policy(C.Structure):
+    _fields_ = [("w_speech", C.c_int32), ("delay", C.c_int32), ("n_sink_speech", C.c_int32),
+                ("w_out", C.c_int32), ("n_sink_out", C.c_int32)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("kernel_launches", C.c_int64), ("append_calls", C.c_int64), ("evict_calls", C.c_int64),
+                ("attn_calls", C.c_int64), ("free_pages", C.c_int64), ("attn_grid", C.c_int32),
+                ("attn_smem_bytes", C.c_int32), ("attn_variant", C.c_int32), ("sm_count", C.c_int32)]
+
+
+class MurmurError(RuntimeError):
+    def __init__(self, status: int, what: str = ""):
+        self.status = status
+        super().__init__(f"{STATUS_NAMES.get(status, status)} {what}".strip())
+
+
+_lib: Optional[C.CDLL] = None
+
+
+def lib() -> C.CDLL:
+    """Loads (building if needed) libmurmur.so.  Raises if it cannot - there is no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path) or _build._stale():
+        path = _build.build()
+    L = C.CDLL(path)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    L.murmur_pool_bytes.restype = C.c_size_t
+    L.murmur_pool_bytes.argtypes = [C.POINTER(CacheDesc)]
+    L.murmur_workspace_bytes.restype = C.c_size_t
+    L.murmur_workspace_bytes.argtypes = [C.POINTER(CacheDesc)]
+    L.murmur_cache_create.argtypes = [C.POINTER(CacheDesc), C.POINTER(vp), vp]
+    L.murmur_cache_destroy.argtypes = [vp]
+    L.murmur_seq_begin.argtypes = [vp, i32, i32, i32, i32, C.POINTER(Policy), vp]
+    L.murmur_seq_end.argtypes = [vp, i32, vp]
+    L.murmur_kv_append.argtypes = [vp, vp, vp, i32, vp, vp, i32, i32, vp]
+    L.murmur_kv_evict.argtypes = [vp, vp, i32, vp]
+    L.murmur_decode_attn.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, C.c_float, vp]
+    L.murmur_decode_step_host.argtypes = [vp, vp, i32, vp, vp, vp, vp, C.c_float, vp]
+    L.murmur_seq_get_state.argtypes = [vp, i32, vp, vp]
+    L.murmur_kv_get_retained.argtypes = [vp, i32, vp, i32, vp, vp]
+    L.murmur_kv_get_page_list.argtypes = [vp, i32, vp, vp, i32, vp, vp]
+    L.murmur_kv_get_runs.argtypes = [vp, i32, vp, i32, vp, vp]
+    L.murmur_kv_get_free_stack.argtypes = [vp, vp, i64, vp, vp]
+    L.murmur_kv_gather.argtypes = [vp, i32, vp, i32, i32, i32, vp, vp, vp]
+    L.murmur_get_last_error.argtypes = [vp, vp, vp]
+    L.murmur_set_option.argtypes = [vp, i32, i32]
+    L.murmur_get_stats.argtypes = [vp, C.POINTER(Stats)]
+    L.murmur_reset_stats.argtypes = [vp]
+    L.murmur_status_str.restype = C.c_char_p
+    L.murmur_status_str.argtypes = [C.c_int]
+    L.murmur_last_cuda_error.restype = C.c_char_p
+    L.murmur_last_cuda_error.argtypes = [vp]
+    L.murmur_version.restype = C.c_char_p
+    for name in EXPORTED_SYMBOLS:
+        fn = getattr(L, name)
+        if fn.restype is C.c_int:  # default restype: status codes
+            fn.restype = C.c_int
+    _lib = L
+    return L
+
+
+def _ids(a: Sequence[int]) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+
+
+def _stream() -> int:
+    return int(torch.cuda.current_stream().cuda_stream)
+
+
+class MurmurCache:
+    """Owns the device buffers (torch tensors) and the murmur_cache_t handle."""
+
+    def __init__(self, n_layers: int, n_q_heads: int, n_kv_heads: int, head_dim: int, page_size: int,
+                 max_seqs: int, max_blocks_per_seq: int, n_pages: int, device="cuda:0"):
+        self.L = lib()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.n_layers, self.n_q, self.n_kv, self.d = n_layers, n_q_heads, n_kv_heads, head_dim
+        self.page_size, self.max_seqs, self.max_blocks, self.n_pages = page_size, max_seqs, max_blocks_per_seq, n_pages
+        d = CacheDesc(n_layers, n_q_heads, n_kv_heads, head_dim, page_size, max_seqs, max_blocks_per_seq, n_pages,
+                      None, None, None, 0)
+        pool_bytes = self.L.murmur_pool_bytes(C.byref(d))
+        ws_bytes = self.L.murmur_workspace_bytes(C.byref(d))
+        if pool_bytes == 0 or ws_bytes == 0:
+            raise MurmurError(5, "unsupported geometry")
+        self.k_pool = torch.empty(pool_bytes, dtype=torch.uint8, device=self.device)
+        self.v_pool = torch.empty(pool_bytes, dtype=torch.uint8, device=self.device)
+        self.workspace = torch.empty(ws_bytes, dtype=torch.uint8, device=self.device)
+        d.k_pool, d.v_pool, d.workspace = self.k_pool.data_ptr(), self.v_pool.data_ptr(), self.workspace.data_ptr()
+        d.workspace_bytes = ws_bytes
+        self.desc = d
+        h = C.c_void_p()
+        self._check(self.L.murmur_cache_create(C.byref(d), C.byref(h), _stream()))
+        self.h = h
+
+    def close(self):
+        if getattr(self, "h", None):
+            torch.cuda.synchronize(self.device)
+            self.L.murmur_cache_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int):
+        if st != 0:
+            what = ""
+            if st == 4 and getattr(self, "h", None):
+                what = self.L.murmur_last_cuda_error(self.h).decode()
+            raise MurmurError(st, what)
+
+    # ---- lifecycle ----------------------------------------------------------------------
+    def seq_begin(self, seq: int, n_prefix: int, n_speech: int, n_mid: int, policy: Tuple[int, int, int, int, int]):
+        pol = Policy(*policy)
+        self._check(self.L.murmur_seq_begin(self.h, seq, n_prefix, n_speech, n_mid, C.byref(pol), _stream()))
+
+    def seq_end(self, seq: int):
+        self._check(self.L.murmur_seq_end(self.h, seq, _stream()))
+
+    # ---- hot path -----------------------------------------------------------------------
+    def kv_append(self, seq_ids, n_tokens, k_new: torch.Tensor, v_new: torch.Tensor, layer_begin: int = 0,
+                  layer_end: Optional[int] = None):
+        layer_end = self.n_layers if layer_end is None else layer_end
+        ids, nt = _ids(seq_ids), _ids(n_tokens)
+        total = int(nt.sum())
+        for t in (k_new, v_new):
+            assert t.dtype == torch.bfloat16 and t.is_cuda and t.is_contiguous()
+            assert t.numel() == (layer_end - layer_begin) * total * self.n_kv * self.d, "k_new/v_new shape"
+        self._check(self.L.murmur_kv_append(self.h, ids.ctypes.data, nt.ctypes.data, len(ids), k_new.data_ptr(),
+                                            v_new.data_ptr(), layer_begin, layer_end, _stream()))
+
+    def kv_evict(self, seq_ids):
+        ids = _ids(seq_ids)
+        self._check(self.L.murmur_kv_evict(self.h, ids.ctypes.data, len(ids), _stream()))
+
+    def decode_attn(self, seq_ids, q: torch.Tensor, out: Optional[torch.Tensor] = None,
+                    lse: Optional[torch.Tensor] = None, sm_scale: Optional[float] = None, layer_begin: int = 0,
+                    layer_end: Optional[int] = None) -> torch.Tensor:
+        layer_end = self.n_layers if layer_end is None else layer_end
+        ids = _ids(seq_ids)
+        shape = (layer_end - layer_begin, len(ids), self.n_q, self.d)
+        assert q.dtype == torch.bfloat16 and q.is_cuda and q.is_contiguous() and tuple(q.shape) == shape
+        if out is None:
+            out = torch.empty(shape, dtype=torch.bfloat16, device=self.device)
+        assert out.dtype == torch.bfloat16 and out.is_contiguous() and tuple(out.shape) == shape
+        if lse is not None:
+            assert lse.dtype == torch.float32 and lse.is_contiguous() and tuple(lse.shape) == shape[:3]
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        self._check(self.L.murmur_decode_attn(self.h, ids.ctypes.data, len(ids), q.data_ptr(), out.data_ptr(),
+                                              lse.data_ptr() if lse is not None else None, layer_begin, layer_end,
+                                              C.c_float(sm_scale), _stream()))
+        return out
+
+    def decode_step_host(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor,
+                         out: torch.Tensor, sm_scale: Optional[float] = None):
+        """All tensors are HOST (ideally pinned) bf16; enqueues H2D + append + evict + attn + D2H."""
+        ids = _ids(seq_ids)
+        for t in (k_new, v_new, q, out):
+            assert t.dtype == torch.bfloat16 and not t.is_cuda and t.is_contiguous()
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        self._check(self.L.murmur_decode_step_host(self.h, ids.ctypes.data, len(ids), k_new.data_ptr(),
+                                                   v_new.data_ptr(), q.data_ptr(), out.data_ptr(),
+                                                   C.c_float(sm_scale), _stream()))
+
+    # ---- introspection ------------------------------------------------------------------
+    def seq_state(self, seq: int) -> dict:
+        a = np.zeros(6, dtype=np.int32)
+        self._check(self.L.murmur_seq_get_state(self.h, seq, a.ctypes.data, _stream()))
+        return dict(zip(("length", "t", "n_live", "n_runs", "n_tiles", "n_retained"), (int(x) for x in a)))
+
+    def retained(self, seq: int) -> np.ndarray:
+        cap = self.max_blocks * self.page_size
+        a = np.zeros(cap, dtype=np.int32)
+        n = C.c_int32(0)
+        self._check(self.L.murmur_kv_get_retained(self.h, seq, a.ctypes.data, cap, C.byref(n), _stream()))
+        return a[: n.value].copy()
+
+    def page_list(self, seq: int) -> Tuple[np.ndarray, np.ndarray]:
+        pages = np.zeros(self.max_blocks, dtype=np.int32)
+        blocks = np.zeros(self.max_blocks, dtype=np.int32)
+        n = C.c_int32(0)
+        self._check(self.L.murmur_kv_get_page_list(self.h, seq, pages.ctypes.data, blocks.ctypes.data,
+                                                   self.max_blocks, C.byref(n), _stream()))
+        return pages[: n.value].copy(), blocks[: n.value].copy()
+
+    def runs(self, seq: int):
+        a = np.zeros(18, dtype=np.int32)
+        n = C.c_int32(0)
+        self._check(self.L.murmur_kv_get_runs(self.h, seq, a.ctypes.data, 6, C.byref(n), _stream()))
+        return [tuple(int(x) for x in a[3 * r: 3 * r + 3]) for r in range(n.value)]
+
+    def free_stack(self) -> np.ndarray:
+        a = np.zeros(self.n_pages, dtype=np.int32)
+        n = C.c_int64(0)
+        self._check(self.L.murmur_kv_get_free_stack(self.h, a.ctypes.data, self.n_pages, C.byref(n), _stream()))
+        return a[: n.value].copy()
+
+    def gather(self, seq: int, positions, layer_begin: int = 0, layer_end: Optional[int] = None):
+        layer_end = self.n_layers if layer_end is None else layer_end
+        pos = _ids(positions)
+        shape = (layer_end - layer_begin, len(pos), self.n_kv, self.d)
+        k = torch.empty(shape, dtype=torch.bfloat16, device=self.device)
+        v = torch.empty(shape, dtype=torch.bfloat16, device=self.device)
+        self._check(self.L.murmur_kv_gather(self.h, seq, pos.ctypes.data, len(pos), layer_begin, layer_end,
+                                            k.data_ptr(), v.data_ptr(), _stream()))
+        return k, v
+
+    def last_error(self) -> int:
+        e = C.c_int32(0)
+        self._check(self.L.murmur_get_last_error(self.h, C.byref(e), _stream()))
+        return e.value
+
+    def set_option(self, option: int, value: int):
+        self._check(self.L.murmur_set_option(self.h, option, value))
+
+    def stats(self) -> dict:
+        s = Stats()
+        self._check(self.L.murmur_get_stats(self.h, C.byref(s)))
+        return {f: getattr(s, f) for f, _ in Stats._fields_}
+
+    def reset_stats(self):
+        self._check(self.L.murmur_reset_stats(self.h))
+
+
+def version() -> str:
+    return lib().murmur_version().decode()

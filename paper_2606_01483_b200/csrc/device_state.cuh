@@ -1,0 +1,117 @@
+// Device-resident state of a murmur cache and the by-value view handed to every kernel.
+//
+// HBM layout:
+//   K pool, V pool : [layer][page][kv_head][slot][128] bf16 - a (layer, page, head) chunk is
+//                    page_size * 256 contiguous bytes.  Inside a 256-byte row the sixteen 16-byte
+//                    chunks are stored XOR-swizzled by (slot & 7): logical chunk c of slot s sits
+//                    at chunk position c ^ (s & 7).  A 1-D bulk copy of any slot range therefore
+//                    lands in shared memory already laid out for conflict-free ldmatrix.
+//   workspace      : SeqDev[max_seqs] | block_table | live_pages | live_blocks | tiles |
+//                    free_stack | ctrl words | item counters | split-K partials | staging
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "policy_math.cuh"
+
+namespace murmur {
+
+constexpr int kHeadDim = 128;
+constexpr int kRowBytes = kHeadDim * 2;  // one K or V row of one head
+constexpr int kTileRows = 64;            // rows of one attention tile (tokens)
+constexpr int kMaxGroup = 8;             // query heads per KV head, padded to the MMA N = 8
+constexpr int kMaxRuns = 6;
+constexpr int kMaxSeqsPerLaunch = 128;
+constexpr int kOStride = 132;            // floats per head row in split-K partials / merge scratch
+constexpr int kPartialFloats = kMaxGroup * kOStride + 2 * kMaxGroup;  // o[8][132] + m[8] + l[8]
+constexpr int kMaxAttnGrid = 1024;       // upper bound on CTAs of the persistent attention kernel
+
+// ctrl word indices
+enum { kCtrlFreeTop = 0, kCtrlError = 1, kCtrlAppendTicket = 2, kCtrlWords = 8 };
+
+struct SeqDev {  // 128 bytes
+  int32_t P, S, M, len;
+  int32_t w_s, d, k_s, w_o, k_o;
+  int32_t active;
+  int32_t n_live;      // live (allocated) blocks after the last evict
+  int32_t n_runs;      // maximal intervals of the retained set
+  int32_t n_tiles;     // attention tiles (tensor-core path)
+  int32_t n_retained;  // |A(t)|
+  int32_t runs[kMaxRuns][3];  // first_pos, n_tok, index of first block in live list
+};
+static_assert(sizeof(SeqDev) == 128, "SeqDev must be 128 bytes");
+
+struct __align__(16) TileDesc {  // 32 bytes: one <= 64-row tile of one run, same for all layers/heads
+  int32_t page[4];     // physical pages of the tile, in order (unused = -1)
+  int32_t row_begin;   // first valid row of the tile buffer (= first slot in page[0])
+  int32_t row_end;     // one past the last valid row (rows are page j * p + slot)
+  int32_t n_pages;
+  int32_t first_pos;   // absolute position of row_begin (debug / profiler use)
+};
+static_assert(sizeof(TileDesc) == 32, "TileDesc must be 32 bytes");
+
+struct CacheView {
+  int32_t n_layers, n_q, n_kv, p, p_log2, max_seqs, max_blocks, group;
+  int64_t n_pages;
+  uint16_t* k_pool;
+  uint16_t* v_pool;
+  SeqDev* seqs;
+  int32_t* block_table;  // [max_seqs][max_blocks] logical block -> page / -1
+  int32_t* live_pages;   // [max_seqs][max_blocks]
+  int32_t* live_blocks;  // [max_seqs][max_blocks]
+  TileDesc* tiles;       // [max_seqs][max_blocks]
+  int32_t* free_stack;   // [n_pages]
+  int32_t* ctrl;         // [kCtrlWords]
+  int32_t* item_counters;  // [n_layers][max_seqs][n_kv] split-K arrival counters (self-resetting)
+  float* partials;       // [2 * kMaxAttnGrid][kPartialFloats]
+};
+
+struct SeqList {  // per-launch sequence list, passed by value (no H2D copy, graph-capturable)
+  int32_t n;
+  int32_t ids[kMaxSeqsPerLaunch];
+};
+
+struct AppendList {
+  int32_t n;
+  int32_t ids[kMaxSeqsPerLaunch];
+  int32_t n_tok[kMaxSeqsPerLaunch];
+};
+
+// Byte offset of row (layer, page, head, slot) in a pool.
+__host__ __device__ __forceinline__ size_t row_offset(const CacheView& c, int layer, int page, int head, int slot) {
+  return ((((size_t)layer * (size_t)c.n_pages + (size_t)page) * c.n_kv + head) * c.p + slot) * (size_t)kRowBytes;
+}
+
+__device__ __forceinline__ SeqParams load_params(const SeqDev& s) {
+  SeqParams r;
+  r.P = s.P; r.S = s.S; r.M = s.M; r.len = s.len;
+  r.w_s = s.w_s; r.d = s.d; r.k_s = s.k_s; r.w_o = s.w_o; r.k_o = s.k_o;
+  return r;
+}
+
+// ---- host launchers (one per .cu) ------------------------------------------------------------
+struct LaunchInfo {
+  int launches;   // kernels launched
+  int grid;       // CTAs of the main kernel
+  int smem;       // dynamic smem of the main kernel
+};
+
+cudaError_t launch_init(const CacheView& c, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_seq_begin(const CacheView& c, int seq, const SeqParams& sp, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_seq_end(const CacheView& c, int seq, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_append(const CacheView& c, const AppendList& list, int total_tokens, const void* k_new,
+                          const void* v_new, int layer_begin, int layer_end, bool reserve, int sm_count,
+                          cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_evict(const CacheView& c, const SeqList& list, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_attn_generic(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total,
+                                const void* q, void* out, float* lse, int layer_begin, int layer_end,
+                                float sm_scale, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
+                            void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
+                            cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_expand_retained(const CacheView& c, int seq, int32_t* pos_out_dev, int cap, cudaStream_t st,
+                                   LaunchInfo* info);
+cudaError_t launch_gather(const CacheView& c, int seq, const int32_t* positions_dev, int n, int layer_begin,
+                          int layer_end, void* k_out, void* v_out, cudaStream_t st, LaunchInfo* info);
+
+}  // namespace murmur

@@ -1,0 +1,581 @@
+// Host side of the C ABI (include/murmur.h): handle, workspace carve-up, argument validation
+// against a host mirror of the integer state, kernel dispatch, introspection.
+//
+// The mirror holds, per sequence, only (regions, policy, length, length at the last evict, blocks
+// freed so far); with the closed form in policy_math.cuh that is enough to know the free-page
+// count exactly, so page exhaustion is reported synchronously and all-or-nothing without ever
+// reading device memory.  Every state transition itself runs in the kernels.
+#include <cuda_runtime.h>
+
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/murmur.h"
+#include "device_state.cuh"
+
+using namespace murmur;
+
+namespace {
+
+struct HostSeq {
+  bool active = false;
+  SeqParams sp{};
+  int32_t evict_len = -1;   // length when murmur_kv_evict last ran (-1: never)
+  int32_t freed_blocks = 0;  // blocks of this sequence returned to the pool so far
+};
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct Carve {
+  size_t seqs, block_table, live_pages, live_blocks, tiles, free_stack, ctrl, counters, partials;
+  size_t stage_k, stage_v, stage_q, stage_out, scratch;
+  size_t total;
+  int stage_seqs;
+  size_t scratch_ints;
+};
+
+bool geometry_ok(const murmur_cache_desc_t* d) {
+  if (!d) return false;
+  if (d->head_dim != kHeadDim) return false;
+  if (d->n_layers < 1 || d->n_kv_heads < 1 || d->n_q_heads < 1) return false;
+  if (d->n_q_heads % d->n_kv_heads) return false;
+  if (d->n_q_heads / d->n_kv_heads > kMaxGroup) return false;
+  if (d->page_size < 1 || d->page_size > kTileRows || (d->page_size & (d->page_size - 1))) return false;
+  if (d->max_seqs < 1 || d->max_blocks_per_seq < 1 || d->n_pages < 1) return false;
+  if (d->n_pages > 0x7fffffffLL) return false;
+  if ((int64_t)d->max_blocks_per_seq * d->page_size > 0x7fffffffLL) return false;
+  return true;
+}
+
+Carve carve(const murmur_cache_desc_t* d) {
+  Carve c{};
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    const size_t at = off;
+    off = align_up(off + bytes);
+    return at;
+  };
+  const size_t tab = (size_t)d->max_seqs * d->max_blocks_per_seq;
+  c.seqs = take((size_t)d->max_seqs * sizeof(SeqDev));
+  c.block_table = take(tab * 4);
+  c.live_pages = take(tab * 4);
+  c.live_blocks = take(tab * 4);
+  c.tiles = take(tab * sizeof(TileDesc));
+  c.free_stack = take((size_t)d->n_pages * 4);
+  c.ctrl = take(kCtrlWords * 4);
+  c.counters = take((size_t)d->n_layers * kMaxSeqsPerLaunch * d->n_kv_heads * 4);
+  c.partials = take((size_t)2 * kMaxAttnGrid * kPartialFloats * 4);
+  c.stage_seqs = d->max_seqs < kMaxSeqsPerLaunch ? d->max_seqs : kMaxSeqsPerLaunch;
+  const size_t kv_b = (size_t)d->n_layers * c.stage_seqs * d->n_kv_heads * kRowBytes;
+  const size_t q_b = (size_t)d->n_layers * c.stage_seqs * d->n_q_heads * kRowBytes;
+  c.stage_k = take(kv_b);
+  c.stage_v = take(kv_b);
+  c.stage_q = take(q_b);
+  c.stage_out = take(q_b);
+  c.scratch_ints = (size_t)d->max_blocks_per_seq * d->page_size;
+  c.scratch = take(c.scratch_ints * 4);
+  c.total = off;
+  return c;
+}
+
+}  // namespace
+
+struct murmur_cache {
+  murmur_cache_desc_t desc;
+  CacheView view;
+  Carve cv;
+  std::vector<HostSeq> seqs;
+  int64_t free_pages;
+  int sm_count;
+  int attn_variant_opt;
+  int attn_grid_opt;
+  murmur_stats_t stats;
+  cudaError_t last_cuda;
+  uint8_t* ws;
+};
+
+namespace {
+
+murmur_status_t cuda_fail(murmur_cache* c, cudaError_t e) {
+  c->last_cuda = e;
+  return MURMUR_ERR_CUDA;
+}
+
+#define MM_CUDA(c, expr)                                  \
+  do {                                                    \
+    cudaError_t e__ = (expr);                             \
+    if (e__ != cudaSuccess) return cuda_fail((c), e__);   \
+  } while (0)
+
+void note(murmur_cache* c, const LaunchInfo& li) { c->stats.kernel_launches += li.launches; }
+
+inline int32_t blocks_for(int32_t len, int32_t p) { return (len + p - 1) / p; }
+
+// ids in range, active, distinct
+murmur_status_t check_ids(murmur_cache* c, const int32_t* ids, int32_t n) {
+  if (!ids || n < 0) return MURMUR_ERR_INVALID_ARG;
+  for (int i = 0; i < n; ++i) {
+    if (ids[i] < 0 || ids[i] >= c->desc.max_seqs) return MURMUR_ERR_INVALID_ARG;
+    for (int j = 0; j < i; ++j)
+      if (ids[j] == ids[i]) return MURMUR_ERR_INVALID_ARG;
+  }
+  for (int i = 0; i < n; ++i)
+    if (!c->seqs[ids[i]].active) return MURMUR_ERR_STATE;
+  return MURMUR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t murmur_pool_bytes(const murmur_cache_desc_t* d) {
+  if (!geometry_ok(d)) return 0;
+  return (size_t)d->n_layers * (size_t)d->n_pages * d->n_kv_heads * d->page_size * kRowBytes;
+}
+
+size_t murmur_workspace_bytes(const murmur_cache_desc_t* d) {
+  if (!geometry_ok(d)) return 0;
+  return carve(d).total;
+}
+
+murmur_status_t murmur_cache_create(const murmur_cache_desc_t* d, murmur_cache_t** out, void* stream) {
+  if (!d || !out) return MURMUR_ERR_INVALID_ARG;
+  if (!geometry_ok(d)) return MURMUR_ERR_UNSUPPORTED;
+  if (!d->k_pool || !d->v_pool || !d->workspace) return MURMUR_ERR_INVALID_ARG;
+  if (((uintptr_t)d->k_pool | (uintptr_t)d->v_pool | (uintptr_t)d->workspace) & (kAlign - 1)) return MURMUR_ERR_INVALID_ARG;
+  const Carve cv = carve(d);
+  if (d->workspace_bytes < cv.total) return MURMUR_ERR_INVALID_ARG;
+  murmur_cache* c = new (std::nothrow) murmur_cache();
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  c->desc = *d;
+  c->cv = cv;
+  c->ws = reinterpret_cast<uint8_t*>(d->workspace);
+  c->seqs.assign(d->max_seqs, HostSeq());
+  c->free_pages = d->n_pages;
+  c->attn_variant_opt = MURMUR_ATTN_AUTO;
+  c->attn_grid_opt = 0;
+  std::memset(&c->stats, 0, sizeof c->stats);
+  c->last_cuda = cudaSuccess;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) {
+    delete c;
+    return MURMUR_ERR_CUDA;
+  }
+  CacheView& v = c->view;
+  v.n_layers = d->n_layers; v.n_q = d->n_q_heads; v.n_kv = d->n_kv_heads;
+  v.p = d->page_size;
+  v.p_log2 = 0;
+  while ((1 << v.p_log2) < d->page_size) ++v.p_log2;
+  v.max_seqs = d->max_seqs; v.max_blocks = d->max_blocks_per_seq;
+  v.group = d->n_q_heads / d->n_kv_heads;
+  v.n_pages = d->n_pages;
+  v.k_pool = reinterpret_cast<uint16_t*>(d->k_pool);
+  v.v_pool = reinterpret_cast<uint16_t*>(d->v_pool);
+  v.seqs = reinterpret_cast<SeqDev*>(c->ws + cv.seqs);
+  v.block_table = reinterpret_cast<int32_t*>(c->ws + cv.block_table);
+  v.live_pages = reinterpret_cast<int32_t*>(c->ws + cv.live_pages);
+  v.live_blocks = reinterpret_cast<int32_t*>(c->ws + cv.live_blocks);
+  v.tiles = reinterpret_cast<TileDesc*>(c->ws + cv.tiles);
+  v.free_stack = reinterpret_cast<int32_t*>(c->ws + cv.free_stack);
+  v.ctrl = reinterpret_cast<int32_t*>(c->ws + cv.ctrl);
+  v.item_counters = reinterpret_cast<int32_t*>(c->ws + cv.counters);
+  v.partials = reinterpret_cast<float*>(c->ws + cv.partials);
+  LaunchInfo li{};
+  e = launch_init(v, (cudaStream_t)stream, &li);
+  if (e != cudaSuccess) {
+    delete c;
+    return MURMUR_ERR_CUDA;
+  }
+  note(c, li);
+  c->stats.sm_count = c->sm_count;
+  c->stats.free_pages = c->free_pages;
+  *out = c;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_cache_destroy(murmur_cache_t* c) {
+  delete c;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_seq_begin(murmur_cache_t* c, int32_t seq, int32_t n_prefix, int32_t n_speech, int32_t n_mid,
+                                 const murmur_policy_t* pol, void* stream) {
+  if (!c || !pol) return MURMUR_ERR_INVALID_ARG;
+  if (seq < 0 || seq >= c->desc.max_seqs) return MURMUR_ERR_INVALID_ARG;
+  if (n_prefix < 0 || n_speech < 0 || n_mid < 0) return MURMUR_ERR_INVALID_ARG;
+  if (pol->w_speech < 0 || pol->delay < 0 || pol->n_sink_speech < 0 || pol->w_out < 0 || pol->n_sink_out < 0)
+    return MURMUR_ERR_INVALID_ARG;
+  if ((int64_t)n_prefix + n_speech + n_mid > (int64_t)c->desc.max_blocks_per_seq * c->desc.page_size)
+    return MURMUR_ERR_INVALID_ARG;
+  HostSeq& hs = c->seqs[seq];
+  if (hs.active) return MURMUR_ERR_STATE;
+  SeqParams sp{};
+  sp.P = n_prefix; sp.S = n_speech; sp.M = n_mid; sp.len = 0;
+  sp.w_s = pol->w_speech; sp.d = pol->delay; sp.k_s = pol->n_sink_speech;
+  sp.w_o = pol->w_out; sp.k_o = pol->n_sink_out;
+  LaunchInfo li{};
+  MM_CUDA(c, launch_seq_begin(c->view, seq, sp, (cudaStream_t)stream, &li));
+  note(c, li);
+  hs = HostSeq();
+  hs.active = true;
+  hs.sp = sp;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_seq_end(murmur_cache_t* c, int32_t seq, void* stream) {
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  if (seq < 0 || seq >= c->desc.max_seqs) return MURMUR_ERR_INVALID_ARG;
+  HostSeq& hs = c->seqs[seq];
+  if (!hs.active) return MURMUR_ERR_STATE;
+  LaunchInfo li{};
+  MM_CUDA(c, launch_seq_end(c->view, seq, (cudaStream_t)stream, &li));
+  note(c, li);
+  c->free_pages += blocks_for(hs.sp.len, c->desc.page_size) - hs.freed_blocks;
+  c->stats.free_pages = c->free_pages;
+  hs = HostSeq();
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_append(murmur_cache_t* c, const int32_t* seq_ids, const int32_t* n_tokens, int32_t n_seqs,
+                                 const void* k_new, const void* v_new, int32_t layer_begin, int32_t layer_end,
+                                 void* stream) {
+  if (!c || !n_tokens) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs);
+  if (st != MURMUR_OK) return st;
+  if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
+  const bool reserve = (layer_begin == 0);
+  const int32_t p = c->desc.page_size;
+  int64_t total = 0, need = 0;
+  for (int i = 0; i < n_seqs; ++i) {
+    if (n_tokens[i] < 0) return MURMUR_ERR_INVALID_ARG;
+    const HostSeq& hs = c->seqs[seq_ids[i]];
+    total += n_tokens[i];
+    if (reserve) {
+      const int64_t new_len = (int64_t)hs.sp.len + n_tokens[i];
+      if (new_len > (int64_t)c->desc.max_blocks_per_seq * p) return MURMUR_ERR_STATE;
+      need += blocks_for((int32_t)new_len, p) - blocks_for(hs.sp.len, p);
+    } else if (n_tokens[i] > hs.sp.len) {
+      return MURMUR_ERR_STATE;  // rows for positions that were never reserved
+    }
+  }
+  if (total > 0x7fffffffLL) return MURMUR_ERR_INVALID_ARG;
+  if (total > 0 && (!k_new || !v_new)) return MURMUR_ERR_INVALID_ARG;
+  if (reserve && need > c->free_pages) return MURMUR_ERR_OOM_PAGES;  // all-or-nothing
+  if (n_seqs == 0 || total == 0) return MURMUR_OK;
+
+  // split into launches of <= 128 sequences, in call order
+  const size_t row_tok = (size_t)c->desc.n_kv_heads * kRowBytes;
+  int64_t tok_done = 0;
+  for (int base = 0; base < n_seqs; base += kMaxSeqsPerLaunch) {
+    AppendList list;
+    list.n = (n_seqs - base) < kMaxSeqsPerLaunch ? (n_seqs - base) : kMaxSeqsPerLaunch;
+    int64_t chunk_tok = 0;
+    for (int i = 0; i < list.n; ++i) {
+      list.ids[i] = seq_ids[base + i];
+      list.n_tok[i] = n_tokens[base + i];
+      chunk_tok += n_tokens[base + i];
+    }
+    if (chunk_tok > 0) {
+      if (base == 0 && list.n == n_seqs) {
+        LaunchInfo li{};
+        MM_CUDA(c, launch_append(c->view, list, (int)chunk_tok, k_new, v_new, layer_begin, layer_end, reserve,
+                                 c->sm_count, (cudaStream_t)stream, &li));
+        note(c, li);
+      } else {
+        // several chunks: the source is [layer][all tokens][...], so each layer is its own launch
+        for (int layer = layer_begin; layer < layer_end; ++layer) {
+          const size_t off = ((size_t)(layer - layer_begin) * (size_t)total + (size_t)tok_done) * row_tok;
+          LaunchInfo li{};
+          MM_CUDA(c, launch_append(c->view, list, (int)chunk_tok, (const uint8_t*)k_new + off,
+                                   (const uint8_t*)v_new + off, layer, layer + 1,
+                                   reserve && layer == layer_begin, c->sm_count, (cudaStream_t)stream, &li));
+          note(c, li);
+        }
+      }
+    }
+    tok_done += chunk_tok;
+  }
+  if (reserve) {
+    for (int i = 0; i < n_seqs; ++i) c->seqs[seq_ids[i]].sp.len += n_tokens[i];
+    c->free_pages -= need;
+    c->stats.free_pages = c->free_pages;
+  }
+  c->stats.append_calls += 1;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_evict(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, void* stream) {
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs);
+  if (st != MURMUR_OK) return st;
+  for (int base = 0; base < n_seqs; base += kMaxSeqsPerLaunch) {
+    SeqList list;
+    list.n = (n_seqs - base) < kMaxSeqsPerLaunch ? (n_seqs - base) : kMaxSeqsPerLaunch;
+    for (int i = 0; i < list.n; ++i) list.ids[i] = seq_ids[base + i];
+    LaunchInfo li{};
+    MM_CUDA(c, launch_evict(c->view, list, (cudaStream_t)stream, &li));
+    note(c, li);
+  }
+  for (int i = 0; i < n_seqs; ++i) {
+    HostSeq& hs = c->seqs[seq_ids[i]];
+    const int32_t dead = dead_block_count(hs.sp, c->desc.page_size);
+    c->free_pages += dead - hs.freed_blocks;
+    hs.freed_blocks = dead;
+    hs.evict_len = hs.sp.len;
+  }
+  c->stats.free_pages = c->free_pages;
+  c->stats.evict_calls += 1;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q, void* out,
+                                   float* lse, int32_t layer_begin, int32_t layer_end, float sm_scale, void* stream) {
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs);
+  if (st != MURMUR_OK) return st;
+  if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
+  if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
+  if (n_seqs == 0) return MURMUR_OK;
+  if (!q || !out) return MURMUR_ERR_INVALID_ARG;
+  for (int i = 0; i < n_seqs; ++i) {
+    const HostSeq& hs = c->seqs[seq_ids[i]];
+    if (hs.sp.len < 1 || hs.evict_len != hs.sp.len) return MURMUR_ERR_STATE;
+    if (retained_count(hs.sp) < 1) return MURMUR_ERR_STATE;  // Eq. 1 over an empty set is undefined
+  }
+  int variant = c->attn_variant_opt;
+  if (variant == MURMUR_ATTN_AUTO) variant = (c->desc.page_size >= 16) ? MURMUR_ATTN_MMA : MURMUR_ATTN_GENERIC;
+  if (variant == MURMUR_ATTN_MMA && c->desc.page_size < 16) return MURMUR_ERR_UNSUPPORTED;
+  const int grid = c->attn_grid_opt > 0 ? c->attn_grid_opt : c->sm_count;
+  for (int base = 0; base < n_seqs; base += kMaxSeqsPerLaunch) {
+    SeqList list;
+    list.n = (n_seqs - base) < kMaxSeqsPerLaunch ? (n_seqs - base) : kMaxSeqsPerLaunch;
+    for (int i = 0; i < list.n; ++i) list.ids[i] = seq_ids[base + i];
+    LaunchInfo li{};
+    if (variant == MURMUR_ATTN_MMA) {
+      MM_CUDA(c, launch_attn_mma(c->view, list, base, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, grid,
+                                 (cudaStream_t)stream, &li));
+    } else {
+      MM_CUDA(c, launch_attn_generic(c->view, list, base, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale,
+                                     (cudaStream_t)stream, &li));
+    }
+    note(c, li);
+    c->stats.attn_grid = li.grid;
+    c->stats.attn_smem_bytes = li.smem;
+  }
+  c->stats.attn_variant = variant;
+  c->stats.attn_calls += 1;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs,
+                                        const void* k_new_host, const void* v_new_host, const void* q_host,
+                                        void* out_host, float sm_scale, void* stream) {
+  if (!c || !k_new_host || !v_new_host || !q_host || !out_host) return MURMUR_ERR_INVALID_ARG;
+  if (n_seqs < 1 || n_seqs > c->cv.stage_seqs) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs);
+  if (st != MURMUR_OK) return st;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t kv_b = (size_t)c->desc.n_layers * n_seqs * c->desc.n_kv_heads * kRowBytes;
+  const size_t q_b = (size_t)c->desc.n_layers * n_seqs * c->desc.n_q_heads * kRowBytes;
+  uint8_t* dk = c->ws + c->cv.stage_k;
+  uint8_t* dv = c->ws + c->cv.stage_v;
+  uint8_t* dq = c->ws + c->cv.stage_q;
+  uint8_t* dout = c->ws + c->cv.stage_out;
+  // validate the append before any copy so that a failing call leaves everything untouched
+  int32_t ones[kMaxSeqsPerLaunch];
+  int64_t need = 0;
+  for (int i = 0; i < n_seqs; ++i) {
+    ones[i] = 1;
+    const HostSeq& hs = c->seqs[seq_ids[i]];
+    if ((int64_t)hs.sp.len + 1 > (int64_t)c->desc.max_blocks_per_seq * c->desc.page_size) return MURMUR_ERR_STATE;
+    need += blocks_for(hs.sp.len + 1, c->desc.page_size) - blocks_for(hs.sp.len, c->desc.page_size);
+  }
+  if (need > c->free_pages) return MURMUR_ERR_OOM_PAGES;
+  MM_CUDA(c, cudaMemcpyAsync(dk, k_new_host, kv_b, cudaMemcpyHostToDevice, s));
+  MM_CUDA(c, cudaMemcpyAsync(dv, v_new_host, kv_b, cudaMemcpyHostToDevice, s));
+  MM_CUDA(c, cudaMemcpyAsync(dq, q_host, q_b, cudaMemcpyHostToDevice, s));
+  st = murmur_kv_append(c, seq_ids, ones, n_seqs, dk, dv, 0, c->desc.n_layers, stream);
+  if (st != MURMUR_OK) return st;
+  st = murmur_kv_evict(c, seq_ids, n_seqs, stream);
+  if (st != MURMUR_OK) return st;
+  st = murmur_decode_attn(c, seq_ids, n_seqs, dq, dout, nullptr, 0, c->desc.n_layers, sm_scale, stream);
+  if (st != MURMUR_OK) return st;
+  MM_CUDA(c, cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, s));
+  return MURMUR_OK;
+}
+
+// ---- introspection ------------------------------------------------------------------------------
+static murmur_status_t check_seq(murmur_cache_t* c, int32_t seq) {
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  if (seq < 0 || seq >= c->desc.max_seqs) return MURMUR_ERR_INVALID_ARG;
+  if (!c->seqs[seq].active) return MURMUR_ERR_STATE;
+  return MURMUR_OK;
+}
+
+static murmur_status_t read_seqdev(murmur_cache_t* c, int32_t seq, SeqDev* sd, cudaStream_t s) {
+  MM_CUDA(c, cudaStreamSynchronize(s));
+  MM_CUDA(c, cudaMemcpy(sd, c->view.seqs + seq, sizeof(SeqDev), cudaMemcpyDeviceToHost));
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_seq_get_state(murmur_cache_t* c, int32_t seq, int32_t* state_out, void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!state_out) return MURMUR_ERR_INVALID_ARG;
+  SeqDev sd;
+  st = read_seqdev(c, seq, &sd, (cudaStream_t)stream);
+  if (st != MURMUR_OK) return st;
+  state_out[0] = sd.len;
+  state_out[1] = sd.len - (sd.P + sd.S + sd.M) > 0 ? sd.len - (sd.P + sd.S + sd.M) : 0;
+  state_out[2] = sd.n_live;
+  state_out[3] = sd.n_runs;
+  state_out[4] = sd.n_tiles;
+  state_out[5] = sd.n_retained;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_get_retained(murmur_cache_t* c, int32_t seq, int32_t* pos_out, int32_t cap, int32_t* n_out,
+                                       void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!n_out || cap < 0 || (cap > 0 && !pos_out)) return MURMUR_ERR_INVALID_ARG;
+  SeqDev sd;
+  st = read_seqdev(c, seq, &sd, (cudaStream_t)stream);
+  if (st != MURMUR_OK) return st;
+  *n_out = sd.n_retained;
+  if (sd.n_retained > cap) return MURMUR_ERR_INVALID_ARG;
+  if (sd.n_retained == 0) return MURMUR_OK;
+  if ((size_t)sd.n_retained > c->cv.scratch_ints) return MURMUR_ERR_STATE;
+  int32_t* scratch = reinterpret_cast<int32_t*>(c->ws + c->cv.scratch);
+  LaunchInfo li{};
+  MM_CUDA(c, launch_expand_retained(c->view, seq, scratch, (int)c->cv.scratch_ints, (cudaStream_t)stream, &li));
+  note(c, li);
+  MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  MM_CUDA(c, cudaMemcpy(pos_out, scratch, (size_t)sd.n_retained * 4, cudaMemcpyDeviceToHost));
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_get_page_list(murmur_cache_t* c, int32_t seq, int32_t* pages_out, int32_t* blocks_out,
+                                        int32_t cap, int32_t* n_out, void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!n_out || cap < 0) return MURMUR_ERR_INVALID_ARG;
+  SeqDev sd;
+  st = read_seqdev(c, seq, &sd, (cudaStream_t)stream);
+  if (st != MURMUR_OK) return st;
+  *n_out = sd.n_live;
+  if (sd.n_live > cap) return MURMUR_ERR_INVALID_ARG;
+  const size_t off = (size_t)seq * c->desc.max_blocks_per_seq;
+  if (pages_out && sd.n_live)
+    MM_CUDA(c, cudaMemcpy(pages_out, c->view.live_pages + off, (size_t)sd.n_live * 4, cudaMemcpyDeviceToHost));
+  if (blocks_out && sd.n_live)
+    MM_CUDA(c, cudaMemcpy(blocks_out, c->view.live_blocks + off, (size_t)sd.n_live * 4, cudaMemcpyDeviceToHost));
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_get_runs(murmur_cache_t* c, int32_t seq, int32_t* runs_out, int32_t cap_runs, int32_t* n_out,
+                                   void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!n_out || !runs_out) return MURMUR_ERR_INVALID_ARG;
+  SeqDev sd;
+  st = read_seqdev(c, seq, &sd, (cudaStream_t)stream);
+  if (st != MURMUR_OK) return st;
+  *n_out = sd.n_runs;
+  if (sd.n_runs > cap_runs) return MURMUR_ERR_INVALID_ARG;
+  for (int r = 0; r < sd.n_runs; ++r)
+    for (int k = 0; k < 3; ++k) runs_out[3 * r + k] = sd.runs[r][k];
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_get_free_stack(murmur_cache_t* c, int32_t* pages_out, int64_t cap, int64_t* n_out,
+                                         void* stream) {
+  if (!c || !n_out) return MURMUR_ERR_INVALID_ARG;
+  MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  int32_t top = 0;
+  MM_CUDA(c, cudaMemcpy(&top, c->view.ctrl + kCtrlFreeTop, 4, cudaMemcpyDeviceToHost));
+  *n_out = top;
+  if (top > cap) return MURMUR_ERR_INVALID_ARG;
+  if (pages_out && top > 0)
+    MM_CUDA(c, cudaMemcpy(pages_out, c->view.free_stack, (size_t)top * 4, cudaMemcpyDeviceToHost));
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_gather(murmur_cache_t* c, int32_t seq, const int32_t* positions, int32_t n,
+                                 int32_t layer_begin, int32_t layer_end, void* k_out, void* v_out, void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!positions || n < 0 || !k_out || !v_out) return MURMUR_ERR_INVALID_ARG;
+  if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
+  if ((size_t)n > c->cv.scratch_ints) return MURMUR_ERR_INVALID_ARG;
+  for (int i = 0; i < n; ++i)
+    if (positions[i] < 0 || positions[i] >= c->seqs[seq].sp.len) return MURMUR_ERR_INVALID_ARG;
+  if (n == 0) return MURMUR_OK;
+  int32_t* scratch = reinterpret_cast<int32_t*>(c->ws + c->cv.scratch);
+  cudaStream_t s = (cudaStream_t)stream;
+  MM_CUDA(c, cudaStreamSynchronize(s));
+  MM_CUDA(c, cudaMemcpy(scratch, positions, (size_t)n * 4, cudaMemcpyHostToDevice));
+  LaunchInfo li{};
+  MM_CUDA(c, launch_gather(c->view, seq, scratch, n, layer_begin, layer_end, k_out, v_out, s, &li));
+  note(c, li);
+  MM_CUDA(c, cudaStreamSynchronize(s));
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_get_last_error(murmur_cache_t* c, int32_t* device_err_out, void* stream) {
+  if (!c || !device_err_out) return MURMUR_ERR_INVALID_ARG;
+  MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  MM_CUDA(c, cudaMemcpy(device_err_out, c->view.ctrl + kCtrlError, 4, cudaMemcpyDeviceToHost));
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_set_option(murmur_cache_t* c, int32_t option, int32_t value) {
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  switch (option) {
+    case MURMUR_OPT_ATTN_VARIANT:
+      if (value < MURMUR_ATTN_AUTO || value > MURMUR_ATTN_MMA) return MURMUR_ERR_INVALID_ARG;
+      c->attn_variant_opt = value;
+      return MURMUR_OK;
+    case MURMUR_OPT_ATTN_GRID:
+      if (value < 0 || value > kMaxAttnGrid) return MURMUR_ERR_INVALID_ARG;
+      c->attn_grid_opt = value;
+      return MURMUR_OK;
+    default:
+      return MURMUR_ERR_INVALID_ARG;
+  }
+}
+
+murmur_status_t murmur_get_stats(murmur_cache_t* c, murmur_stats_t* out) {
+  if (!c || !out) return MURMUR_ERR_INVALID_ARG;
+  *out = c->stats;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_reset_stats(murmur_cache_t* c) {
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  c->stats.kernel_launches = 0;
+  c->stats.append_calls = c->stats.evict_calls = c->stats.attn_calls = 0;
+  return MURMUR_OK;
+}
+
+const char* murmur_last_cuda_error(murmur_cache_t* c) { return c ? cudaGetErrorString(c->last_cuda) : "null handle"; }
+
+const char* murmur_status_str(murmur_status_t s) {
+  switch (s) {
+    case MURMUR_OK: return "MURMUR_OK";
+    case MURMUR_ERR_INVALID_ARG: return "MURMUR_ERR_INVALID_ARG";
+    case MURMUR_ERR_STATE: return "MURMUR_ERR_STATE";
+    case MURMUR_ERR_OOM_PAGES: return "MURMUR_ERR_OOM_PAGES";
+    case MURMUR_ERR_CUDA: return "MURMUR_ERR_CUDA";
+    case MURMUR_ERR_UNSUPPORTED: return "MURMUR_ERR_UNSUPPORTED";
+  }
+  return "MURMUR_ERR_?";
+}
+
+const char* murmur_version(void) { return "murmur-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,368 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle, on a real GPU.
+
+Integer state (retained sets, compacted page tables, run descriptors, free stack) must be
+bit-exact; attention within max-abs 2e-2 / mean-abs 2e-3 (BASELINE.json north_star).
+Small and reduced-layer cases compare every element; the full-size cases (configs 2, 3, 5 at
+28 layers, in the launch configuration bench.py times) compare all integer state and
+sampled (sequence, layer) attention outputs the oracle computes one by one.
+"""
+import math
+import random
+
+import numpy as np
+import pytest
+import torch
+
+import workloads
+from workloads import Config, Geometry, seq_spec
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return "cuda:0"
+
+
+def _mk(cfg, dev, **kw):
+    from tests.harness import SideBySide
+
+    return SideBySide(cfg, device=dev, **kw)
+
+
+def _variants(page_size):
+    from paper_2606_01483_b200 import MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA
+
+    return [MURMUR_ATTN_GENERIC] + ([MURMUR_ATTN_MMA] if page_size >= 16 else [])
+
+
+# -------------------------------------------------------------------------------- config 1
+@pytest.mark.parametrize("variant_idx", [0, 1])
+def test_config1_every_step_every_head(dev, variant_idx):
+    cfg = workloads.config1()
+    variant = _variants(cfg.page_size)[variant_idx]
+    sbs = _mk(cfg, dev, variant=variant)
+    ids = [0]
+    sbs.bulk_prefill(ids, 128)
+    sbs.check_integer_state(ids)
+    assert sbs.gpu.seq_state(0)["n_retained"] == 64 + 128 + 4 + 64
+    for step in range(32):
+        sbs.append_step(ids)
+        sbs.evict(ids)
+        sbs.check_integer_state(ids)
+        q, out, lse = sbs.attend(ids, want_lse=True)
+        sbs.check_attention(ids, q, out, lse)
+        if step in (0, 15, 31):
+            sbs.check_gather(0)
+    assert sbs.t_of(0) == 160
+    # evict is idempotent
+    before = sbs.gpu.free_stack().tolist()
+    sbs.gpu.kv_evict(ids)
+    assert sbs.gpu.free_stack().tolist() == before
+    sbs.check_integer_state(ids)
+    sbs.close()
+
+
+# -------------------------------------------------------------------------------- worked example
+def test_worked_example_tiny_pages(dev, golden):
+    """SURVEY 8(c) table through the GPU path with p = 4 (generic attention path)."""
+    cfg = Config("worked", 9, Geometry(n_layers=2), 4,
+                 (seq_spec(2, 10, 8, 4, 3, delay=2, n_sink_speech=0, n_sink_out=1),))
+    sbs = _mk(cfg, dev, n_pages=6)
+    sbs.bulk_prefill([0], 0, evict=False)
+    for line in golden("worked_example_hybrid.txt"):
+        t_s, _l, A_s, _ra, blocks_s = [x.strip() for x in line.split("|")]
+        sbs.append_step([0])
+        sbs.evict([0])
+        assert sbs.gpu.seq_state(0)["t"] == int(t_s)
+        assert sbs.gpu.retained(0).tolist() == [int(x) for x in A_s.split()]
+        assert sbs.gpu.page_list(0)[1].tolist() == [int(x) for x in blocks_s.split()]
+        sbs.check_integer_state([0])
+        q, out, lse = sbs.attend([0], want_lse=True)
+        sbs.check_attention([0], q, out, lse)
+    assert sbs.gpu.free_stack().tolist()[-1] == 1
+    assert sbs.gpu.runs(0) == [(0, 2, 0), (8, 5, 1), (17, 3, 3)]
+    sbs.close()
+
+
+# -------------------------------------------------------------------------------- random property cases
+@pytest.mark.parametrize("seed", range(6))
+def test_random_small_cases_stepwise(dev, seed):
+    rng = random.Random(100 + seed)
+    p = rng.choice([1, 2, 4, 8, 16, 32, 64])
+    n_seqs = rng.randint(1, 4)
+    seqs = []
+    for _ in range(n_seqs):
+        S = rng.randint(0, 150)
+        seqs.append(seq_spec(rng.randint(0, 70), S, rng.randint(3, 40), rng.choice([0, 1, 7, 40, 64, 200]),
+                             rng.choice([0, 1, 5, 33, 100]), M=rng.choice([0, 0, 3]),
+                             delay=rng.choice([0, 1, 6, 20]), n_sink_speech=rng.choice([0, 0, 2, 9]),
+                             n_sink_out=rng.choice([0, 1, 4])))
+    cfg = Config(f"rand{seed}", 50 + seed, Geometry(n_layers=2), p, tuple(seqs))
+    for variant in _variants(p):
+        sbs = _mk(cfg, dev, variant=variant)
+        ids = list(range(n_seqs))
+        sbs.bulk_prefill(ids, 0, evict=False)
+        active = list(ids)
+        step = 0
+        while active:
+            sbs.append_step(active)
+            order = active[::-1] if step % 2 else active  # call order defines the free-stack order
+            sbs.evict(order)
+            sbs.check_integer_state(active)
+            # a sequence whose retained set is empty (P = 0, all windows 0) cannot be attended
+            att = [i for i in active if len(sbs.oracle.retained(i)) > 0]
+            if att:
+                q, out, lse = sbs.attend(att, want_lse=True)
+                sbs.check_attention(att, q, out, lse)
+            for i in list(active):
+                if sbs.t_of(i) >= cfg.seqs[i].T:
+                    sbs.gpu.seq_end(i)
+                    sbs.oracle.seq_end(i)
+                    active.remove(i)
+            step += 1
+        assert sbs.gpu.free_stack().tolist() == sbs.oracle.free_stack
+        assert len(sbs.oracle.free_stack) == sbs.oracle.N
+        sbs.close()
+
+
+# -------------------------------------------------------------------------------- config 2, reduced layers
+def test_config2_two_layers_stepwise_around_delay_and_window_edges(dev):
+    cfg = workloads.config2().with_layers(2).with_seqs(workloads.config2().seqs[:5])
+    sbs = _mk(cfg, dev)
+    ids = list(range(cfg.batch))
+    sbs.bulk_prefill(ids, 250)
+    sbs.check_integer_state(ids)
+    for step in range(16):  # t = 251 .. 266 crosses d = 256 and k_o + w_o = 260
+        sbs.append_step(ids)
+        sbs.evict(ids)
+        sbs.check_integer_state(ids)
+        q, out, lse = sbs.attend(ids, want_lse=True)
+        sbs.check_attention(ids, q, out, lse)
+    assert sbs.gpu.seq_state(0)["n_retained"] == 836
+    sbs.check_gather(2, layers=(0, 1))
+    sbs.close()
+
+
+def test_split_k_grid_invariance(dev):
+    """Any partition of the tile list (1, 3, 37, 148, 1000 CTAs) gives the same answer within
+    rounding, and each is within tolerance of the oracle (pins the cross-CTA LSE merge)."""
+    from paper_2606_01483_b200 import MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA, MURMUR_OPT_ATTN_GRID, MURMUR_OPT_ATTN_VARIANT
+
+    cfg = workloads.config2().with_layers(3).with_seqs(workloads.config2().seqs[:3])
+    sbs = _mk(cfg, dev)
+    ids = [0, 1, 2]
+    sbs.bulk_prefill(ids, 300)
+    sbs.append_step(ids)
+    sbs.evict(ids)
+    q = sbs.queries(ids)
+    outs = []
+    for grid in (1, 3, 37, 148, 1000):
+        sbs.gpu.set_option(MURMUR_OPT_ATTN_GRID, grid)
+        lse = torch.empty(q.shape[:3], dtype=torch.float32, device=dev)
+        out = sbs.gpu.decode_attn(ids, q, lse=lse, sm_scale=sbs.scale)
+        sbs.check_attention(ids, q, out, lse)
+        outs.append(out.float())
+    for o in outs[1:]:
+        assert (o - outs[0]).abs().max().item() <= 2e-2
+    sbs.gpu.set_option(MURMUR_OPT_ATTN_VARIANT, MURMUR_ATTN_GENERIC)
+    out = sbs.gpu.decode_attn(ids, q, sm_scale=sbs.scale)
+    assert (out.float() - outs[0]).abs().max().item() <= 2e-2
+    sbs.gpu.set_option(MURMUR_OPT_ATTN_VARIANT, MURMUR_ATTN_MMA)
+    sbs.close()
+
+
+def test_window_off_equals_full_attention(dev):
+    """I1 on the GPU: windows >= lengths -> every position retained, nothing freed."""
+    W = workloads.WINDOW_OFF
+    cfg = Config("full", 7, Geometry(n_layers=2), 16, (seq_spec(64, 300, 40, W, W), seq_spec(10, 77, 40, W, W)))
+    sbs = _mk(cfg, dev)
+    ids = [0, 1]
+    sbs.bulk_prefill(ids, 30)
+    for _ in range(3):
+        sbs.append_step(ids)
+        sbs.evict(ids)
+        sbs.check_integer_state(ids)
+        for i in ids:
+            assert sbs.gpu.retained(i).tolist() == list(range(sbs.oracle.seqs[i].length))
+        q, out, lse = sbs.attend(ids, want_lse=True)
+        sbs.check_attention(ids, q, out, lse)
+    sbs.close()
+
+
+def test_large_logits_sink_scale_16(dev):
+    """P10: sink keys x16 (logits ~ +-60) stay finite in the fp32 softmax."""
+    cfg = Config("sinks", 8, Geometry(n_layers=1), 64, (seq_spec(64, 200, 10, 64, 32),))
+    sbs = _mk(cfg, dev)
+    k, v = sbs.data[0].prefill_kv()
+    k = k.clone()
+    k[:, :4] = (k[:, :4].float() * 4.0).to(torch.bfloat16)  # x4 on top of the recipe's x4
+    sbs.data[0]._prefill = (k, v)
+    sbs.bulk_prefill([0], 5)
+    q, out, lse = sbs.attend([0], want_lse=True)
+    assert torch.isfinite(out.float()).all() and torch.isfinite(lse).all()
+    sbs.check_attention([0], q, out, lse)
+    sbs.close()
+
+
+# -------------------------------------------------------------------------------- config 4 (sweep), reduced
+@pytest.mark.parametrize("ws,wo", [(128, 64), (256, 1024), (1024, 256), (2250, 64), (2250, 1024)])
+def test_config4_sweep_points_two_layers(dev, ws, wo):
+    cfg = workloads.config4(ws, wo).with_layers(2).with_seqs(workloads.config4(ws, wo).seqs[:2])
+    sbs = _mk(cfg, dev)
+    ids = [0, 1]
+    sbs.bulk_prefill(ids, 1100)
+    for _ in range(2):
+        sbs.append_step(ids)
+        sbs.evict(ids)
+        sbs.check_integer_state(ids)
+        q, out, lse = sbs.attend(ids, want_lse=True)
+        sbs.check_attention(ids, q, out, lse)
+    want = 64 + min(ws, 2250) + 4 + min(wo, sbs.t_of(0) - 4)
+    assert sbs.gpu.seq_state(0)["n_retained"] == want
+    sbs.close()
+
+
+# -------------------------------------------------------------------------------- config 5 (ragged), reduced
+def test_config5_ragged_two_layers_sequences_finish_at_different_steps(dev):
+    full = workloads.config5()
+    cfg = full.with_layers(2)
+    sbs = _mk(cfg, dev)
+    ids = list(range(cfg.batch))
+    # every sequence starts 1..12 tokens before its own end so that they leave the batch one by one
+    rng = random.Random(5)
+    left = {i: rng.randint(1, 12) for i in ids}
+    for i in ids:  # per-sequence bulk prefill (different t0), evicted straight away
+        sbs.bulk_prefill([i], cfg.seqs[i].T - left[i])
+    sbs.check_integer_state(ids)
+    active = list(ids)
+    while active:
+        sbs.append_step(active)
+        sbs.evict(active)
+        sbs.check_integer_state(active)
+        q, out, lse = sbs.attend(active, want_lse=True)
+        sbs.check_attention(active, q, out, lse)
+        for i in list(active):
+            if sbs.t_of(i) >= cfg.seqs[i].T:
+                sbs.gpu.seq_end(i)
+                sbs.oracle.seq_end(i)
+                active.remove(i)
+        assert sbs.gpu.free_stack().tolist() == sbs.oracle.free_stack
+    assert len(sbs.oracle.free_stack) == sbs.oracle.N
+    sbs.close()
+
+
+# -------------------------------------------------------------------------------- full-size, sampled
+def _full_size_steps(sbs, ids, n_steps, sample_layers, seq_subset):
+    for _ in range(n_steps):
+        sbs.append_step(ids)
+        sbs.evict(ids)
+        sbs.check_integer_state(ids)
+        q, out, lse = sbs.attend(ids, want_lse=True)
+        assert torch.isfinite(out.float()).all()
+        sbs.check_attention(ids, q, out, lse, layers=sample_layers, seq_subset=seq_subset)
+
+
+def test_config2_full_size_28_layers_sampled(dev):
+    cfg = workloads.config2()
+    sbs = _mk(cfg, dev, use_c_oracle=True)
+    ids = list(range(12))
+    sbs.bulk_prefill(ids, 300)
+    sbs.check_integer_state(ids)
+    _full_size_steps(sbs, ids, 3, sample_layers=[0, 13, 27], seq_subset=[0, 5, 11])
+    assert sbs.gpu.stats()["attn_grid"] == sbs.gpu.stats()["sm_count"]
+    sbs.close()
+
+
+@pytest.mark.parametrize("evicted", [False, True])
+def test_config3_full_size_28_layers_sampled(dev, evicted):
+    cfg = workloads.config3(evicted)
+    sbs = _mk(cfg, dev, use_c_oracle=True)
+    sbs.bulk_prefill([0], 1030)  # past d = 1024 and k_o + w_o = 516
+    sbs.check_integer_state([0])
+    _full_size_steps(sbs, [0], 2, sample_layers=[0, 27], seq_subset=[0])
+    want = (64 + 27000 + sbs.t_of(0)) if not evicted else (64 + 2048 + 4 + 512)
+    assert sbs.gpu.seq_state(0)["n_retained"] == want
+    sbs.close()
+
+
+def test_config5_full_size_28_layers_sampled(dev):
+    cfg = workloads.config5()
+    sbs = _mk(cfg, dev, use_c_oracle=True)
+    ids = list(range(32))
+    for i in ids:
+        sbs.bulk_prefill([i], min(cfg.seqs[i].T - 2, 1200))
+    sbs.check_integer_state(ids)
+    _full_size_steps(sbs, ids, 2, sample_layers=[5, 27], seq_subset=[0, 9, 31])
+    sbs.close()
+
+
+# -------------------------------------------------------------------------------- host-buffer entry
+def test_decode_step_host_matches_device_calls(dev):
+    cfg = workloads.config1().with_layers(3)
+    a = _mk(cfg, dev)
+    a.bulk_prefill([0], 100)
+    for _ in range(3):
+        u = a.t_of(0)
+        k, v = a.data[0].out_kv(u, u + 1)
+        q = a.data[0].q_step(u + 1).unsqueeze(1).contiguous()
+        kh, vh, qh = k.cpu().pin_memory(), v.cpu().pin_memory(), q.cpu().pin_memory()
+        oh = torch.empty(q.shape, dtype=torch.bfloat16).pin_memory()
+        a.gpu.decode_step_host([0], kh, vh, qh, oh)
+        torch.cuda.synchronize()
+        a._store(0, k, v)
+        a.oracle.append([0], [1])
+        a.oracle.evict([0])
+        a.check_integer_state([0])
+        a.check_attention([0], q, oh.to(dev))
+    a.close()
+
+
+# -------------------------------------------------------------------------------- errors
+def test_error_behaviour_leaves_state_unchanged(dev):
+    from paper_2606_01483_b200 import MurmurCache, MurmurError
+
+    c = MurmurCache(2, 28, 4, 128, 16, max_seqs=3, max_blocks_per_seq=8, n_pages=5, device=dev)
+    pol = (8, 4, 0, 8, 1)
+    c.seq_begin(0, 4, 20, 0, pol)
+    c.seq_begin(1, 4, 20, 0, pol)
+
+    def kv(n):
+        return torch.zeros(2, n, 4, 128, dtype=torch.bfloat16, device=dev)
+
+    with pytest.raises(MurmurError) as e:
+        c.seq_begin(0, 1, 1, 1, pol)
+    assert e.value.status == 2
+    with pytest.raises(MurmurError) as e:
+        c.kv_append([2], [1], kv(1), kv(1))  # inactive
+    assert e.value.status == 2
+    with pytest.raises(MurmurError) as e:
+        c.kv_append([0, 0], [1, 1], kv(2), kv(2))  # duplicate
+    assert e.value.status == 1
+    with pytest.raises(MurmurError) as e:
+        c.kv_append([7], [1], kv(1), kv(1))  # out of range
+    assert e.value.status == 1
+    c.kv_append([0], [40], kv(40), kv(40))  # 3 pages
+    with pytest.raises(MurmurError) as e:
+        c.kv_append([1, 0], [20, 20], kv(40), kv(40))  # needs 2 + 1 pages, 2 free: all-or-nothing
+    assert e.value.status == 3
+    assert c.seq_state(0)["length"] == 40 and c.seq_state(1)["length"] == 0
+    assert c.free_stack().tolist() == [4, 3]
+    with pytest.raises(MurmurError) as e:
+        c.kv_append([0], [200], kv(200), kv(200))  # > max_blocks_per_seq
+    assert e.value.status == 2
+    q = torch.zeros(2, 1, 28, 128, dtype=torch.bfloat16, device=dev)
+    with pytest.raises(MurmurError) as e:
+        c.decode_attn([0], q)  # not evicted since the last append
+    assert e.value.status == 2
+    c.kv_evict([0])
+    c.decode_attn([0], q)
+    with pytest.raises(MurmurError) as e:
+        c.decode_attn([1], q)  # empty sequence
+    assert e.value.status == 2
+    assert c.last_error() == 0
+    c.seq_end(0)
+    assert sorted(c.free_stack().tolist()) == [0, 1, 2, 3, 4]
+    c.close()
