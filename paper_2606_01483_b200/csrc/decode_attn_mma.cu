@@ -10,16 +10,17 @@
 //           murmur_kv_evict; identical for all layers and heads of a sequence.
 //   The flattened tile list (layer, seq, head, tile) is cut into `grid` equal contiguous ranges,
 //   one per CTA (split-K across the retained length whenever a cut falls inside an item).
-// Per CTA: 1 producer warp + 4 consumer warps, a 6-stage ring of (K tile, V tile) buffers.
+// Per CTA: 1 producer warp + 6 consumer warps, a 6-stage ring of (K tile, V tile) buffers
+//   (tile n lives in stage n % 6 and is consumed by warp n % 6, so each stage has one owner).
 //   producer : one lane per tile issues 1-D bulk copies (cp.async.bulk, TMA engine) of each
 //              page's contiguous row range straight into the stage buffer; rows are stored
 //              pre-swizzled in HBM, so the copy needs no tensor map and ldmatrix is
 //              conflict-free.  Bytes copied = retained rows exactly.
-//   consumer : warp w takes every 4th tile.  S^T[64 tok x 8 heads] = K Q^T with mma.sync
+//   consumer : warp w takes every 6th tile.  S^T[64 tok x 8 heads] = K Q^T with mma.sync
 //              m16n8k16 bf16 (tokens are M, the padded head group is N: 7/8 useful), fp32
 //              online softmax in exp2 form, P^T moved to the B-operand layout with movmatrix,
 //              O^T[128 d x 8 heads] += V^T P^T with ldmatrix.trans.
-//   merge    : the four warps' (m, l, O) are merged through shared memory; an item that spans
+//   merge    : the six warps' (m, l, O) are merged through shared memory; an item that spans
 //              several CTAs is finished by the LAST contributor (arrival counter): partials go
 //              to a workspace slot, the last one merges them by the log-sum-exp rule.
 #include <cuda_bf16.h>
@@ -30,7 +31,10 @@ namespace murmur {
 namespace {
 
 constexpr int kStages = 6;
-constexpr int kConsumerWarps = 4;
+constexpr int kConsumerWarps = 6;
+// Every stage must always be consumed by the same warp: a warp that waited on a stage it had not
+// seen the previous phase of could pass try_wait.parity one phase early (parity aliasing).
+static_assert(kStages % kConsumerWarps == 0, "a stage must belong to exactly one consumer warp");
 constexpr int kConsumerThreads = kConsumerWarps * 32;
 constexpr int kMmaThreads = kConsumerThreads + 32;
 constexpr int kTileBytes = kTileRows * kRowBytes;            // 16 KB per K or V tile
@@ -385,7 +389,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     }
     n += (uint32_t)seg;
 
-    // ---- merge the four warps' partial states (LSE rule) ----
+    // ---- merge the consumer warps' partial states (LSE rule) ----
 #pragma unroll
     for (int sh = 4; sh <= 16; sh <<= 1) {
       l0 += __shfl_xor_sync(0xffffffffu, l0, sh);
@@ -409,7 +413,9 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 
     const int layer_c = cur.layer;
     const size_t out_row0 = ((size_t)layer_c * prm.n_seqs_total + prm.seq_base + cur.i) * c.n_q + (size_t)cur.h * G;
-    // thread `tid` owns column d = tid of every head
+    // thread `tid` < 128 owns column d = tid of every head; the other consumer threads only sync
+    const bool owner = tid < kHeadDim;
+    const int col = owner ? tid : 0;
     float accv[kMaxGroup], Mh[kMaxGroup], Lh[kMaxGroup];
 #pragma unroll
     for (int h = 0; h < kMaxGroup; ++h) {
@@ -422,7 +428,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         const float mw = s.scratch[w][kMaxGroup * kOStride + h];
         const float f = (mw == -INFINITY) ? 0.f : ex2((mw - M) * c2);
         L += s.scratch[w][kMaxGroup * kOStride + kMaxGroup + h] * f;
-        acc += s.scratch[w][h * kOStride + tid] * f;
+        acc += s.scratch[w][h * kOStride + col] * f;
       }
       accv[h] = acc; Mh[h] = M; Lh[h] = L;
     }
@@ -430,7 +436,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     if (complete) {
 #pragma unroll
       for (int h = 0; h < kMaxGroup; ++h) {
-        if (h < G) {
+        if (h < G && owner) {
           prm.out[(out_row0 + h) * kHeadDim + tid] = __bfloat16_as_ushort(__float2bfloat16_rn(accv[h] / Lh[h]));
           if (prm.lse != nullptr && tid == 0) prm.lse[out_row0 + h] = Mh[h] * prm.sm_scale + __logf(Lh[h]);
         }
@@ -442,8 +448,10 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       const long long c_last = ((item_lo + nt_i) * geff - 1) / total;
       const int slot = 2 * (int)cta + (first_segment ? 0 : 1);
       float* part = c.partials + (size_t)slot * kPartialFloats;
+      if (owner) {
 #pragma unroll
-      for (int h = 0; h < kMaxGroup; ++h) part[h * kOStride + tid] = accv[h];
+        for (int h = 0; h < kMaxGroup; ++h) part[h * kOStride + tid] = accv[h];
+      }
       if (tid < kMaxGroup) {
         part[kMaxGroup * kOStride + tid] = Mh[tid];
         part[kMaxGroup * kOStride + kMaxGroup + tid] = Lh[tid];
@@ -452,11 +460,12 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       consumer_bar();
       int* counter = c.item_counters + ((size_t)layer_c * n_seqs + cur.i) * n_kv + cur.h;
       if (tid == 0) {
+        __threadfence();  // release: every thread's partial (ordered by the barrier) before the ticket
         const int old = atomicAdd(counter, 1);
         s.flag = (old == (int)(c_last - c_first));
       }
       consumer_bar();
-      if (s.flag) {
+      if (s.flag && owner) {
         __threadfence();
         float M[kMaxGroup], L[kMaxGroup], acc[kMaxGroup];
 #pragma unroll

@@ -27,7 +27,7 @@ def dev():
 
 
 def _mk(cfg, dev, **kw):
-    from tests.harness import SideBySide
+    from harness import SideBySide
 
     return SideBySide(cfg, device=dev, **kw)
 
