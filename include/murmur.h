@@ -167,6 +167,16 @@ MURMUR_API murmur_status_t murmur_decode_attn(murmur_cache_t* cache, const int32
                                               const void* q, void* out, float* lse, int32_t layer_begin,
                                               int32_t layer_end, float sm_scale, void* stream);
 
+/* One whole decode step from DEVICE buffers: append one token to every listed sequence (all
+ * layers) -> evict -> decode_attn, enqueued by ONE host call (PAPER.md:112-116, 136-146, 101-104:
+ * the per-step loop body of Alg. 1 / Alg. 2 followed by Eq. 1).
+ *   k_new, v_new : DEVICE bf16 [n_layers][n_seqs][n_kv_heads][head_dim]
+ *   q, out       : DEVICE bf16 [n_layers][n_seqs][n_q_heads][head_dim];  lse as above or NULL
+ * n_seqs <= MURMUR_MAX_SEQS_PER_LAUNCH.  Validated as a whole before anything is enqueued. */
+MURMUR_API murmur_status_t murmur_decode_step(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                              const void* k_new, const void* v_new, const void* q, void* out,
+                                              float* lse, float sm_scale, void* stream);
+
 /* One whole decode step from HOST buffers (the end-to-end entry): copies k_new, v_new, q
  * (HOST, pinned or pageable, layouts as above with 1 token per sequence and all layers) to
  * device staging, runs append -> evict -> decode_attn, copies out (HOST bf16

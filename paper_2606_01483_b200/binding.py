@@ -28,7 +28,7 @@ STATUS_NAMES = {0: "MURMUR_OK", 1: "MURMUR_ERR_INVALID_ARG", 2: "MURMUR_ERR_STAT
 EXPORTED_SYMBOLS = [
     "murmur_pool_bytes", "murmur_workspace_bytes", "murmur_cache_create", "murmur_cache_destroy",
     "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
-    "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
+    "murmur_decode_step", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
     "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
     "murmur_last_cuda_error", "murmur_version",
@@ -83,6 +83,7 @@ def lib() -> C.CDLL:
     L.murmur_kv_append.argtypes = [vp, vp, vp, i32, vp, vp, i32, i32, vp]
     L.murmur_kv_evict.argtypes = [vp, vp, i32, vp]
     L.murmur_decode_attn.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, C.c_float, vp]
+    L.murmur_decode_step.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, C.c_float, vp]
     L.murmur_decode_step_host.argtypes = [vp, vp, i32, vp, vp, vp, vp, C.c_float, vp]
     L.murmur_seq_get_state.argtypes = [vp, i32, vp, vp]
     L.murmur_kv_get_retained.argtypes = [vp, i32, vp, i32, vp, vp]
@@ -201,6 +202,16 @@ class MurmurCache:
                                               lse.data_ptr() if lse is not None else None, layer_begin, layer_end,
                                               C.c_float(sm_scale), _stream()))
         return out
+
+    def decode_step(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor, out: torch.Tensor,
+                    lse: Optional[torch.Tensor] = None, sm_scale: Optional[float] = None):
+        """append (1 token per sequence, all layers) -> evict -> decode_attn in one C call; DEVICE tensors."""
+        ids = seq_ids if isinstance(seq_ids, np.ndarray) and seq_ids.dtype == np.int32 else _ids(seq_ids)
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        self._check(self.L.murmur_decode_step(self.h, ids.ctypes.data, len(ids), k_new.data_ptr(), v_new.data_ptr(),
+                                              q.data_ptr(), out.data_ptr(),
+                                              lse.data_ptr() if lse is not None else None, C.c_float(sm_scale),
+                                              _stream()))
 
     def decode_step_host(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor,
                          out: torch.Tensor, sm_scale: Optional[float] = None):

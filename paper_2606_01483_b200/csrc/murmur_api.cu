@@ -371,12 +371,45 @@ murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, in
   return MURMUR_OK;
 }
 
+// validates a 1-token-per-sequence append before anything is enqueued (all-or-nothing)
+static murmur_status_t check_step(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs) {
+  if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs);
+  if (st != MURMUR_OK) return st;
+  int64_t need = 0;
+  for (int i = 0; i < n_seqs; ++i) {
+    const HostSeq& hs = c->seqs[seq_ids[i]];
+    if ((int64_t)hs.sp.len + 1 > (int64_t)c->desc.max_blocks_per_seq * c->desc.page_size) return MURMUR_ERR_STATE;
+    need += blocks_for(hs.sp.len + 1, c->desc.page_size) - blocks_for(hs.sp.len, c->desc.page_size);
+  }
+  if (need > c->free_pages) return MURMUR_ERR_OOM_PAGES;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_decode_step(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* k_new,
+                                   const void* v_new, const void* q, void* out, float* lse, float sm_scale,
+                                   void* stream) {
+  if (!c || !k_new || !v_new || !q || !out) return MURMUR_ERR_INVALID_ARG;
+  if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_step(c, seq_ids, n_seqs);
+  if (st != MURMUR_OK) return st;
+  int32_t ones[kMaxSeqsPerLaunch];
+  for (int i = 0; i < n_seqs; ++i) ones[i] = 1;
+  st = murmur_kv_append(c, seq_ids, ones, n_seqs, k_new, v_new, 0, c->desc.n_layers, stream);
+  if (st != MURMUR_OK) return st;
+  st = murmur_kv_evict(c, seq_ids, n_seqs, stream);
+  if (st != MURMUR_OK) return st;
+  return murmur_decode_attn(c, seq_ids, n_seqs, q, out, lse, 0, c->desc.n_layers, sm_scale, stream);
+}
+
 murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs,
                                         const void* k_new_host, const void* v_new_host, const void* q_host,
                                         void* out_host, float sm_scale, void* stream) {
   if (!c || !k_new_host || !v_new_host || !q_host || !out_host) return MURMUR_ERR_INVALID_ARG;
+  if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
   if (n_seqs < 1 || n_seqs > c->cv.stage_seqs) return MURMUR_ERR_INVALID_ARG;
-  murmur_status_t st = check_ids(c, seq_ids, n_seqs);
+  // validate before any copy so that a failing call leaves everything untouched
+  murmur_status_t st = check_step(c, seq_ids, n_seqs);
   if (st != MURMUR_OK) return st;
   cudaStream_t s = (cudaStream_t)stream;
   const size_t kv_b = (size_t)c->desc.n_layers * n_seqs * c->desc.n_kv_heads * kRowBytes;
@@ -385,24 +418,10 @@ murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_id
   uint8_t* dv = c->ws + c->cv.stage_v;
   uint8_t* dq = c->ws + c->cv.stage_q;
   uint8_t* dout = c->ws + c->cv.stage_out;
-  // validate the append before any copy so that a failing call leaves everything untouched
-  int32_t ones[kMaxSeqsPerLaunch];
-  int64_t need = 0;
-  for (int i = 0; i < n_seqs; ++i) {
-    ones[i] = 1;
-    const HostSeq& hs = c->seqs[seq_ids[i]];
-    if ((int64_t)hs.sp.len + 1 > (int64_t)c->desc.max_blocks_per_seq * c->desc.page_size) return MURMUR_ERR_STATE;
-    need += blocks_for(hs.sp.len + 1, c->desc.page_size) - blocks_for(hs.sp.len, c->desc.page_size);
-  }
-  if (need > c->free_pages) return MURMUR_ERR_OOM_PAGES;
   MM_CUDA(c, cudaMemcpyAsync(dk, k_new_host, kv_b, cudaMemcpyHostToDevice, s));
   MM_CUDA(c, cudaMemcpyAsync(dv, v_new_host, kv_b, cudaMemcpyHostToDevice, s));
   MM_CUDA(c, cudaMemcpyAsync(dq, q_host, q_b, cudaMemcpyHostToDevice, s));
-  st = murmur_kv_append(c, seq_ids, ones, n_seqs, dk, dv, 0, c->desc.n_layers, stream);
-  if (st != MURMUR_OK) return st;
-  st = murmur_kv_evict(c, seq_ids, n_seqs, stream);
-  if (st != MURMUR_OK) return st;
-  st = murmur_decode_attn(c, seq_ids, n_seqs, dq, dout, nullptr, 0, c->desc.n_layers, sm_scale, stream);
+  st = murmur_decode_step(c, seq_ids, n_seqs, dk, dv, dq, dout, nullptr, sm_scale, stream);
   if (st != MURMUR_OK) return st;
   MM_CUDA(c, cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, s));
   return MURMUR_OK;
