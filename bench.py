@@ -354,6 +354,13 @@ def run_murmur(args):
     if sampler:
         sampler.window(w0, w1)
     st = cache.stats()
+    if args.timeline and rank == 0:  # per-CTA trace of the last attention launch of region A (profiling aid)
+        tl = cache.attn_timeline().astype(np.int64)
+        t_first = int(tl[:, 0].min())
+        with open(args.timeline, "w") as f:
+            f.write("# cta start_ns end_ns smid tiles   (ns relative to the first CTA start)\n")
+            for b in range(tl.shape[0]):
+                f.write("%d %d %d %d %d\n" % (b, tl[b, 0] - t_first, tl[b, 1] - t_first if tl[b, 1] else -1, tl[b, 2], tl[b, 3]))
 
     # ---- region B: K steps with per-kernel events ---------------------------------------------
     n_ret_b0 = sum(cache.seq_state(i)["n_retained"] for i in range(B))
@@ -540,6 +547,7 @@ def main():
     ap.add_argument("--variant", default="", choices=["", "generic", "mma"])
     ap.add_argument("--grid", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--timeline", default="", help="write the per-CTA trace of one attention launch to this file")
     ap.add_argument("--cpu-budget-s", default="12")
     ap.add_argument("--ref-budget-s", default="120")
     args = ap.parse_args()

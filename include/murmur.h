@@ -209,6 +209,12 @@ MURMUR_API murmur_status_t murmur_kv_gather(murmur_cache_t* cache, int32_t seq, 
 /* Device error word: 0 or the first MURMUR_ERR_* a kernel detected since creation. */
 MURMUR_API murmur_status_t murmur_get_last_error(murmur_cache_t* cache, int32_t* device_err_out, void* stream);
 
+/* Per-CTA trace of the LAST tensor-core attention launch (profiling aid): out is HOST
+ * uint64[n][4] = {globaltimer ns at CTA start, at CTA end, SM id, tiles processed}; *n_out = CTAs
+ * of that launch (0 if the last launch was the generic variant). */
+MURMUR_API murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* cache, uint64_t* out, int32_t cap_ctas,
+                                                      int32_t* n_out, void* stream);
+
 /* ---- options / stats --------------------------------------------------------------------- */
 MURMUR_API murmur_status_t murmur_set_option(murmur_cache_t* cache, int32_t option, int32_t value);
 MURMUR_API murmur_status_t murmur_get_stats(murmur_cache_t* cache, murmur_stats_t* out);

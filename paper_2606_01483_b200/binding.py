@@ -30,6 +30,7 @@ EXPORTED_SYMBOLS = [
     "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
     "murmur_decode_step", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
+    "murmur_debug_attn_timeline",
     "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
     "murmur_last_cuda_error", "murmur_version",
 ]
@@ -92,6 +93,7 @@ def lib() -> C.CDLL:
     L.murmur_kv_get_free_stack.argtypes = [vp, vp, i64, vp, vp]
     L.murmur_kv_gather.argtypes = [vp, i32, vp, i32, i32, i32, vp, vp, vp]
     L.murmur_get_last_error.argtypes = [vp, vp, vp]
+    L.murmur_debug_attn_timeline.argtypes = [vp, vp, i32, vp, vp]
     L.murmur_set_option.argtypes = [vp, i32, i32]
     L.murmur_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.murmur_reset_stats.argtypes = [vp]
@@ -271,6 +273,13 @@ class MurmurCache:
         e = C.c_int32(0)
         self._check(self.L.murmur_get_last_error(self.h, C.byref(e), _stream()))
         return e.value
+
+    def attn_timeline(self) -> np.ndarray:
+        """uint64 [n_ctas, 4] = (start ns, end ns, SM id, tiles) of the last tensor-core attention launch."""
+        a = np.zeros((1024, 4), dtype=np.uint64)
+        n = C.c_int32(0)
+        self._check(self.L.murmur_debug_attn_timeline(self.h, a.ctypes.data, 1024, C.byref(n), _stream()))
+        return a[: n.value].copy()
 
     def set_option(self, option: int, value: int):
         self._check(self.L.murmur_set_option(self.h, option, value))

@@ -31,20 +31,25 @@ namespace murmur {
 namespace {
 
 constexpr int kStages = 6;
-constexpr int kConsumerWarps = 6;
-// Every stage must always be consumed by the same warp: a warp that waited on a stage it had not
-// seen the previous phase of could pass try_wait.parity one phase early (parity aliasing).
-static_assert(kStages % kConsumerWarps == 0, "a stage must belong to exactly one consumer warp");
+constexpr int kSliceWarps = 4;   // the four 16-row slices of a 64-row tile, one warp each
+constexpr int kGroups = 2;       // warp groups; group g consumes tiles n with n % kGroups == g
+constexpr int kConsumerWarps = kSliceWarps * kGroups;
+// A stage must always be consumed by the same warps: a warp that waited on a stage it had not seen
+// the previous phase of could pass try_wait.parity one phase early (parity aliasing).
+static_assert(kStages % kGroups == 0, "a stage must belong to exactly one consumer group");
+static_assert(kTileRows == kSliceWarps * 16, "one m16 slice per warp");
 constexpr int kConsumerThreads = kConsumerWarps * 32;
 constexpr int kMmaThreads = kConsumerThreads + 32;
 constexpr int kTileBytes = kTileRows * kRowBytes;            // 16 KB per K or V tile
 constexpr int kQBytes = kMaxGroup * kRowBytes;               // 2 KB
 constexpr int kScratchFloats = kMaxGroup * kOStride + 2 * kMaxGroup;  // o[8][132], m[8], l[8]
+constexpr int kFragFloats = 36 * 32;                         // o[32] + m[2] + l[2] per lane, [reg][lane]
+static_assert(kFragFloats >= kScratchFloats, "the two merge layouts share one buffer");
 
 struct __align__(128) SmemLayout {
   uint8_t kv[kStages][2][kTileBytes];
   uint8_t q[2][kQBytes];
-  float scratch[kConsumerWarps][kScratchFloats];
+  float scratch[kSliceWarps][kFragFloats];  // group merge (fragment layout), then slice merge (o[8][132], m, l)
   unsigned long long full_k[kStages], full_v[kStages], empty[kStages], q_full[2], q_empty[2];
   int meta[kStages][2];  // row_begin, row_end of the tile in each stage
   int nt[kMaxSeqsPerLaunch];
@@ -111,6 +116,16 @@ __device__ __forceinline__ float ex2(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ unsigned smid() {
+  unsigned r;
+  asm volatile("mov.u32 %0, %%smid;" : "=r"(r));
+  return r;
+}
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory"); }
 
 // ---- walking the flattened (layer, seq, head, tile) list ---------------------------------------------
@@ -159,13 +174,20 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   SmemLayout& s = *reinterpret_cast<SmemLayout*>(smem_raw);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int n_seqs = list.n, n_kv = c.n_kv, G = c.group;
+  unsigned long long* trace = c.timeline + (size_t)blockIdx.x * kTimelineWords;
+  if (tid == 0) {
+    trace[0] = globaltimer_ns();
+    trace[1] = 0ull;
+    trace[2] = smid();
+    trace[3] = 0ull;
+  }
 
   // ---- setup: barriers, tile counts, zeroed padding rows of the Q buffers ------------------------
   if (tid == 0) {
     for (int i = 0; i < kStages; ++i) {
       mbar_init(&s.full_k[i], 1);
       mbar_init(&s.full_v[i], 1);
-      mbar_init(&s.empty[i], 1);
+      mbar_init(&s.empty[i], kSliceWarps);
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(&s.q_full[i], 1);
@@ -198,66 +220,94 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 
   if (warp == kConsumerWarps) {
     // =================================== producer warp ===================================
+    // Walks its tile range in batches of <= 32 tiles of one item (lane j issues tile j); the
+    // descriptors of the NEXT batch are loaded before the current one is issued, so their
+    // global-load latency hides behind the copies.
     Cursor cur = locate(s, n_seqs, n_kv, lo);
-    long long remaining = hi - lo;
+    long long remaining = hi - lo;  // tiles left, counted from the start of the current item's segment
+    int seg = (int)min((long long)(s.nt[cur.i] - cur.k), remaining);
+    int base = 0, cnt = min(32, seg);
     uint32_t n = 0;  // tile sequence number of this CTA
     int item_no = 0;
+    TileDesc td;
+    if (lane < cnt) td = c.tiles[(size_t)list.ids[cur.i] * c.max_blocks + cur.k + lane];
     while (remaining > 0) {
-      const int id = list.ids[cur.i];
-      const int seg = (int)min((long long)(s.nt[cur.i] - cur.k), remaining);
+      // ---- next batch (prefetch its descriptors) ----
+      Cursor ncur = cur;
+      int nseg = seg, nbase = base + cnt, ncnt = 0;
+      long long nrem = remaining;
+      const bool item_done = nbase >= seg;
+      if (item_done) {
+        nrem = remaining - seg;
+        nbase = 0;
+        if (nrem > 0) {
+          next_item(s, n_seqs, n_kv, ncur);
+          nseg = (int)min((long long)s.nt[ncur.i], nrem);
+        }
+      }
+      if (nrem > 0) ncnt = min(32, nseg - nbase);
+      TileDesc ntd;
+      if (lane < ncnt) ntd = c.tiles[(size_t)list.ids[ncur.i] * c.max_blocks + ncur.k + nbase + lane];
+
+      // ---- current batch ----
       const int layer = prm.layer_begin + cur.layer;
-      if (lane == 0) {  // stage this item's G query rows
+      if (base == 0 && lane == 0) {  // first batch of an item: stage its G query rows
         const int qb = item_no & 1;
         mbar_wait(&s.q_empty[qb], ((item_no >> 1) & 1) ^ 1);
         const size_t row = ((size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i) * c.n_q + (size_t)cur.h * G;
         mbar_expect_tx(&s.q_full[qb], (uint32_t)(G * kRowBytes));
         bulk_g2s(&s.q[qb][0], prm.q + row * kHeadDim, (uint32_t)(G * kRowBytes), &s.q_full[qb]);
       }
-      const TileDesc* tiles = c.tiles + (size_t)id * c.max_blocks + cur.k;
-      for (int base = 0; base < seg; base += 32) {
-        const int mine = base + lane;
-        TileDesc td;
-        if (mine < seg) td = tiles[mine];
-        const int cnt = min(32, seg - base);
-        for (int j = 0; j < cnt; ++j) {
-          if (lane == j) {
-            const uint32_t nn = n + (uint32_t)j;
-            const int st = (int)(nn % kStages);
-            const uint32_t ph = (nn / kStages) & 1u;
-            mbar_wait(&s.empty[st], ph ^ 1u);
-            s.meta[st][0] = td.row_begin;
-            s.meta[st][1] = td.row_end;
-            const uint32_t bytes = (uint32_t)(td.row_end - td.row_begin) * kRowBytes;
-            mbar_expect_tx(&s.full_k[st], bytes);
-            mbar_expect_tx(&s.full_v[st], bytes);
+      for (int j = 0; j < cnt; ++j) {
+        if (lane == j) {
+          const uint32_t nn = n + (uint32_t)j;
+          const int st = (int)(nn % kStages);
+          const uint32_t ph = (nn / kStages) & 1u;
+          mbar_wait(&s.empty[st], ph ^ 1u);
+          s.meta[st][0] = td.row_begin;
+          s.meta[st][1] = td.row_end;
+          const uint32_t bytes = (uint32_t)(td.row_end - td.row_begin) * kRowBytes;
+          mbar_expect_tx(&s.full_k[st], bytes);
+          mbar_expect_tx(&s.full_v[st], bytes);
 #pragma unroll
-            for (int kv = 0; kv < 2; ++kv) {
-              const uint8_t* pool = kv ? vpool : kpool;
-              unsigned long long* bar = kv ? &s.full_v[st] : &s.full_k[st];
+          for (int kv = 0; kv < 2; ++kv) {
+            const uint8_t* pool = kv ? vpool : kpool;
+            unsigned long long* bar = kv ? &s.full_v[st] : &s.full_k[st];
 #pragma unroll
-              for (int pg = 0; pg < 4; ++pg) {
-                if (pg < td.n_pages) {
-                  const int r0 = (pg == 0) ? td.row_begin : pg * c.p;
-                  const int r1 = (pg == td.n_pages - 1) ? td.row_end : (pg + 1) * c.p;
-                  const uint8_t* src = pool + row_offset(c, layer, td.page[pg], cur.h, r0 - pg * c.p);
-                  bulk_g2s(&s.kv[st][kv][r0 * kRowBytes], src, (uint32_t)(r1 - r0) * kRowBytes, bar);
-                }
+            for (int pg = 0; pg < 4; ++pg) {
+              if (pg < td.n_pages) {
+                const int r0 = (pg == 0) ? td.row_begin : pg * c.p;
+                const int r1 = (pg == td.n_pages - 1) ? td.row_end : (pg + 1) * c.p;
+                const uint8_t* src = pool + row_offset(c, layer, td.page[pg], cur.h, r0 - pg * c.p);
+                bulk_g2s(&s.kv[st][kv][r0 * kRowBytes], src, (uint32_t)(r1 - r0) * kRowBytes, bar);
               }
             }
           }
-          __syncwarp();
         }
-        n += (uint32_t)cnt;
+        __syncwarp();
       }
-      remaining -= seg;
-      ++item_no;
-      next_item(s, n_seqs, n_kv, cur);
+      n += (uint32_t)cnt;
+      if (item_done) {
+        ++item_no;
+        remaining = nrem;
+      }
+      cur = ncur;
+      seg = nseg;
+      base = nbase;
+      cnt = ncnt;
+      td = ntd;
     }
     return;
   }
 
   // ===================================== consumer warps =====================================
+  // Warp (grp, w4): group grp takes every kGroups-th tile; inside a tile the warp owns rows
+  // [16 w4, 16 w4 + 16).  All four warps of a group finish a tile within a few hundred cycles,
+  // so a stage is handed back to the producer almost as soon as its data has landed and nearly
+  // the whole ring stays in flight.  Each warp keeps its own online-softmax state (m, l, O^T)
+  // over the rows it has seen; the states are merged at the end of the item.
   const float c2 = prm.sm_scale * 1.4426950408889634f;  // scores are kept raw; exp2((s - m) * c2)
+  const int w4 = warp & (kSliceWarps - 1), grp = warp / kSliceWarps;
   const int lrow = lane >> 2;         // row inside an 8-row group / head index of B fragments
   const int lcol = (lane & 3) * 2;    // first of the two heads (or tokens) this lane owns
   // ldmatrix lane addressing (row inside the 16-row group, 16-byte chunk select, swizzle key)
@@ -266,6 +316,9 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   const int lv_row = (lane >> 4) * 8 + (lane & 7);        // V (transposed): (rows 0-7, c), (0-7, c+1),
   const int lv_chk = (lane >> 3) & 1;                     //   (8-15, c), (8-15, c+1)
   const int key = lane & 7;
+  const int slice0 = w4 * 16;                             // first row of this warp's slice
+  const uint32_t k_off = (uint32_t)(slice0 + lm_row) * kRowBytes;
+  const uint32_t v_off = (uint32_t)(slice0 + lv_row) * kRowBytes;
 
   Cursor cur = locate(s, n_seqs, n_kv, lo);
   long long remaining = hi - lo;
@@ -273,7 +326,6 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   uint32_t n = 0;
   int item_no = 0;
   bool first_segment = true;
-  float* my_scratch = s.scratch[warp];
 
   while (remaining > 0) {
     const int nt_i = s.nt[cur.i];
@@ -300,88 +352,74 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 #pragma unroll
     for (int dt = 0; dt < 8; ++dt) o[dt][0] = o[dt][1] = o[dt][2] = o[dt][3] = 0.f;
 
-    for (int tt = 0; tt < seg; ++tt) {
+    for (int tt = (grp + kGroups - (int)(n % kGroups)) % kGroups; tt < seg; tt += kGroups) {
       const uint32_t nn = n + (uint32_t)tt;
-      if ((int)(nn % kConsumerWarps) != warp) continue;
       const int st = (int)(nn % kStages);
       const uint32_t ph = (nn / kStages) & 1u;
       mbar_wait(&s.full_k[st], ph);
       const int rb = s.meta[st][0], re = s.meta[st][1];
-      const uint32_t kbase = smem_u32(&s.kv[st][0][0]);
-      const uint32_t vbase = smem_u32(&s.kv[st][1][0]);
-
-      // ---- S^T = K Q^T for the 16-row groups that hold valid rows ----
-      float sc[4][4];
-      float mx0 = -INFINITY, mx1 = -INFINITY;
+      const bool act = (slice0 < re) && (slice0 + 16 > rb);  // warp-uniform: the slice holds valid rows
+      uint32_t pb0 = 0u, pb1 = 0u;
+      if (act) {
+        // ---- S^T[16 x 8] = K Q^T, two independent accumulator chains ----
+        const uint32_t rowaddr = smem_u32(&s.kv[st][0][0]) + k_off;
+        float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-      for (int mt = 0; mt < 4; ++mt) {
-        sc[mt][0] = sc[mt][1] = sc[mt][2] = sc[mt][3] = 0.f;
-        if (mt * 16 < re && mt * 16 + 16 > rb) {
-          const uint32_t rowaddr = kbase + (uint32_t)(mt * 16 + lm_row) * kRowBytes;
-#pragma unroll
-          for (int ks = 0; ks < 8; ++ks) {
-            uint32_t a[4];
-            ldsm_x4(a, rowaddr + (uint32_t)(((2 * ks + lm_chk) ^ key) << 4));
-            mma_bf16(sc[mt], a, qf[ks][0], qf[ks][1]);
-          }
-          const int r0 = mt * 16 + lrow, r1 = r0 + 8;
-          if (r0 < rb || r0 >= re) sc[mt][0] = sc[mt][1] = -INFINITY;
-          if (r1 < rb || r1 >= re) sc[mt][2] = sc[mt][3] = -INFINITY;
-          mx0 = fmaxf(mx0, fmaxf(sc[mt][0], sc[mt][2]));
-          mx1 = fmaxf(mx1, fmaxf(sc[mt][1], sc[mt][3]));
-        } else {
-          sc[mt][0] = sc[mt][1] = sc[mt][2] = sc[mt][3] = -INFINITY;
+        for (int ks = 0; ks < 8; ks += 2) {
+          uint32_t a[4], b[4];
+          ldsm_x4(a, rowaddr + (uint32_t)(((2 * ks + lm_chk) ^ key) << 4));
+          ldsm_x4(b, rowaddr + (uint32_t)(((2 * ks + 2 + lm_chk) ^ key) << 4));
+          mma_bf16(sa, a, qf[ks][0], qf[ks][1]);
+          mma_bf16(sb, b, qf[ks + 1][0], qf[ks + 1][1]);
         }
-      }
+        float s0 = sa[0] + sb[0], s1 = sa[1] + sb[1], s2 = sa[2] + sb[2], s3 = sa[3] + sb[3];
+        const int r0 = slice0 + lrow, r1 = r0 + 8;
+        if (r0 < rb || r0 >= re) s0 = s1 = -INFINITY;
+        if (r1 < rb || r1 >= re) s2 = s3 = -INFINITY;
+        float mx0 = fmaxf(s0, s2), mx1 = fmaxf(s1, s3);
 #pragma unroll
-      for (int sh = 4; sh <= 16; sh <<= 1) {
-        mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, sh));
-        mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, sh));
-      }
-      const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
-      const float cr0 = ex2((m0 - mn0) * c2), cr1 = ex2((m1 - mn1) * c2);
-      m0 = mn0;
-      m1 = mn1;
-      l0 *= cr0;
-      l1 *= cr1;
-#pragma unroll
-      for (int dt = 0; dt < 8; ++dt) {
-        o[dt][0] *= cr0; o[dt][1] *= cr1; o[dt][2] *= cr0; o[dt][3] *= cr1;
-      }
-      // ---- P^T fragments: exp2, bf16, transpose into the B-operand layout ----
-      const float ms0 = mn0 * c2, ms1 = mn1 * c2;
-      uint32_t pb[4][2];
-#pragma unroll
-      for (int mt = 0; mt < 4; ++mt) {
-        const float p0 = ex2(sc[mt][0] * c2 - ms0), p1 = ex2(sc[mt][1] * c2 - ms1);
-        const float p2 = ex2(sc[mt][2] * c2 - ms0), p3 = ex2(sc[mt][3] * c2 - ms1);
-        l0 += p0 + p2;
-        l1 += p1 + p3;
-        pb[mt][0] = movmatrix_t(pack_bf16(p0, p1));
-        pb[mt][1] = movmatrix_t(pack_bf16(p2, p3));
-      }
-      // ---- O^T += V^T P^T ----
-      mbar_wait(&s.full_v[st], ph);
-#pragma unroll
-      for (int kt = 0; kt < 4; ++kt) {
-        if (kt * 16 < re && kt * 16 + 16 > rb) {
-          const uint32_t rowaddr = vbase + (uint32_t)(kt * 16 + lv_row) * kRowBytes;
-          const bool edge = (kt * 16 < rb) || (kt * 16 + 16 > re);
-          uint32_t mk01 = 0xffffffffu, mk23 = 0xffffffffu;
-          if (edge) {  // rows outside [rb, re) were never copied: zero them in the A fragment
-            const int t0 = kt * 16 + lcol;
-            mk01 = ((t0 >= rb && t0 < re) ? 0x0000ffffu : 0u) | ((t0 + 1 >= rb && t0 + 1 < re) ? 0xffff0000u : 0u);
-            mk23 = ((t0 + 8 >= rb && t0 + 8 < re) ? 0x0000ffffu : 0u) | ((t0 + 9 >= rb && t0 + 9 < re) ? 0xffff0000u : 0u);
-          }
+        for (int sh = 4; sh <= 16; sh <<= 1) {
+          mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, sh));
+          mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, sh));
+        }
+        const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);  // finite: the slice has a valid row
+        if (__any_sync(0xffffffffu, (mn0 != m0) || (mn1 != m1))) {
+          const float cr0 = ex2((m0 - mn0) * c2), cr1 = ex2((m1 - mn1) * c2);
+          m0 = mn0;
+          m1 = mn1;
+          l0 *= cr0;
+          l1 *= cr1;
 #pragma unroll
           for (int dt = 0; dt < 8; ++dt) {
-            uint32_t a[4];
-            ldsm_x4_t(a, rowaddr + (uint32_t)(((2 * dt + lv_chk) ^ key) << 4));
-            if (edge) {
-              a[0] &= mk01; a[1] &= mk01; a[2] &= mk23; a[3] &= mk23;
-            }
-            mma_bf16(o[dt], a, pb[kt][0], pb[kt][1]);
+            o[dt][0] *= cr0; o[dt][1] *= cr1; o[dt][2] *= cr0; o[dt][3] *= cr1;
           }
+        }
+        // ---- P^T fragment: exp2, bf16, transpose into the B-operand layout ----
+        const float ms0 = m0 * c2, ms1 = m1 * c2;
+        const float p0 = ex2(s0 * c2 - ms0), p1 = ex2(s1 * c2 - ms1);
+        const float p2 = ex2(s2 * c2 - ms0), p3 = ex2(s3 * c2 - ms1);
+        l0 += p0 + p2;
+        l1 += p1 + p3;
+        pb0 = movmatrix_t(pack_bf16(p0, p1));
+        pb1 = movmatrix_t(pack_bf16(p2, p3));
+      }
+      // ---- O^T[128 x 8] += V^T P^T over this warp's 16 rows ----
+      mbar_wait(&s.full_v[st], ph);
+      if (act) {
+        const uint32_t rowaddr = smem_u32(&s.kv[st][1][0]) + v_off;
+        const bool edge = (slice0 < rb) || (slice0 + 16 > re);
+        uint32_t mk01 = 0xffffffffu, mk23 = 0xffffffffu;
+        if (edge) {  // rows outside [rb, re) were never copied: zero them in the A fragment
+          const int t0 = slice0 + lcol;
+          mk01 = ((t0 >= rb && t0 < re) ? 0x0000ffffu : 0u) | ((t0 + 1 >= rb && t0 + 1 < re) ? 0xffff0000u : 0u);
+          mk23 = ((t0 + 8 >= rb && t0 + 8 < re) ? 0x0000ffffu : 0u) | ((t0 + 9 >= rb && t0 + 9 < re) ? 0xffff0000u : 0u);
+        }
+#pragma unroll
+        for (int dt = 0; dt < 8; ++dt) {
+          uint32_t a[4];
+          ldsm_x4_t(a, rowaddr + (uint32_t)(((2 * dt + lv_chk) ^ key) << 4));
+          a[0] &= mk01; a[1] &= mk01; a[2] &= mk23; a[3] &= mk23;
+          mma_bf16(o[dt], a, pb0, pb1);
         }
       }
       __syncwarp();
@@ -389,25 +427,66 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     }
     n += (uint32_t)seg;
 
-    // ---- merge the consumer warps' partial states (LSE rule) ----
+    // ---- merge 1: groups 1.. hand their state to group 0 (same fragment layout, lane for lane) ----
 #pragma unroll
-    for (int sh = 4; sh <= 16; sh <<= 1) {
-      l0 += __shfl_xor_sync(0xffffffffu, l0, sh);
-      l1 += __shfl_xor_sync(0xffffffffu, l1, sh);
-    }
+    for (int r = 1; r < kGroups; ++r) {
+      float* fs = s.scratch[w4];
+      if (grp == r) {
 #pragma unroll
-    for (int dt = 0; dt < 8; ++dt) {
-      const int d = dt * 16 + lrow;
-      my_scratch[lcol * kOStride + d] = o[dt][0];
-      my_scratch[(lcol + 1) * kOStride + d] = o[dt][1];
-      my_scratch[lcol * kOStride + d + 8] = o[dt][2];
-      my_scratch[(lcol + 1) * kOStride + d + 8] = o[dt][3];
+        for (int dt = 0; dt < 8; ++dt) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) fs[(dt * 4 + e) * 32 + lane] = o[dt][e];
+        }
+        fs[32 * 32 + lane] = m0;
+        fs[33 * 32 + lane] = m1;
+        fs[34 * 32 + lane] = l0;
+        fs[35 * 32 + lane] = l1;
+      }
+      consumer_bar();
+      if (grp == 0) {
+        const float mo0 = fs[32 * 32 + lane], mo1 = fs[33 * 32 + lane];
+        const float mn0 = fmaxf(m0, mo0), mn1 = fmaxf(m1, mo1);
+        const float fa0 = (m0 == -INFINITY) ? 0.f : ex2((m0 - mn0) * c2);
+        const float fa1 = (m1 == -INFINITY) ? 0.f : ex2((m1 - mn1) * c2);
+        const float fb0 = (mo0 == -INFINITY) ? 0.f : ex2((mo0 - mn0) * c2);
+        const float fb1 = (mo1 == -INFINITY) ? 0.f : ex2((mo1 - mn1) * c2);
+        l0 = l0 * fa0 + fs[34 * 32 + lane] * fb0;
+        l1 = l1 * fa1 + fs[35 * 32 + lane] * fb1;
+#pragma unroll
+        for (int dt = 0; dt < 8; ++dt) {
+          o[dt][0] = o[dt][0] * fa0 + fs[(dt * 4 + 0) * 32 + lane] * fb0;
+          o[dt][1] = o[dt][1] * fa1 + fs[(dt * 4 + 1) * 32 + lane] * fb1;
+          o[dt][2] = o[dt][2] * fa0 + fs[(dt * 4 + 2) * 32 + lane] * fb0;
+          o[dt][3] = o[dt][3] * fa1 + fs[(dt * 4 + 3) * 32 + lane] * fb1;
+        }
+        m0 = mn0;
+        m1 = mn1;
+      }
+      consumer_bar();
     }
-    if (lrow == 0) {
-      my_scratch[kMaxGroup * kOStride + lcol] = m0;
-      my_scratch[kMaxGroup * kOStride + lcol + 1] = m1;
-      my_scratch[kMaxGroup * kOStride + kMaxGroup + lcol] = l0;
-      my_scratch[kMaxGroup * kOStride + kMaxGroup + lcol + 1] = l1;
+
+    // ---- merge 2: the four row slices of group 0, through shared memory in [head][d] layout ----
+    if (grp == 0) {
+#pragma unroll
+      for (int sh = 4; sh <= 16; sh <<= 1) {
+        l0 += __shfl_xor_sync(0xffffffffu, l0, sh);
+        l1 += __shfl_xor_sync(0xffffffffu, l1, sh);
+      }
+      float* my_scratch = s.scratch[w4];
+#pragma unroll
+      for (int dt = 0; dt < 8; ++dt) {
+        const int d = dt * 16 + lrow;
+        my_scratch[lcol * kOStride + d] = o[dt][0];
+        my_scratch[(lcol + 1) * kOStride + d] = o[dt][1];
+        my_scratch[lcol * kOStride + d + 8] = o[dt][2];
+        my_scratch[(lcol + 1) * kOStride + d + 8] = o[dt][3];
+      }
+      if (lrow == 0) {
+        my_scratch[kMaxGroup * kOStride + lcol] = m0;
+        my_scratch[kMaxGroup * kOStride + lcol + 1] = m1;
+        my_scratch[kMaxGroup * kOStride + kMaxGroup + lcol] = l0;
+        my_scratch[kMaxGroup * kOStride + kMaxGroup + lcol + 1] = l1;
+      }
     }
     consumer_bar();
 
@@ -417,20 +496,22 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     const bool owner = tid < kHeadDim;
     const int col = owner ? tid : 0;
     float accv[kMaxGroup], Mh[kMaxGroup], Lh[kMaxGroup];
+    if (owner) {
 #pragma unroll
-    for (int h = 0; h < kMaxGroup; ++h) {
-      float M = -INFINITY;
+      for (int h = 0; h < kMaxGroup; ++h) {
+        float M = -INFINITY;
 #pragma unroll
-      for (int w = 0; w < kConsumerWarps; ++w) M = fmaxf(M, s.scratch[w][kMaxGroup * kOStride + h]);
-      float L = 0.f, acc = 0.f;
+        for (int w = 0; w < kSliceWarps; ++w) M = fmaxf(M, s.scratch[w][kMaxGroup * kOStride + h]);
+        float L = 0.f, acc = 0.f;
 #pragma unroll
-      for (int w = 0; w < kConsumerWarps; ++w) {
-        const float mw = s.scratch[w][kMaxGroup * kOStride + h];
-        const float f = (mw == -INFINITY) ? 0.f : ex2((mw - M) * c2);
-        L += s.scratch[w][kMaxGroup * kOStride + kMaxGroup + h] * f;
-        acc += s.scratch[w][h * kOStride + col] * f;
+        for (int w = 0; w < kSliceWarps; ++w) {
+          const float mw = s.scratch[w][kMaxGroup * kOStride + h];
+          const float f = (mw == -INFINITY) ? 0.f : ex2((mw - M) * c2);
+          L += s.scratch[w][kMaxGroup * kOStride + kMaxGroup + h] * f;
+          acc += s.scratch[w][h * kOStride + col] * f;
+        }
+        accv[h] = acc; Mh[h] = M; Lh[h] = L;
       }
-      accv[h] = acc; Mh[h] = M; Lh[h] = L;
     }
 
     if (complete) {
@@ -452,9 +533,12 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 #pragma unroll
         for (int h = 0; h < kMaxGroup; ++h) part[h * kOStride + tid] = accv[h];
       }
-      if (tid < kMaxGroup) {
-        part[kMaxGroup * kOStride + tid] = Mh[tid];
-        part[kMaxGroup * kOStride + kMaxGroup + tid] = Lh[tid];
+      if (tid == 0) {
+#pragma unroll
+        for (int h = 0; h < kMaxGroup; ++h) {
+          part[kMaxGroup * kOStride + h] = Mh[h];
+          part[kMaxGroup * kOStride + kMaxGroup + h] = Lh[h];
+        }
       }
       __threadfence();
       consumer_bar();
@@ -504,6 +588,10 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     first_segment = false;
     ++item_no;
     next_item(s, n_seqs, n_kv, cur);
+  }
+  if (tid == 0) {
+    trace[1] = globaltimer_ns();
+    trace[3] = (unsigned long long)(hi - lo);
   }
 }
 

@@ -25,6 +25,7 @@ constexpr int kMaxSeqsPerLaunch = 128;
 constexpr int kOStride = 132;            // floats per head row in split-K partials / merge scratch
 constexpr int kPartialFloats = kMaxGroup * kOStride + 2 * kMaxGroup;  // o[8][132] + m[8] + l[8]
 constexpr int kMaxAttnGrid = 1024;       // upper bound on CTAs of the persistent attention kernel
+constexpr int kTimelineWords = 4;        // globaltimer at CTA start, at CTA end, SM id, tiles processed
 
 // ctrl word indices
 enum { kCtrlFreeTop = 0, kCtrlError = 1, kCtrlAppendTicket = 2, kCtrlWords = 8 };
@@ -64,6 +65,7 @@ struct CacheView {
   int32_t* ctrl;         // [kCtrlWords]
   int32_t* item_counters;  // [n_layers][max_seqs][n_kv] split-K arrival counters (self-resetting)
   float* partials;       // [2 * kMaxAttnGrid][kPartialFloats]
+  unsigned long long* timeline;  // [kMaxAttnGrid][kTimelineWords] per-CTA trace of the last attention launch
 };
 
 struct SeqList {  // per-launch sequence list, passed by value (no H2D copy, graph-capturable)

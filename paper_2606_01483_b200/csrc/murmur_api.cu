@@ -29,7 +29,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Carve {
-  size_t seqs, block_table, live_pages, live_blocks, tiles, free_stack, ctrl, counters, partials;
+  size_t seqs, block_table, live_pages, live_blocks, tiles, free_stack, ctrl, counters, partials, timeline;
   size_t stage_k, stage_v, stage_q, stage_out, scratch;
   size_t total;
   int stage_seqs;
@@ -67,6 +67,7 @@ Carve carve(const murmur_cache_desc_t* d) {
   c.ctrl = take(kCtrlWords * 4);
   c.counters = take((size_t)d->n_layers * kMaxSeqsPerLaunch * d->n_kv_heads * 4);
   c.partials = take((size_t)2 * kMaxAttnGrid * kPartialFloats * 4);
+  c.timeline = take((size_t)kMaxAttnGrid * kTimelineWords * 8);
   c.stage_seqs = d->max_seqs < kMaxSeqsPerLaunch ? d->max_seqs : kMaxSeqsPerLaunch;
   const size_t kv_b = (size_t)d->n_layers * c.stage_seqs * d->n_kv_heads * kRowBytes;
   const size_t q_b = (size_t)d->n_layers * c.stage_seqs * d->n_q_heads * kRowBytes;
@@ -184,6 +185,7 @@ murmur_status_t murmur_cache_create(const murmur_cache_desc_t* d, murmur_cache_t
   v.ctrl = reinterpret_cast<int32_t*>(c->ws + cv.ctrl);
   v.item_counters = reinterpret_cast<int32_t*>(c->ws + cv.counters);
   v.partials = reinterpret_cast<float*>(c->ws + cv.partials);
+  v.timeline = reinterpret_cast<unsigned long long*>(c->ws + cv.timeline);
   LaunchInfo li{};
   e = launch_init(v, (cudaStream_t)stream, &li);
   if (e != cudaSuccess) {
@@ -549,6 +551,18 @@ murmur_status_t murmur_get_last_error(murmur_cache_t* c, int32_t* device_err_out
   if (!c || !device_err_out) return MURMUR_ERR_INVALID_ARG;
   MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
   MM_CUDA(c, cudaMemcpy(device_err_out, c->view.ctrl + kCtrlError, 4, cudaMemcpyDeviceToHost));
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* c, uint64_t* out, int32_t cap_ctas, int32_t* n_out,
+                                           void* stream) {
+  if (!c || !n_out || cap_ctas < 0 || (cap_ctas > 0 && !out)) return MURMUR_ERR_INVALID_ARG;
+  const int n = c->stats.attn_variant == MURMUR_ATTN_MMA ? c->stats.attn_grid : 0;
+  *n_out = n;
+  if (n > cap_ctas) return MURMUR_ERR_INVALID_ARG;
+  MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  if (n > 0)
+    MM_CUDA(c, cudaMemcpy(out, c->view.timeline, (size_t)n * kTimelineWords * 8, cudaMemcpyDeviceToHost));
   return MURMUR_OK;
 }
 
