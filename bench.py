@@ -292,6 +292,10 @@ def run_murmur(args):
         cache.set_option(binding.MURMUR_OPT_ATTN_VARIANT, {"generic": 1, "mma": 2}[args.variant])
     if args.grid:
         cache.set_option(binding.MURMUR_OPT_ATTN_GRID, args.grid)
+    if args.no_pdl:
+        cache.set_option(binding.MURMUR_OPT_PDL, 0)
+    if args.no_fuse:
+        cache.set_option(binding.MURMUR_OPT_FUSE_STEP, 0)
     data = [workloads.SeqData(cfg, i, device=dev) for i in range(B)]
     k_steps, v_steps, q_steps = [], [], []
     for i, s in enumerate(cfg.seqs):
@@ -357,7 +361,11 @@ def run_murmur(args):
     if args.timeline and rank == 0:  # per-CTA trace of the last attention launch of region A (profiling aid)
         tl = cache.attn_timeline().astype(np.int64)
         t_first = int(tl[:, 0].min())
+        tr = cache.step_trace().astype(np.int64)
         with open(args.timeline, "w") as f:
+            f.write("# step prologue stamps (ns relative to the first attention CTA start): append_start %d ticket %d "
+                    "commit %d evict_start %d evict_end %d | last CTA: wait_done %d state_loaded %d prefix %d loads_issued %d "
+                    "tasks %d pages_consumed %d block %d\n" % (tuple(int(x) - t_first for x in tr[:11]) + (int(tr[11]),)))
             f.write("# cta start_ns end_ns smid tiles   (ns relative to the first CTA start)\n")
             for b in range(tl.shape[0]):
                 f.write("%d %d %d %d %d\n" % (b, tl[b, 0] - t_first, tl[b, 1] - t_first if tl[b, 1] else -1, tl[b, 2], tl[b, 3]))
@@ -547,6 +555,8 @@ def main():
     ap.add_argument("--variant", default="", choices=["", "generic", "mma"])
     ap.add_argument("--grid", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-pdl", action="store_true", help="A/B: launch the step's kernels without programmatic dependent launch")
+    ap.add_argument("--no-fuse", action="store_true", help="A/B: murmur_decode_step as three launches (append, evict, attention)")
     ap.add_argument("--timeline", default="", help="write the per-CTA trace of one attention launch to this file")
     ap.add_argument("--cpu-budget-s", default="12")
     ap.add_argument("--ref-budget-s", default="120")

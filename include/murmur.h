@@ -111,6 +111,10 @@ typedef struct {
 /* Options for murmur_set_option. */
 #define MURMUR_OPT_ATTN_VARIANT 1 /* value: MURMUR_ATTN_AUTO / _GENERIC / _MMA */
 #define MURMUR_OPT_ATTN_GRID 2    /* value: CTAs for the persistent attention kernel; 0 = one per SM */
+#define MURMUR_OPT_PDL 3          /* value: 1 (default) = kernels of a step are launched with programmatic
+                                     dependent launch (each waits on-device for its predecessor), 0 = plain */
+#define MURMUR_OPT_FUSE_STEP 4    /* value: 1 (default) = murmur_decode_step runs append + evict as ONE launch
+                                     (the append kernel's last CTA applies the policy), 0 = two launches */
 #define MURMUR_ATTN_AUTO 0    /* tensor-core split-K kernel when page_size >= 16, else generic */
 #define MURMUR_ATTN_GENERIC 1 /* one CTA per (layer, sequence, KV head), FFMA, no smem staging */
 #define MURMUR_ATTN_MMA 2     /* persistent split-K kernel: bulk-copy staging + mma.sync bf16 */
@@ -168,7 +172,9 @@ MURMUR_API murmur_status_t murmur_decode_attn(murmur_cache_t* cache, const int32
                                               int32_t layer_end, float sm_scale, void* stream);
 
 /* One whole decode step from DEVICE buffers: append one token to every listed sequence (all
- * layers) -> evict -> decode_attn, enqueued by ONE host call (PAPER.md:112-116, 136-146, 101-104:
+ * layers) -> evict -> decode_attn, enqueued by ONE host call as TWO launches (the step prologue =
+ * append with the eviction fused into its last CTA, then the attention kernel, which is launched
+ * programmatically dependent so that its set-up overlaps the prologue) (PAPER.md:112-116, 136-146, 101-104:
  * the per-step loop body of Alg. 1 / Alg. 2 followed by Eq. 1).
  *   k_new, v_new : DEVICE bf16 [n_layers][n_seqs][n_kv_heads][head_dim]
  *   q, out       : DEVICE bf16 [n_layers][n_seqs][n_q_heads][head_dim];  lse as above or NULL
@@ -210,10 +216,18 @@ MURMUR_API murmur_status_t murmur_kv_gather(murmur_cache_t* cache, int32_t seq, 
 MURMUR_API murmur_status_t murmur_get_last_error(murmur_cache_t* cache, int32_t* device_err_out, void* stream);
 
 /* Per-CTA trace of the LAST tensor-core attention launch (profiling aid): out is HOST
- * uint64[n][4] = {globaltimer ns at CTA start, at CTA end, SM id, tiles processed}; *n_out = CTAs
+ * uint64[n][4] = {globaltimer ns when the CTA started its work, at CTA end, SM id, tiles processed}; *n_out = CTAs
  * of that launch (0 if the last launch was the generic variant). */
 MURMUR_API murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* cache, uint64_t* out, int32_t cap_ctas,
                                                       int32_t* n_out, void* stream);
+
+/* globaltimer stamps (ns) of the LAST step prologue (profiling aid), HOST uint64[16]:
+ * [0] append kernel start (CTA 0, after its dependency wait)  [1] last append CTA through the ticket
+ * [2] integer state committed  [3] eviction body start  [4] eviction body end;  the last CTA's own
+ * phases: [5] after its dependency wait [6] old state loaded [7] prefix sums done [8] row loads
+ * issued [9] eviction tasks done [10] page ids consumed [11] its block index; rest unused.
+ * Same clock as murmur_debug_attn_timeline. */
+MURMUR_API murmur_status_t murmur_debug_step_trace(murmur_cache_t* cache, uint64_t* out16, void* stream);
 
 /* ---- options / stats --------------------------------------------------------------------- */
 MURMUR_API murmur_status_t murmur_set_option(murmur_cache_t* cache, int32_t option, int32_t value);

@@ -19,6 +19,8 @@ from . import build as _build
 MURMUR_WINDOW_OFF = 0x7FFFFFFF
 MURMUR_OPT_ATTN_VARIANT = 1
 MURMUR_OPT_ATTN_GRID = 2
+MURMUR_OPT_PDL = 3
+MURMUR_OPT_FUSE_STEP = 4
 MURMUR_ATTN_AUTO, MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA = 0, 1, 2
 
 STATUS_NAMES = {0: "MURMUR_OK", 1: "MURMUR_ERR_INVALID_ARG", 2: "MURMUR_ERR_STATE", 3: "MURMUR_ERR_OOM_PAGES",
@@ -30,7 +32,7 @@ EXPORTED_SYMBOLS = [
     "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
     "murmur_decode_step", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
-    "murmur_debug_attn_timeline",
+    "murmur_debug_attn_timeline", "murmur_debug_step_trace",
     "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
     "murmur_last_cuda_error", "murmur_version",
 ]
@@ -94,6 +96,7 @@ def lib() -> C.CDLL:
     L.murmur_kv_gather.argtypes = [vp, i32, vp, i32, i32, i32, vp, vp, vp]
     L.murmur_get_last_error.argtypes = [vp, vp, vp]
     L.murmur_debug_attn_timeline.argtypes = [vp, vp, i32, vp, vp]
+    L.murmur_debug_step_trace.argtypes = [vp, vp, vp]
     L.murmur_set_option.argtypes = [vp, i32, i32]
     L.murmur_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.murmur_reset_stats.argtypes = [vp]
@@ -280,6 +283,12 @@ class MurmurCache:
         n = C.c_int32(0)
         self._check(self.L.murmur_debug_attn_timeline(self.h, a.ctypes.data, 1024, C.byref(n), _stream()))
         return a[: n.value].copy()
+
+    def step_trace(self) -> np.ndarray:
+        """uint64 [16]: globaltimer stamps of the last step prologue (see murmur_debug_step_trace)."""
+        a = np.zeros(16, dtype=np.uint64)
+        self._check(self.L.murmur_debug_step_trace(self.h, a.ctypes.data, _stream()))
+        return a
 
     def set_option(self, option: int, value: int):
         self._check(self.L.murmur_set_option(self.h, option, value))

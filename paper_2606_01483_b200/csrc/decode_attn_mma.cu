@@ -87,6 +87,21 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                    smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
+// Same, with an L2 cache policy.  K/V rows are read once per step and never again before ~575 MB
+// of other rows have gone by: evict_first keeps them from flushing the small hot state (tables,
+// q, the rows the next step appends) out of the 126 MB L2.
+__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, uint32_t bytes, unsigned long long* bar,
+                                              unsigned long long pol) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+      : "memory");
+}
 __device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
   asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
                : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
@@ -115,11 +130,6 @@ __device__ __forceinline__ float ex2(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
-}
-__device__ __forceinline__ unsigned long long globaltimer_ns() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  return t;
 }
 __device__ __forceinline__ unsigned smid() {
   unsigned r;
@@ -175,12 +185,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int n_seqs = list.n, n_kv = c.n_kv, G = c.group;
   unsigned long long* trace = c.timeline + (size_t)blockIdx.x * kTimelineWords;
-  if (tid == 0) {
-    trace[0] = globaltimer_ns();
-    trace[1] = 0ull;
-    trace[2] = smid();
-    trace[3] = 0ull;
-  }
+  pdl_launch_dependents();
 
   // ---- setup: barriers, tile counts, zeroed padding rows of the Q buffers ------------------------
   if (tid == 0) {
@@ -195,8 +200,17 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  for (int i = tid; i < n_seqs; i += kMmaThreads) s.nt[i] = c.seqs[list.ids[i]].n_tiles;
   for (int i = tid; i < 2 * kQBytes / 4; i += kMmaThreads) reinterpret_cast<uint32_t*>(&s.q[0][0])[i] = 0u;
+  // Everything above touches only this CTA's shared memory; from here on the kernel reads what
+  // the step prologue (append + evict) wrote and writes buffers the previous launch may still use.
+  pdl_wait();
+  if (tid == 0) {
+    trace[0] = globaltimer_ns();
+    trace[1] = 0ull;
+    trace[2] = smid();
+    trace[3] = 0ull;
+  }
+  for (int i = tid; i < n_seqs; i += kMmaThreads) s.nt[i] = c.seqs[list.ids[i]].n_tiles;
   __syncthreads();
   if (tid == 0) {
     int acc = 0;
@@ -223,6 +237,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     // Walks its tile range in batches of <= 32 tiles of one item (lane j issues tile j); the
     // descriptors of the NEXT batch are loaded before the current one is issued, so their
     // global-load latency hides behind the copies.
+    const unsigned long long kv_policy = l2_policy_evict_first();
     Cursor cur = locate(s, n_seqs, n_kv, lo);
     long long remaining = hi - lo;  // tiles left, counted from the start of the current item's segment
     int seg = (int)min((long long)(s.nt[cur.i] - cur.k), remaining);
@@ -279,7 +294,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
                 const int r0 = (pg == 0) ? td.row_begin : pg * c.p;
                 const int r1 = (pg == td.n_pages - 1) ? td.row_end : (pg + 1) * c.p;
                 const uint8_t* src = pool + row_offset(c, layer, td.page[pg], cur.h, r0 - pg * c.p);
-                bulk_g2s(&s.kv[st][kv][r0 * kRowBytes], src, (uint32_t)(r1 - r0) * kRowBytes, bar);
+                bulk_g2s_hint(&s.kv[st][kv][r0 * kRowBytes], src, (uint32_t)(r1 - r0) * kRowBytes, bar, kv_policy);
               }
             }
           }
@@ -599,7 +614,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 
 cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                             void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
-                            cudaStream_t st, LaunchInfo* info) {
+                            bool pdl, cudaStream_t st, LaunchInfo* info) {
   static bool attr_set = false;
   const int smem = (int)sizeof(SmemLayout);
   if (!attr_set) {
@@ -617,11 +632,11 @@ cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_bas
   prm.layer_begin = layer_begin;
   prm.n_layers_call = layer_end - layer_begin;
   prm.sm_scale = sm_scale;
-  attn_mma_kernel<<<grid, kMmaThreads, smem, st>>>(c, list, prm);
+  PdlLaunch l(dim3((unsigned)grid), dim3(kMmaThreads), (size_t)smem, st, pdl);
   info->launches += 1;
   info->grid = grid;
   info->smem = smem;
-  return cudaGetLastError();
+  return cudaLaunchKernelEx(&l.cfg, attn_mma_kernel, c, list, prm);
 }
 
 }  // namespace murmur

@@ -25,6 +25,7 @@ constexpr int kMaxSeqsPerLaunch = 128;
 constexpr int kOStride = 132;            // floats per head row in split-K partials / merge scratch
 constexpr int kPartialFloats = kMaxGroup * kOStride + 2 * kMaxGroup;  // o[8][132] + m[8] + l[8]
 constexpr int kMaxAttnGrid = 1024;       // upper bound on CTAs of the persistent attention kernel
+constexpr int kStepTraceWords = 16;      // globaltimer stamps of the step prologue (after the per-CTA entries)
 constexpr int kTimelineWords = 4;        // globaltimer at CTA start, at CTA end, SM id, tiles processed
 
 // ctrl word indices
@@ -68,6 +69,22 @@ struct CacheView {
   unsigned long long* timeline;  // [kMaxAttnGrid][kTimelineWords] per-CTA trace of the last attention launch
 };
 
+#ifdef __CUDACC__
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+// Step-prologue trace (profiling aid): word k of the block behind the per-CTA attention entries.
+// 0 append start (CTA 0, after the dependency wait)   1 last append CTA passed the ticket
+// 2 commit done   3 evict body start   4 evict body end
+// 5.. the last CTA's own phases: 5 after its dependency wait, 6 old state loaded, 7 prefix sums
+// done, 8 row loads issued, 9 eviction tasks done, 10 page ids consumed, 11 block index
+__device__ __forceinline__ void step_stamp(const CacheView& c, int k) {
+  c.timeline[(size_t)kMaxAttnGrid * kTimelineWords + k] = globaltimer_ns();
+}
+#endif
+
 struct SeqList {  // per-launch sequence list, passed by value (no H2D copy, graph-capturable)
   int32_t n;
   int32_t ids[kMaxSeqsPerLaunch];
@@ -91,6 +108,35 @@ __device__ __forceinline__ SeqParams load_params(const SeqDev& s) {
   return r;
 }
 
+// ---- programmatic dependent launch (PDL) ------------------------------------------------------
+// Every kernel of the decode step starts with pdl_launch_dependents() (the next kernel of the
+// stream may become resident and run its prologue) and calls pdl_wait() before its first access
+// to memory another kernel of the stream may have written - or may still be reading, for data it
+// is about to overwrite.  griddepcontrol.wait returns when ALL prerequisite grids have completed
+// and flushed, so the ordering is that of ordinary stream serialisation; only launch latency and
+// kernel prologues overlap.  Both are no-ops when the kernel was launched without the attribute.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+#endif
+
+// Launch configuration helper: sets the programmatic-stream-serialisation attribute when `pdl`.
+struct PdlLaunch {
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[1];
+  PdlLaunch(dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl) {
+    cfg = cudaLaunchConfig_t{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+  }
+};
+
 // ---- host launchers (one per .cu) ------------------------------------------------------------
 struct LaunchInfo {
   int launches;   // kernels launched
@@ -102,15 +148,15 @@ cudaError_t launch_init(const CacheView& c, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_seq_begin(const CacheView& c, int seq, const SeqParams& sp, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_seq_end(const CacheView& c, int seq, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_append(const CacheView& c, const AppendList& list, int total_tokens, const void* k_new,
-                          const void* v_new, int layer_begin, int layer_end, bool reserve, int sm_count,
-                          cudaStream_t st, LaunchInfo* info);
-cudaError_t launch_evict(const CacheView& c, const SeqList& list, cudaStream_t st, LaunchInfo* info);
+                          const void* v_new, int layer_begin, int layer_end, bool reserve, bool fuse_evict,
+                          int sm_count, bool pdl, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_evict(const CacheView& c, const SeqList& list, bool pdl, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_attn_generic(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total,
                                 const void* q, void* out, float* lse, int layer_begin, int layer_end,
                                 float sm_scale, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                             void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
-                            cudaStream_t st, LaunchInfo* info);
+                            bool pdl, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_expand_retained(const CacheView& c, int seq, int32_t* pos_out_dev, int cap, cudaStream_t st,
                                    LaunchInfo* info);
 cudaError_t launch_gather(const CacheView& c, int seq, const int32_t* positions_dev, int n, int layer_begin,

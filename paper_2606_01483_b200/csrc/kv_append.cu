@@ -6,7 +6,10 @@
 // from the top of the free stack in call order (C3) - scatters its share of the rows
 // into the pre-swizzled pools, and the LAST CTA to finish (ticket counter) commits the new
 // lengths, block-table entries and free-stack height.  No host sync, graph-capturable.
-#include "device_state.cuh"
+// With fuse_evict (the decode-step prologue) the eviction for the same sequences rides along:
+// its table products are computed by warps of all CTAs before the ticket, and the last CTA only
+// frees the dead pages after the commit - append -> evict is one launch.
+#include "evict_body.cuh"
 
 namespace murmur {
 namespace {
@@ -74,102 +77,239 @@ __global__ void seq_end_kernel(CacheView c, int seq) {
 }
 
 // ---- append -----------------------------------------------------------------------------------
-constexpr int kAppendThreads = 256;
+constexpr int kAppendThreads = 256;  // small enough to be co-resident with an attention CTA (registers)
+
+// One half-warp moves one 256-byte row (16 lanes x 16 bytes).  Unit u of a call = (K|V, layer, token, head).
+struct RowUnit {
+  const uint4* src;
+  int page;              // loaded, not yet consumed: dst() is the first use
+  int layer, head, slot, sub, is_v;
+  __device__ __forceinline__ uint4* dst(const CacheView& c) const {
+    // pre-swizzled row (see device_state.cuh)
+    uint8_t* pool = reinterpret_cast<uint8_t*>(is_v ? c.v_pool : c.k_pool);
+    return reinterpret_cast<uint4*>(pool + row_offset(c, layer, page, head, slot)) + (sub ^ (slot & 7));
+  }
+};
+
+__device__ __forceinline__ RowUnit locate_row(const CacheView& c, const AppendList& list, long long u, long long rows_src,
+                                              int total_tokens, int layer_begin, int n, int free_top, int sub,
+                                              const uint4* k_new, const uint4* v_new, const int* s_tok_off,
+                                              const int* s_blk_off, const int* s_old_nblk, const SeqParams* s_sp) {
+  const int is_v = u >= rows_src;
+  const long long r = is_v ? u - rows_src : u;
+  int head, tau, layer;
+  if (rows_src < 0x7fffffffLL) {  // 32-bit index arithmetic (64-bit division is ~100 instructions)
+    const unsigned r32 = (unsigned)r, r2 = r32 / (unsigned)c.n_kv;
+    head = (int)(r32 - r2 * (unsigned)c.n_kv);
+    const unsigned lq = r2 / (unsigned)total_tokens;
+    tau = (int)(r2 - lq * (unsigned)total_tokens);
+    layer = layer_begin + (int)lq;
+  } else {
+    head = (int)(r % c.n_kv);
+    const long long r2 = r / c.n_kv;
+    tau = (int)(r2 % total_tokens);
+    layer = layer_begin + (int)(r2 / total_tokens);
+  }
+  int lo = 0, hi = n - 1;  // largest i with s_tok_off[i] <= tau
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (s_tok_off[mid] <= tau) lo = mid; else hi = mid - 1;
+  }
+  const int i = lo;
+  const int x = s_sp[i].len + (tau - s_tok_off[i]);
+  const int b = x >> c.p_log2;
+  const int slot = x & (c.p - 1);
+  RowUnit ru;
+  if (b < s_old_nblk[i]) ru.page = c.block_table[(size_t)list.ids[i] * c.max_blocks + b];
+  else ru.page = c.free_stack[free_top - 1 - (s_blk_off[i] + (b - s_old_nblk[i]))];
+  ru.src = (is_v ? v_new : k_new) + r * 16 + sub;
+  ru.layer = layer; ru.head = head; ru.slot = slot; ru.sub = sub; ru.is_v = is_v;
+  return ru;
+}
+
+// Block -> page as the eviction tasks of the fused prologue see it: blocks the append is about to
+// map are not in the table yet (the commit comes after the ticket) - their pages are the ones the
+// append pops, free_stack[top - (b - old_nblk)].
+struct StepLookup {
+  const int32_t* tab;
+  const int32_t* free_stack;
+  int old_nblk, top;
+  __device__ __forceinline__ int operator()(int b) const { return b < old_nblk ? tab[b] : free_stack[top - (b - old_nblk)]; }
+};
+
+// Products 1 and 2 of the eviction (evict_body.cuh) for the post-append state, spread over the
+// warps of ALL CTAs; they read only state that nothing rewrites before the ticket.
+__device__ __forceinline__ void fused_evict_tasks(const CacheView& c, const AppendList& list, int n, int free_top,
+                                                  const SeqParams* s_sp, const int* s_blk_off, const int* s_old_nblk) {
+  const int warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  for (int task = (int)blockIdx.x + (int)gridDim.x * warp; task < 2 * n; task += (int)gridDim.x * n_warps) {
+    const int role = 1 + task / n, i = task % n;
+    SeqParams sp = s_sp[i];
+    sp.len += list.n_tok[i];
+    const StepLookup lk{c.block_table + (size_t)list.ids[i] * c.max_blocks, c.free_stack, s_old_nblk[i],
+                        free_top - 1 - s_blk_off[i]};
+    evict_task(c, list.ids[i], sp, role, lk);
+  }
+}
 
 __global__ void __launch_bounds__(kAppendThreads)
-append_kernel(CacheView c, AppendList list, int total_tokens, const uint4* __restrict__ k_new,
-              const uint4* __restrict__ v_new, int layer_begin, int n_layers_call, int reserve) {
+append_kernel(const __grid_constant__ CacheView c, const __grid_constant__ AppendList list, int total_tokens,
+              const uint4* __restrict__ k_new, const uint4* __restrict__ v_new, int layer_begin, int n_layers_call,
+              int reserve, int fuse_evict) {
   __shared__ int s_tok_off[kMaxSeqsPerLaunch + 1];
   __shared__ int s_blk_off[kMaxSeqsPerLaunch + 1];
-  __shared__ int s_old_len[kMaxSeqsPerLaunch];
   __shared__ int s_old_nblk[kMaxSeqsPerLaunch];
+  __shared__ int s_ndead[kMaxSeqsPerLaunch];
+  __shared__ int s_off[kMaxSeqsPerLaunch + 1];
+  __shared__ SeqParams s_sp[kMaxSeqsPerLaunch];  // .len = fill level BEFORE this call's tokens
   __shared__ int s_flag;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, n_threads = blockDim.x;
   const int n = list.n;
+  pdl_launch_dependents();
+  pdl_wait();  // the previous kernel may still be reading the tables this one rewrites
+  if (blockIdx.x == 0 && tid == 0) step_stamp(c, 0);
+  const unsigned long long t_wait = globaltimer_ns();
   const int free_top = c.ctrl[kCtrlFreeTop];
 
   // Phase A: per-sequence old fill level and new-block demand (same result in every CTA).
-  if (tid < n) {
-    const SeqDev& s = c.seqs[list.ids[tid]];
-    const int old_len = reserve ? s.len : s.len - list.n_tok[tid];
-    s_old_len[tid] = old_len;
-    s_old_nblk[tid] = (old_len + c.p - 1) >> c.p_log2;
-    if (!s.active || old_len < 0) set_error(c, 2);
+  for (int i = tid; i < n; i += n_threads) {
+    const SeqDev& s = c.seqs[list.ids[i]];
+    SeqParams sp = load_params(s);
+    if (!reserve) sp.len -= list.n_tok[i];
+    if (!s.active || sp.len < 0) set_error(c, 2);
+    s_sp[i] = sp;
+    s_old_nblk[i] = (max(sp.len, 0) + c.p - 1) >> c.p_log2;
   }
   __syncthreads();
-  if (tid == 0) {  // exclusive prefix sums over <= 128 sequences, in call order
-    int tok = 0, blk = 0, bad = 0;
-    for (int i = 0; i < n; ++i) {
-      s_tok_off[i] = tok;
-      s_blk_off[i] = blk;
-      const int new_len = s_old_len[i] + list.n_tok[i];
-      const int new_nblk = (new_len + c.p - 1) >> c.p_log2;
-      if (new_nblk > c.max_blocks) bad = 1;
-      tok += list.n_tok[i];
-      blk += new_nblk - s_old_nblk[i];
+  const unsigned long long t_ld = globaltimer_ns();
+  if (tid < 32) {  // exclusive prefix sums over <= 128 sequences, in call order: 4 per lane + warp scan
+    int tok4[4], blk4[4], tok = 0, blk = 0, bad = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int i = tid * 4 + k;
+      tok4[k] = tok;
+      blk4[k] = blk;
+      if (i < n) {
+        const int new_len = s_sp[i].len + list.n_tok[i];
+        const int new_nblk = (new_len + c.p - 1) >> c.p_log2;
+        if (new_nblk > c.max_blocks || s_sp[i].len < 0) bad = 1;
+        tok += list.n_tok[i];
+        blk += new_nblk - s_old_nblk[i];
+      }
     }
-    s_tok_off[n] = tok;
-    s_blk_off[n] = blk;
-    int ok = 1;
-    if (bad) { set_error(c, 2); ok = 0; }
-    if (reserve && blk > free_top) { set_error(c, 3); ok = 0; }  // all-or-nothing
-    if (tok != total_tokens) { set_error(c, 1); ok = 0; }
-    s_flag = ok;
+    int tok_inc = tok, blk_inc = blk;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t2 = __shfl_up_sync(0xffffffffu, tok_inc, o), b2 = __shfl_up_sync(0xffffffffu, blk_inc, o);
+      if (tid >= o) { tok_inc += t2; blk_inc += b2; }
+    }
+    const int tok_ex = tok_inc - tok, blk_ex = blk_inc - blk;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int i = tid * 4 + k;
+      if (i < n) {
+        s_tok_off[i] = tok_ex + tok4[k];
+        s_blk_off[i] = blk_ex + blk4[k];
+      }
+    }
+    bad = __any_sync(0xffffffffu, bad);
+    const int tok_all = __shfl_sync(0xffffffffu, tok_inc, 31), blk_all = __shfl_sync(0xffffffffu, blk_inc, 31);
+    if (tid == 0) {
+      s_tok_off[n] = tok_all;
+      s_blk_off[n] = blk_all;
+      int ok = 1;
+      if (bad) { set_error(c, 2); ok = 0; }
+      if (reserve && blk_all > free_top) { set_error(c, 3); ok = 0; }  // all-or-nothing
+      if (tok_all != total_tokens) { set_error(c, 1); ok = 0; }
+      s_flag = ok;
+    }
   }
   __syncthreads();
   if (!s_flag) return;
+  const unsigned long long t_a = globaltimer_ns();
 
-  // Phase B: scatter rows.  One half-warp moves one 256-byte row (16 lanes x 16 bytes).
+  // Phase B: scatter rows.  The integer state may be committed as soon as every CTA has READ what
+  // it needs of the old state (page ids); the rows themselves only have to land before the kernel
+  // ends.  When the whole call is one pass over the grid (a decode step), each thread therefore
+  // looks its page up, the CTA takes its ticket, and the row is stored afterwards - so the last
+  // CTA's commit (+ eviction) overlaps the other CTAs' stores.
   const int sub = tid & 15;
+  const int units_per_cta = n_threads >> 4;
   const long long rows_src = (long long)n_layers_call * total_tokens * c.n_kv;  // per K / per V
   const long long units = 2 * rows_src;
-  const long long unit_stride = (long long)gridDim.x * (kAppendThreads / 16);
-  for (long long u = (long long)blockIdx.x * (kAppendThreads / 16) + (tid >> 4); u < units; u += unit_stride) {
-    const int is_v = u >= rows_src;
-    const long long r = is_v ? u - rows_src : u;
-    const int head = (int)(r % c.n_kv);
-    const long long r2 = r / c.n_kv;
-    const int tau = (int)(r2 % total_tokens);
-    const int layer = layer_begin + (int)(r2 / total_tokens);
-    int lo = 0, hi = n - 1;  // largest i with s_tok_off[i] <= tau
-    while (lo < hi) {
-      const int mid = (lo + hi + 1) >> 1;
-      if (s_tok_off[mid] <= tau) lo = mid; else hi = mid - 1;
+  const long long unit_stride = (long long)gridDim.x * units_per_cta;
+  const bool one_pass = units <= unit_stride;
+  int bad_page = 0;
+  unsigned long long t_b = 0, t_l = 0, t_t = 0;
+  if (one_pass) {
+    const long long u = (long long)blockIdx.x * units_per_cta + (tid >> 4);
+    RowUnit ru;
+    ru.page = 0;
+    uint4 val = make_uint4(0u, 0u, 0u, 0u);
+    if (u < units) {
+      ru = locate_row(c, list, u, rows_src, total_tokens, layer_begin, n, free_top, sub, k_new, v_new, s_tok_off,
+                      s_blk_off, s_old_nblk, s_sp);
+      val = *ru.src;
     }
-    const int i = lo;
-    const int x = s_old_len[i] + (tau - s_tok_off[i]);
-    const int b = x >> c.p_log2;
-    const int slot = x & (c.p - 1);
-    int page;
-    if (b < s_old_nblk[i]) page = c.block_table[(size_t)list.ids[i] * c.max_blocks + b];
-    else page = c.free_stack[free_top - 1 - (s_blk_off[i] + (b - s_old_nblk[i]))];
-    const uint4 val = (is_v ? v_new : k_new)[r * 16 + sub];
-    uint8_t* pool = reinterpret_cast<uint8_t*>(is_v ? c.v_pool : c.k_pool);
-    uint4* dst = reinterpret_cast<uint4*>(pool + row_offset(c, layer, page, head, slot));
-    dst[sub ^ (slot & 7)] = val;  // pre-swizzled row (see device_state.cuh)
+    t_l = globaltimer_ns();
+    if (fuse_evict) {
+      fused_evict_tasks(c, list, n, free_top, s_sp, s_blk_off, s_old_nblk);
+      // every CTA also counts the blocks the eviction will free (the dead ranges at the new
+      // lengths; nothing remaps them before the ticket), so that the last CTA can push at once
+      evict_count(c, list.ids, n, s_sp, list.n_tok, s_ndead);
+    }
+    t_t = globaltimer_ns();
+    // the barrier consumes every thread's page id: all of this CTA's reads of the old state are done
+    bad_page = __syncthreads_or(ru.page < 0);
+    t_b = globaltimer_ns();
+    if (reserve) {
+      if (tid == 0) s_flag = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
+      __syncthreads();
+    }
+    if (u < units && ru.page >= 0) *ru.dst(c) = val;
+  } else {
+    for (long long u = (long long)blockIdx.x * units_per_cta + (tid >> 4); u < units; u += unit_stride) {
+      const RowUnit ru = locate_row(c, list, u, rows_src, total_tokens, layer_begin, n, free_top, sub, k_new, v_new,
+                                    s_tok_off, s_blk_off, s_old_nblk, s_sp);
+      if (ru.page >= 0) *ru.dst(c) = *ru.src; else bad_page = 1;
+    }
+    if (fuse_evict) fused_evict_tasks(c, list, n, free_top, s_sp, s_blk_off, s_old_nblk);
+    bad_page = __syncthreads_or(bad_page);  // every store above has consumed its page id
+    if (reserve) {
+      if (tid == 0) s_flag = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
+      __syncthreads();
+    }
   }
-  if (!reserve) return;
+  if (bad_page && tid == 0) set_error(c, 2);
+  if (!reserve || !s_flag) return;
+  if (tid == 0) {
+    unsigned long long* tr = c.timeline + (size_t)kMaxAttnGrid * kTimelineWords;
+    tr[5] = t_wait; tr[6] = t_ld; tr[7] = t_a; tr[8] = t_l; tr[9] = t_t; tr[10] = t_b; tr[11] = blockIdx.x;
+  }
 
-  // Phase C: the last CTA to finish commits the new integer state.
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_flag = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
-  __syncthreads();
-  if (!s_flag) return;
-  __threadfence();
-  for (int i = tid; i < n; i += kAppendThreads) {
+  // Phase C: the last CTA through the ticket commits the new integer state.
+  if (tid == 0) step_stamp(c, 1);
+  for (int i = tid; i < n; i += n_threads) {
     SeqDev& s = c.seqs[list.ids[i]];
-    const int new_len = s_old_len[i] + list.n_tok[i];
+    const int new_len = s_sp[i].len + list.n_tok[i];
     const int new_nblk = (new_len + c.p - 1) >> c.p_log2;
     int32_t* tab = c.block_table + (size_t)list.ids[i] * c.max_blocks;
     for (int b = s_old_nblk[i]; b < new_nblk; ++b)
       tab[b] = c.free_stack[free_top - 1 - (s_blk_off[i] + (b - s_old_nblk[i]))];
     s.len = new_len;
+    s_sp[i].len = new_len;
   }
+  const int free_top_new = free_top - s_blk_off[n];
   if (tid == 0) {
-    c.ctrl[kCtrlFreeTop] = free_top - s_blk_off[n];
+    c.ctrl[kCtrlFreeTop] = free_top_new;
     c.ctrl[kCtrlAppendTicket] = 0;
+    step_stamp(c, 2);
   }
+  if (!fuse_evict) return;
+  __syncthreads();  // the committed lengths and table entries, CTA-wide
+  if (tid == 0) step_stamp(c, 3);
+  evict_free(c, list.ids, n, s_sp, free_top_new, s_ndead, s_off, /*counted=*/one_pass);
+  if (tid == 0) step_stamp(c, 4);
 }
 
 // ---- introspection helpers ------------------------------------------------------------------------
@@ -233,20 +373,22 @@ cudaError_t launch_seq_end(const CacheView& c, int seq, cudaStream_t st, LaunchI
 }
 
 cudaError_t launch_append(const CacheView& c, const AppendList& list, int total_tokens, const void* k_new,
-                          const void* v_new, int layer_begin, int layer_end, bool reserve, int sm_count,
-                          cudaStream_t st, LaunchInfo* info) {
+                          const void* v_new, int layer_begin, int layer_end, bool reserve, bool fuse_evict,
+                          int sm_count, bool pdl, cudaStream_t st, LaunchInfo* info) {
   const int n_layers_call = layer_end - layer_begin;
   const long long units = 2LL * n_layers_call * total_tokens * c.n_kv;
-  long long grid = (units + (kAppendThreads / 16) - 1) / (kAppendThreads / 16);
-  const long long cap = (long long)sm_count * 8;
+  const bool fused = reserve && fuse_evict;
+  const int threads = kAppendThreads;
+  long long grid = (units + (threads / 16) - 1) / (threads / 16);
+  const long long cap = (long long)sm_count * (2048 / threads);
   if (grid > cap) grid = cap;
   if (grid < 1) grid = 1;
-  append_kernel<<<(int)grid, kAppendThreads, 0, st>>>(c, list, total_tokens, reinterpret_cast<const uint4*>(k_new),
-                                                      reinterpret_cast<const uint4*>(v_new), layer_begin,
-                                                      n_layers_call, reserve ? 1 : 0);
+  PdlLaunch l(dim3((unsigned)grid), dim3((unsigned)threads), 0, st, pdl);
   info->launches += 1;
   info->grid = (int)grid;
-  return cudaGetLastError();
+  return cudaLaunchKernelEx(&l.cfg, append_kernel, c, list, total_tokens, reinterpret_cast<const uint4*>(k_new),
+                            reinterpret_cast<const uint4*>(v_new), layer_begin, n_layers_call, reserve ? 1 : 0,
+                            fused ? 1 : 0);
 }
 
 cudaError_t launch_expand_retained(const CacheView& c, int seq, int32_t* pos_out_dev, int cap, cudaStream_t st,

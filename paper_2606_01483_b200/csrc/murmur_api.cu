@@ -67,7 +67,7 @@ Carve carve(const murmur_cache_desc_t* d) {
   c.ctrl = take(kCtrlWords * 4);
   c.counters = take((size_t)d->n_layers * kMaxSeqsPerLaunch * d->n_kv_heads * 4);
   c.partials = take((size_t)2 * kMaxAttnGrid * kPartialFloats * 4);
-  c.timeline = take((size_t)kMaxAttnGrid * kTimelineWords * 8);
+  c.timeline = take(((size_t)kMaxAttnGrid * kTimelineWords + kStepTraceWords) * 8);
   c.stage_seqs = d->max_seqs < kMaxSeqsPerLaunch ? d->max_seqs : kMaxSeqsPerLaunch;
   const size_t kv_b = (size_t)d->n_layers * c.stage_seqs * d->n_kv_heads * kRowBytes;
   const size_t q_b = (size_t)d->n_layers * c.stage_seqs * d->n_q_heads * kRowBytes;
@@ -92,6 +92,8 @@ struct murmur_cache {
   int sm_count;
   int attn_variant_opt;
   int attn_grid_opt;
+  int pdl_opt;         // programmatic dependent launch between the kernels of a step
+  int fuse_step_opt;   // murmur_decode_step: append + evict in one launch
   murmur_stats_t stats;
   cudaError_t last_cuda;
   uint8_t* ws;
@@ -157,6 +159,8 @@ murmur_status_t murmur_cache_create(const murmur_cache_desc_t* d, murmur_cache_t
   c->free_pages = d->n_pages;
   c->attn_variant_opt = MURMUR_ATTN_AUTO;
   c->attn_grid_opt = 0;
+  c->pdl_opt = 1;
+  c->fuse_step_opt = 1;
   std::memset(&c->stats, 0, sizeof c->stats);
   c->last_cuda = cudaSuccess;
   int dev = 0;
@@ -242,9 +246,24 @@ murmur_status_t murmur_seq_end(murmur_cache_t* c, int32_t seq, void* stream) {
   return MURMUR_OK;
 }
 
-murmur_status_t murmur_kv_append(murmur_cache_t* c, const int32_t* seq_ids, const int32_t* n_tokens, int32_t n_seqs,
-                                 const void* k_new, const void* v_new, int32_t layer_begin, int32_t layer_end,
-                                 void* stream) {
+// Host mirror of what an evict at the sequences' current lengths frees (closed form).
+static void mirror_evict(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs) {
+  for (int i = 0; i < n_seqs; ++i) {
+    HostSeq& hs = c->seqs[seq_ids[i]];
+    const int32_t dead = dead_block_count(hs.sp, c->desc.page_size);
+    c->free_pages += dead - hs.freed_blocks;
+    hs.freed_blocks = dead;
+    hs.evict_len = hs.sp.len;
+  }
+  c->stats.free_pages = c->free_pages;
+  c->stats.evict_calls += 1;
+}
+
+// fuse_evict: the append kernel's last CTA also runs the eviction body for the same sequences
+// (single launch of <= 128 sequences, layer_begin == 0 only).
+static murmur_status_t append_impl(murmur_cache_t* c, const int32_t* seq_ids, const int32_t* n_tokens, int32_t n_seqs,
+                                   const void* k_new, const void* v_new, int32_t layer_begin, int32_t layer_end,
+                                   bool fuse_evict, void* stream) {
   if (!c || !n_tokens) return MURMUR_ERR_INVALID_ARG;
   murmur_status_t st = check_ids(c, seq_ids, n_seqs);
   if (st != MURMUR_OK) return st;
@@ -285,7 +304,7 @@ murmur_status_t murmur_kv_append(murmur_cache_t* c, const int32_t* seq_ids, cons
       if (base == 0 && list.n == n_seqs) {
         LaunchInfo li{};
         MM_CUDA(c, launch_append(c->view, list, (int)chunk_tok, k_new, v_new, layer_begin, layer_end, reserve,
-                                 c->sm_count, (cudaStream_t)stream, &li));
+                                 fuse_evict, c->sm_count, c->pdl_opt != 0, (cudaStream_t)stream, &li));
         note(c, li);
       } else {
         // several chunks: the source is [layer][all tokens][...], so each layer is its own launch
@@ -294,7 +313,8 @@ murmur_status_t murmur_kv_append(murmur_cache_t* c, const int32_t* seq_ids, cons
           LaunchInfo li{};
           MM_CUDA(c, launch_append(c->view, list, (int)chunk_tok, (const uint8_t*)k_new + off,
                                    (const uint8_t*)v_new + off, layer, layer + 1,
-                                   reserve && layer == layer_begin, c->sm_count, (cudaStream_t)stream, &li));
+                                   reserve && layer == layer_begin, false, c->sm_count, c->pdl_opt != 0,
+                                   (cudaStream_t)stream, &li));
           note(c, li);
         }
       }
@@ -307,7 +327,14 @@ murmur_status_t murmur_kv_append(murmur_cache_t* c, const int32_t* seq_ids, cons
     c->stats.free_pages = c->free_pages;
   }
   c->stats.append_calls += 1;
+  if (fuse_evict) mirror_evict(c, seq_ids, n_seqs);
   return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_append(murmur_cache_t* c, const int32_t* seq_ids, const int32_t* n_tokens, int32_t n_seqs,
+                                 const void* k_new, const void* v_new, int32_t layer_begin, int32_t layer_end,
+                                 void* stream) {
+  return append_impl(c, seq_ids, n_tokens, n_seqs, k_new, v_new, layer_begin, layer_end, false, stream);
 }
 
 murmur_status_t murmur_kv_evict(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, void* stream) {
@@ -319,18 +346,10 @@ murmur_status_t murmur_kv_evict(murmur_cache_t* c, const int32_t* seq_ids, int32
     list.n = (n_seqs - base) < kMaxSeqsPerLaunch ? (n_seqs - base) : kMaxSeqsPerLaunch;
     for (int i = 0; i < list.n; ++i) list.ids[i] = seq_ids[base + i];
     LaunchInfo li{};
-    MM_CUDA(c, launch_evict(c->view, list, (cudaStream_t)stream, &li));
+    MM_CUDA(c, launch_evict(c->view, list, c->pdl_opt != 0, (cudaStream_t)stream, &li));
     note(c, li);
   }
-  for (int i = 0; i < n_seqs; ++i) {
-    HostSeq& hs = c->seqs[seq_ids[i]];
-    const int32_t dead = dead_block_count(hs.sp, c->desc.page_size);
-    c->free_pages += dead - hs.freed_blocks;
-    hs.freed_blocks = dead;
-    hs.evict_len = hs.sp.len;
-  }
-  c->stats.free_pages = c->free_pages;
-  c->stats.evict_calls += 1;
+  mirror_evict(c, seq_ids, n_seqs);
   return MURMUR_OK;
 }
 
@@ -359,7 +378,7 @@ murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, in
     LaunchInfo li{};
     if (variant == MURMUR_ATTN_MMA) {
       MM_CUDA(c, launch_attn_mma(c->view, list, base, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, grid,
-                                 (cudaStream_t)stream, &li));
+                                 c->pdl_opt != 0, (cudaStream_t)stream, &li));
     } else {
       MM_CUDA(c, launch_attn_generic(c->view, list, base, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale,
                                      (cudaStream_t)stream, &li));
@@ -397,10 +416,13 @@ murmur_status_t murmur_decode_step(murmur_cache_t* c, const int32_t* seq_ids, in
   if (st != MURMUR_OK) return st;
   int32_t ones[kMaxSeqsPerLaunch];
   for (int i = 0; i < n_seqs; ++i) ones[i] = 1;
-  st = murmur_kv_append(c, seq_ids, ones, n_seqs, k_new, v_new, 0, c->desc.n_layers, stream);
+  const bool fuse = c->fuse_step_opt != 0;  // n_seqs <= 128 (check_step): one append launch
+  st = append_impl(c, seq_ids, ones, n_seqs, k_new, v_new, 0, c->desc.n_layers, fuse, stream);
   if (st != MURMUR_OK) return st;
-  st = murmur_kv_evict(c, seq_ids, n_seqs, stream);
-  if (st != MURMUR_OK) return st;
+  if (!fuse) {
+    st = murmur_kv_evict(c, seq_ids, n_seqs, stream);
+    if (st != MURMUR_OK) return st;
+  }
   return murmur_decode_attn(c, seq_ids, n_seqs, q, out, lse, 0, c->desc.n_layers, sm_scale, stream);
 }
 
@@ -566,6 +588,14 @@ murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* c, uint64_t* out, int
   return MURMUR_OK;
 }
 
+murmur_status_t murmur_debug_step_trace(murmur_cache_t* c, uint64_t* out16, void* stream) {
+  if (!c || !out16) return MURMUR_ERR_INVALID_ARG;
+  MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  MM_CUDA(c, cudaMemcpy(out16, c->view.timeline + (size_t)kMaxAttnGrid * kTimelineWords, kStepTraceWords * 8,
+                        cudaMemcpyDeviceToHost));
+  return MURMUR_OK;
+}
+
 murmur_status_t murmur_set_option(murmur_cache_t* c, int32_t option, int32_t value) {
   if (!c) return MURMUR_ERR_INVALID_ARG;
   switch (option) {
@@ -576,6 +606,12 @@ murmur_status_t murmur_set_option(murmur_cache_t* c, int32_t option, int32_t val
     case MURMUR_OPT_ATTN_GRID:
       if (value < 0 || value > kMaxAttnGrid) return MURMUR_ERR_INVALID_ARG;
       c->attn_grid_opt = value;
+      return MURMUR_OK;
+    case MURMUR_OPT_PDL:
+      c->pdl_opt = value != 0;
+      return MURMUR_OK;
+    case MURMUR_OPT_FUSE_STEP:
+      c->fuse_step_opt = value != 0;
       return MURMUR_OK;
     default:
       return MURMUR_ERR_INVALID_ARG;

@@ -101,6 +101,13 @@ MM_HD void blocks_inside(const Interval& iv, int32_t p, int32_t* lo, int32_t* hi
   if (*hi < *lo) *hi = *lo;
 }
 
+// Same for p = 2^plog (device code: no integer division on the step's critical path).
+MM_HD void blocks_inside_log2(const Interval& iv, int32_t plog, int32_t* lo, int32_t* hi) {
+  *lo = (iv.a + (1 << plog) - 1) >> plog;
+  *hi = iv.b >> plog;
+  if (*hi < *lo) *hi = *lo;
+}
+
 // Number of blocks that are dead (hence freed by an evict) when the policy is applied at the
 // current fill level.
 MM_HD int32_t dead_block_count(const SeqParams& s, int32_t p) {

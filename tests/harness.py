@@ -118,6 +118,26 @@ class SideBySide:
         self.gpu.kv_evict(seq_ids)
         self.oracle.evict(seq_ids)
 
+    def fused_step(self, seq_ids: Sequence[int], want_lse: bool = False):
+        """One whole decode step through murmur_decode_step (prologue = append+evict, attention);
+        the oracle side does append -> evict.  Returns (q, out, lse)."""
+        ks, vs = [], []
+        for i in seq_ids:
+            u = self.t_of(i)
+            k, v = self.data[i].out_kv(u, u + 1)
+            ks.append(k)
+            vs.append(v)
+            self._store(i, k, v)
+        k_new = torch.cat(ks, dim=1).contiguous()
+        v_new = torch.cat(vs, dim=1).contiguous()
+        self.oracle.append(seq_ids, [1] * len(seq_ids))
+        self.oracle.evict(seq_ids)
+        q = self.queries(seq_ids)
+        out = torch.empty_like(q)
+        lse = torch.empty(q.shape[:3], dtype=torch.float32, device=self.device) if want_lse else None
+        self.gpu.decode_step(seq_ids, k_new, v_new, q, out, lse, self.scale)
+        return q, out, lse
+
     def queries(self, seq_ids: Sequence[int]) -> torch.Tensor:
         """[L, n_seqs, n_q, d]: query of each sequence's newest output token."""
         qs = [self.data[i].q_step(max(1, self.t_of(i))) for i in seq_ids]
