@@ -296,6 +296,8 @@ def run_murmur(args):
         cache.set_option(binding.MURMUR_OPT_PDL, 0)
     if args.no_fuse:
         cache.set_option(binding.MURMUR_OPT_FUSE_STEP, 0)
+    elif args.fuse >= 0:
+        cache.set_option(binding.MURMUR_OPT_FUSE_STEP, args.fuse)
     data = [workloads.SeqData(cfg, i, device=dev) for i in range(B)]
     k_steps, v_steps, q_steps = [], [], []
     for i, s in enumerate(cfg.seqs):
@@ -368,7 +370,8 @@ def run_murmur(args):
                     "tasks %d pages_consumed %d block %d\n" % (tuple(int(x) - t_first for x in tr[:11]) + (int(tr[11]),)))
             f.write("# cta start_ns end_ns smid tiles   (ns relative to the first CTA start)\n")
             for b in range(tl.shape[0]):
-                f.write("%d %d %d %d %d\n" % (b, tl[b, 0] - t_first, tl[b, 1] - t_first if tl[b, 1] else -1, tl[b, 2], tl[b, 3]))
+                f.write("%d %d %d %d %d\n" % (b, tl[b, 0] - t_first, tl[b, 1] - t_first if tl[b, 1] else -1,
+                                            tl[b, 2] - t_first if tl[b, 2] > (1 << 20) else tl[b, 2], tl[b, 3]))
 
     # ---- region B: K steps with per-kernel events ---------------------------------------------
     n_ret_b0 = sum(cache.seq_state(i)["n_retained"] for i in range(B))
@@ -556,6 +559,7 @@ def main():
     ap.add_argument("--grid", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pdl", action="store_true", help="A/B: launch the step's kernels without programmatic dependent launch")
+    ap.add_argument("--fuse", type=int, default=-1, help="A/B: MURMUR_OPT_FUSE_STEP value (2 = one launch per step, default)")
     ap.add_argument("--no-fuse", action="store_true", help="A/B: murmur_decode_step as three launches (append, evict, attention)")
     ap.add_argument("--timeline", default="", help="write the per-CTA trace of one attention launch to this file")
     ap.add_argument("--cpu-budget-s", default="12")

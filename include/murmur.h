@@ -113,8 +113,11 @@ typedef struct {
 #define MURMUR_OPT_ATTN_GRID 2    /* value: CTAs for the persistent attention kernel; 0 = one per SM */
 #define MURMUR_OPT_PDL 3          /* value: 1 (default) = kernels of a step are launched with programmatic
                                      dependent launch (each waits on-device for its predecessor), 0 = plain */
-#define MURMUR_OPT_FUSE_STEP 4    /* value: 1 (default) = murmur_decode_step runs append + evict as ONE launch
-                                     (the append kernel's last CTA applies the policy), 0 = two launches */
+#define MURMUR_OPT_FUSE_STEP 4    /* murmur_decode_step as: 2 (default) = ONE launch (the attention CTAs derive the
+                                     post-append state themselves, keeper warps scatter the rows, commit and evict;
+                                     needs the tensor-core attention variant, else falls back to 1);
+                                     1 = two launches (append with the eviction fused in, then attention);
+                                     0 = three launches (append, evict, attention) */
 #define MURMUR_ATTN_AUTO 0    /* tensor-core split-K kernel when page_size >= 16, else generic */
 #define MURMUR_ATTN_GENERIC 1 /* one CTA per (layer, sequence, KV head), FFMA, no smem staging */
 #define MURMUR_ATTN_MMA 2     /* persistent split-K kernel: bulk-copy staging + mma.sync bf16 */
@@ -172,9 +175,8 @@ MURMUR_API murmur_status_t murmur_decode_attn(murmur_cache_t* cache, const int32
                                               int32_t layer_end, float sm_scale, void* stream);
 
 /* One whole decode step from DEVICE buffers: append one token to every listed sequence (all
- * layers) -> evict -> decode_attn, enqueued by ONE host call as TWO launches (the step prologue =
- * append with the eviction fused into its last CTA, then the attention kernel, which is launched
- * programmatically dependent so that its set-up overlaps the prologue) (PAPER.md:112-116, 136-146, 101-104:
+ * layers) -> evict -> decode_attn, enqueued by ONE host call as ONE launch by default (see
+ * MURMUR_OPT_FUSE_STEP; the result is identical for every setting) (PAPER.md:112-116, 136-146, 101-104:
  * the per-step loop body of Alg. 1 / Alg. 2 followed by Eq. 1).
  *   k_new, v_new : DEVICE bf16 [n_layers][n_seqs][n_kv_heads][head_dim]
  *   q, out       : DEVICE bf16 [n_layers][n_seqs][n_q_heads][head_dim];  lse as above or NULL

@@ -25,7 +25,7 @@
 //              to a workspace slot, the last one merges them by the log-sum-exp rule.
 #include <cuda_bf16.h>
 
-#include "device_state.cuh"
+#include "evict_body.cuh"
 
 namespace murmur {
 namespace {
@@ -52,10 +52,18 @@ struct __align__(128) SmemLayout {
   float scratch[kSliceWarps][kFragFloats];  // group merge (fragment layout), then slice merge (o[8][132], m, l)
   unsigned long long full_k[kStages], full_v[kStages], empty[kStages], q_full[2], q_empty[2];
   int meta[kStages][2];  // row_begin, row_end of the tile in each stage
-  int nt[kMaxSeqsPerLaunch];
-  int pre[kMaxSeqsPerLaunch + 1];
+  int nt[kMaxSeqsAttn];
+  int pre[kMaxSeqsAttn + 1];
   int flag;
+  // per-sequence state the tiles are generated from (the kernel does not read the evict's tile list)
+  SeqParams sp[kMaxSeqsAttn];    // lengths as attended; step mode: AFTER this step's append
+  TileGen tg[kMaxSeqsAttn];      // runs + tile offsets of each sequence (closed form of sp)
+  int old_nblk[kMaxSeqsAttn];    // blocks mapped in the block table when the kernel starts
+  int newpage[kMaxSeqsAttn];     // step mode: page this step's append maps for the new block, else -1
+  int blk_total;                      // step mode: pages this step's append pops
+  int abort;
 };
+static_assert(sizeof(SmemLayout) <= 227 * 1024, "shared memory budget");
 
 // ---- PTX wrappers ---------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -173,21 +181,59 @@ struct AttnParams {
   const uint16_t* q;
   uint16_t* out;
   float* lse;
+  const uint16_t* k_new;  // step mode: [n_layers][n_seqs][n_kv][128] rows of this step's token
+  const uint16_t* v_new;
   int seq_base, n_seqs_total, layer_begin, n_layers_call;
   float sm_scale;
 };
 
-__global__ void __launch_bounds__(kMmaThreads, 1)
+// Block -> page for tile generation: blocks below old_nblk are in the table; the one block a decode
+// step may add (step mode) is the page the append pops for this sequence.
+struct AttnLookup {
+  const int32_t* tab;
+  int old_nblk, newpage;
+  __device__ __forceinline__ int operator()(int b) const { return b < old_nblk ? tab[b] : newpage; }
+};
+
+// Exclusive scan over <= 128 values held 4 per lane by one warp; returns the grand total.
+__device__ __forceinline__ int warp_scan4(const int (&v)[4], int (&excl)[4], int lane) {
+  int sum = 0;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    excl[k] = sum;
+    sum += v[k];
+  }
+  int inc = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) excl[k] += inc - sum;
+  return __shfl_sync(0xffffffffu, inc, 31);
+}
+
+// kStep = false: murmur_decode_attn (the cache is as murmur_kv_evict left it).
+// kStep = true : the whole decode step in this one launch (murmur_decode_step): every CTA derives
+//   the post-append state itself (lengths + 1, the page a new block gets), attends over it with the
+//   newest token's K/V rows taken straight from k_new / v_new, while one extra "keeper" warp per
+//   CTA scatters those rows into the pools and runs the eviction's table products; the keeper of
+//   the last CTA through a ticket commits the integer state and frees the dead pages.
+template <bool kStep>
+__global__ void __launch_bounds__(kMmaThreads + (kStep ? 32 : 0), 1)
 attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ SeqList list,
                 const __grid_constant__ AttnParams prm) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   SmemLayout& s = *reinterpret_cast<SmemLayout*>(smem_raw);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int n_threads = kMmaThreads + (kStep ? 32 : 0);
   const int n_seqs = list.n, n_kv = c.n_kv, G = c.group;
+  const int p = c.p, plog = c.p_log2;
   unsigned long long* trace = c.timeline + (size_t)blockIdx.x * kTimelineWords;
   pdl_launch_dependents();
 
-  // ---- setup: barriers, tile counts, zeroed padding rows of the Q buffers ------------------------
+  // ---- setup: barriers, zeroed padding rows of the Q buffers ---------------------------------------
   if (tid == 0) {
     for (int i = 0; i < kStages; ++i) {
       mbar_init(&s.full_k[i], 1);
@@ -199,10 +245,13 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       mbar_init(&s.q_empty[i], kConsumerWarps);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    s.abort = 0;
+    s.blk_total = 0;
   }
-  for (int i = tid; i < 2 * kQBytes / 4; i += kMmaThreads) reinterpret_cast<uint32_t*>(&s.q[0][0])[i] = 0u;
+  for (int i = tid; i < 2 * kQBytes / 4; i += n_threads) reinterpret_cast<uint32_t*>(&s.q[0][0])[i] = 0u;
+  __syncthreads();
   // Everything above touches only this CTA's shared memory; from here on the kernel reads what
-  // the step prologue (append + evict) wrote and writes buffers the previous launch may still use.
+  // earlier kernels of the stream wrote and writes buffers the previous launch may still use.
   pdl_wait();
   if (tid == 0) {
     trace[0] = globaltimer_ns();
@@ -210,18 +259,119 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     trace[2] = smid();
     trace[3] = 0ull;
   }
-  for (int i = tid; i < n_seqs; i += kMmaThreads) s.nt[i] = c.seqs[list.ids[i]].n_tiles;
-  __syncthreads();
-  if (tid == 0) {
-    int acc = 0;
-    for (int i = 0; i < n_seqs; ++i) {
-      s.pre[i] = acc;
-      acc += s.nt[i];
+  // ---- per-sequence state: policy + length -> tile count; step mode: the length after this step ----
+  const int free_top = kStep ? c.ctrl[kCtrlFreeTop] : 0;
+  for (int i = tid; i < n_seqs; i += n_threads) {
+    const SeqDev& sd = c.seqs[list.ids[i]];
+    SeqParams sp = load_params(sd);
+    const int old_nblk = (sp.len + p - 1) >> plog;
+    if (kStep) {
+      sp.len += 1;
+      if (!sd.active || ((sp.len + p - 1) >> plog) > c.max_blocks) s.abort = 2;
     }
-    s.pre[n_seqs] = acc;
+    s.sp[i] = sp;
+    s.old_nblk[i] = old_nblk;
+    s.newpage[i] = -1;
+    // the tile table at this length was written by the last evict / decode step (SeqDev.tg);
+    // generate it here only if it is missing (e.g. a bulk append that was not followed by an evict)
+#ifdef MURMUR_EXP_OLD_SETUP
+    s.nt[i] = sd.n_tiles;
+#else
+    if (sd.tg_len[sp.len & 1] == sp.len) {
+      s.tg[i] = sd.tg[sp.len & 1];
+    } else {
+      s.tg[i] = make_tilegen(sp, p, plog);
+    }
+    s.nt[i] = s.tg[i].n_tiles;
+#endif
+  }
+  __syncthreads();
+  if (warp == 0) {  // prefix sums over <= 64 sequences: tiles, and (step mode) new-block demand
+    int v[4], ex[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = (lane * 4 + k < n_seqs) ? s.nt[lane * 4 + k] : 0;
+    const int tiles_all = warp_scan4(v, ex, lane);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (lane * 4 + k < n_seqs) s.pre[lane * 4 + k] = ex[k];
+    if (lane == 0) s.pre[n_seqs] = tiles_all;
+    if (kStep) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int i = lane * 4 + k;
+        v[k] = (i < n_seqs && ((s.sp[i].len + p - 1) >> plog) > s.old_nblk[i]) ? 1 : 0;
+      }
+      const int blk_all = warp_scan4(v, ex, lane);
+      if (blk_all > free_top) {  // cannot happen after the host-side check; all CTAs agree
+        if (lane == 0) s.abort = 3;
+      } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k)  // pops in call order (C3)
+          if (v[k]) s.newpage[lane * 4 + k] = c.free_stack[free_top - 1 - ex[k]];
+      }
+      if (lane == 0) s.blk_total = blk_all;
+    }
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // zeroed Q rows vs later bulk copies
   __syncthreads();
+  if (s.abort) {
+    if (tid == 0) atomicCAS(&c.ctrl[kCtrlError], 0, s.abort);
+    return;
+  }
+
+  const uint8_t* kpool = reinterpret_cast<const uint8_t*>(c.k_pool);
+  const uint8_t* vpool = reinterpret_cast<const uint8_t*>(c.v_pool);
+
+  if (kStep && warp == kConsumerWarps + 1) {
+    // ===================================== keeper warp =====================================
+    // All the old state this CTA needs is in shared memory now: take the ticket first.
+    int last = 0;
+    if (lane == 0) last = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
+    last = __shfl_sync(0xffffffffu, last, 0);
+    // (1) the eviction's table products for the post-append state, spread over the CTAs
+#ifdef MURMUR_EXP_NO_KEEPER
+    if (!last) return;
+#endif
+    for (int task = (int)blockIdx.x; task < 2 * n_seqs; task += (int)gridDim.x) {
+      const int role = 1 + task / n_seqs, i = task % n_seqs;
+      const AttnLookup lk{c.block_table + (size_t)list.ids[i] * c.max_blocks, s.old_nblk[i], s.newpage[i]};
+      evict_task(c, list.ids[i], s.sp[i], role, lk);
+    }
+    // (2) this step's K/V rows into the pools: one half-warp per 256-byte row (pre-swizzled)
+    {
+      const int half = lane >> 4, sub = lane & 15;
+      const unsigned per_kv = (unsigned)prm.n_layers_call * (unsigned)n_seqs * (unsigned)n_kv;
+#ifdef MURMUR_EXP_NO_SCATTER
+      for (unsigned u = 2u * per_kv; u < 2u * per_kv; u += 2u * gridDim.x) {
+#else
+      for (unsigned u = 2u * blockIdx.x + half; u < 2u * per_kv; u += 2u * gridDim.x) {
+#endif
+        const unsigned is_v = u >= per_kv, r = is_v ? u - per_kv : u;
+        const unsigned r2 = r / (unsigned)n_kv, h = r - r2 * (unsigned)n_kv;
+        const unsigned lc = r2 / (unsigned)n_seqs, i = r2 - lc * (unsigned)n_seqs;
+        const int x = s.sp[i].len - 1, b = x >> plog, slot = x & (p - 1);
+        const int page = b < s.old_nblk[i] ? c.block_table[(size_t)list.ids[i] * c.max_blocks + b] : s.newpage[i];
+        if (page < 0) {
+          atomicCAS(&c.ctrl[kCtrlError], 0, 2);
+          continue;
+        }
+        const uint4 val = reinterpret_cast<const uint4*>(is_v ? prm.v_new : prm.k_new)[(size_t)r * 16 + sub];
+        uint8_t* pool = reinterpret_cast<uint8_t*>(is_v ? c.v_pool : c.k_pool);
+        reinterpret_cast<uint4*>(pool + row_offset(c, prm.layer_begin + (int)lc, page, (int)h, slot))[sub ^ (slot & 7)] = val;
+      }
+    }
+    // (3) last CTA through the ticket: commit the append, then free the dead pages
+    if (last) {
+      for (int i = lane; i < n_seqs; i += 32) {
+        c.seqs[list.ids[i]].len = s.sp[i].len;
+        if (s.newpage[i] >= 0) c.block_table[(size_t)list.ids[i] * c.max_blocks + s.old_nblk[i]] = s.newpage[i];
+      }
+      if (lane == 0) c.ctrl[kCtrlAppendTicket] = 0;
+      __syncwarp();
+      evict_free_warp(c, list.ids, n_seqs, s.sp, free_top - s.blk_total);
+    }
+    return;
+  }
 
   const long long total = (long long)prm.n_layers_call * n_kv * s.pre[n_seqs];
   const long long geff = total < (long long)gridDim.x ? total : (long long)gridDim.x;
@@ -229,88 +379,131 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   if (cta >= geff) return;
   const long long lo = cta * total / geff, hi = (cta + 1) * total / geff;
 
-  const uint8_t* kpool = reinterpret_cast<const uint8_t*>(c.k_pool);
-  const uint8_t* vpool = reinterpret_cast<const uint8_t*>(c.v_pool);
-
   if (warp == kConsumerWarps) {
     // =================================== producer warp ===================================
-    // Walks its tile range in batches of <= 32 tiles of one item (lane j issues tile j); the
-    // descriptors of the NEXT batch are loaded before the current one is issued, so their
-    // global-load latency hides behind the copies.
+    // Walks its tile range in batches of <= 32 tiles of one item; lane j owns tile j of the batch.
+    // Everything a tile's copies need (pool offsets, sizes, destination rows) is computed by all
+    // lanes in parallel, right after the previous batch has been issued (the ring is full then, so
+    // the table loads hide behind it), from the sequence's tile table plus one block-table load
+    // per page - so the serial part of issuing a tile (one lane at a time, ring order) is only:
+    // wait for the stage, 2 expect_tx, the copies.  That serial path runs at single-warp latency
+    // and has to stay well below the ~0.75 us a tile takes to stream at this CTA's share of HBM.
     const unsigned long long kv_policy = l2_policy_evict_first();
+    struct TileIssue {
+      unsigned long long off[4];  // byte offset of the page's first copied row in a pool (same in K and V)
+      uint32_t dst[4], bytes[4];  // destination offset in the stage buffer, bytes to copy (0 = none)
+      int row_begin, row_end;     // valid rows of the tile buffer
+      uint32_t tx;                // bytes arriving through bulk copies, per K / V barrier
+      int has_new;                // step mode: the last row is this step's token (not in the pool yet)
+    };
+    auto prep = [&](const Cursor& cc, int tix) {
+      const AttnLookup lk{c.block_table + (size_t)list.ids[cc.i] * c.max_blocks, s.old_nblk[cc.i], s.newpage[cc.i]};
+#ifdef MURMUR_EXP_LOAD_TILES
+      const TileDesc td = kStep ? tile_at(s.tg[cc.i], tix, p, plog, lk) : c.tiles[(size_t)list.ids[cc.i] * c.max_blocks + tix];
+#else
+      const TileDesc td = tile_at(s.tg[cc.i], tix, p, plog, lk);
+#endif
+      TileIssue ti;
+      ti.row_begin = td.row_begin;
+      ti.row_end = td.row_end;
+      // step mode: the newest token (position len - 1) is the last row of the item's last tile
+#ifdef MURMUR_EXP_NO_NEWROW
+      ti.has_new = 0 &&
+#else
+      ti.has_new =
+#endif
+          kStep && td.first_pos + (td.row_end - td.row_begin) - 1 == s.sp[cc.i].len - 1;
+      const int row_end_pool = td.row_end - ti.has_new;
+      ti.tx = (uint32_t)(row_end_pool - td.row_begin) * kRowBytes;
+      const int layer = prm.layer_begin + cc.layer;
+#pragma unroll
+      for (int pg = 0; pg < 4; ++pg) {
+        const int r0 = (pg == 0) ? td.row_begin : pg * p;
+        const int r1 = (pg == td.n_pages - 1) ? row_end_pool : (pg + 1) * p;
+        const bool on = pg < td.n_pages && r1 > r0;
+        ti.off[pg] = on ? row_offset(c, layer, td.page[pg], cc.h, r0 - pg * p) : 0ull;
+        ti.dst[pg] = (uint32_t)r0 * kRowBytes;
+        ti.bytes[pg] = on ? (uint32_t)(r1 - r0) * kRowBytes : 0u;
+      }
+      return ti;
+    };
     Cursor cur = locate(s, n_seqs, n_kv, lo);
     long long remaining = hi - lo;  // tiles left, counted from the start of the current item's segment
     int seg = (int)min((long long)(s.nt[cur.i] - cur.k), remaining);
     int base = 0, cnt = min(32, seg);
-    uint32_t n = 0;  // tile sequence number of this CTA
+    int st = 0;          // ring stage of the next tile
+    uint32_t ph = 0;     // its phase parity
     int item_no = 0;
-    TileDesc td;
-    if (lane < cnt) td = c.tiles[(size_t)list.ids[cur.i] * c.max_blocks + cur.k + lane];
+    TileIssue ti;
+    if (lane < cnt) ti = prep(cur, cur.k + lane);
+    uint4 new_row = make_uint4(0u, 0u, 0u, 0u);
+#ifdef MURMUR_EXP_TRACE_FIRST
+    if (lane == 0) trace[2] = globaltimer_ns();
+#endif
     while (remaining > 0) {
-      // ---- next batch (prefetch its descriptors) ----
-      Cursor ncur = cur;
-      int nseg = seg, nbase = base + cnt, ncnt = 0;
-      long long nrem = remaining;
-      const bool item_done = nbase >= seg;
-      if (item_done) {
-        nrem = remaining - seg;
-        nbase = 0;
-        if (nrem > 0) {
-          next_item(s, n_seqs, n_kv, ncur);
-          nseg = (int)min((long long)s.nt[ncur.i], nrem);
+      // ---- issue the current batch ----
+      if (base == 0) {  // first batch of an item (or of this CTA's segment of it)
+        if (lane == 0) {  // stage its G query rows
+          const int qb = item_no & 1;
+          mbar_wait(&s.q_empty[qb], ((item_no >> 1) & 1) ^ 1);
+          const size_t row = ((size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i) * c.n_q + (size_t)cur.h * G;
+          mbar_expect_tx(&s.q_full[qb], (uint32_t)(G * kRowBytes));
+          bulk_g2s(&s.q[qb][0], prm.q + row * kHeadDim, (uint32_t)(G * kRowBytes), &s.q_full[qb]);
+        }
+        if (kStep) {
+          // this step's K and V rows of the item, straight from k_new / v_new into registers
+          // (lane = (K|V, 16-byte chunk)); stored into the stage buffer when the last tile is issued
+          const size_t src_row = ((size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i) * n_kv + cur.h;
+          new_row = reinterpret_cast<const uint4*>((lane >> 4) ? prm.v_new : prm.k_new)[src_row * 16 + (lane & 15)];
         }
       }
-      if (nrem > 0) ncnt = min(32, nseg - nbase);
-      TileDesc ntd;
-      if (lane < ncnt) ntd = c.tiles[(size_t)list.ids[ncur.i] * c.max_blocks + ncur.k + nbase + lane];
-
-      // ---- current batch ----
-      const int layer = prm.layer_begin + cur.layer;
-      if (base == 0 && lane == 0) {  // first batch of an item: stage its G query rows
-        const int qb = item_no & 1;
-        mbar_wait(&s.q_empty[qb], ((item_no >> 1) & 1) ^ 1);
-        const size_t row = ((size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i) * c.n_q + (size_t)cur.h * G;
-        mbar_expect_tx(&s.q_full[qb], (uint32_t)(G * kRowBytes));
-        bulk_g2s(&s.q[qb][0], prm.q + row * kHeadDim, (uint32_t)(G * kRowBytes), &s.q_full[qb]);
-      }
+      // only the item's last tile can end with this step's token
+      const int j_last = kStep ? (s.nt[cur.i] - 1) - (cur.k + base) : -1;
       for (int j = 0; j < cnt; ++j) {
+        bool has_new = false;
+        if (kStep && j == j_last) {
+          has_new = __shfl_sync(0xffffffffu, ti.has_new, j) != 0;
+          if (has_new) {
+            if (lane == j) mbar_wait(&s.empty[st], ph ^ 1u);
+            __syncwarp();
+            const int r = __shfl_sync(0xffffffffu, ti.row_end, j) - 1;
+            *reinterpret_cast<uint4*>(&s.kv[st][lane >> 4][r * kRowBytes + (((lane & 15) ^ (r & 7)) << 4)]) = new_row;
+            __syncwarp();  // the stores are ordered before lane j's (releasing) arrive below
+          }
+        }
         if (lane == j) {
-          const uint32_t nn = n + (uint32_t)j;
-          const int st = (int)(nn % kStages);
-          const uint32_t ph = (nn / kStages) & 1u;
-          mbar_wait(&s.empty[st], ph ^ 1u);
-          s.meta[st][0] = td.row_begin;
-          s.meta[st][1] = td.row_end;
-          const uint32_t bytes = (uint32_t)(td.row_end - td.row_begin) * kRowBytes;
-          mbar_expect_tx(&s.full_k[st], bytes);
-          mbar_expect_tx(&s.full_v[st], bytes);
+          if (!has_new) mbar_wait(&s.empty[st], ph ^ 1u);
+          s.meta[st][0] = ti.row_begin;
+          s.meta[st][1] = ti.row_end;
+          mbar_expect_tx(&s.full_k[st], ti.tx);  // 0 bytes (a tile that is only the new row) = plain arrive
+          mbar_expect_tx(&s.full_v[st], ti.tx);
 #pragma unroll
-          for (int kv = 0; kv < 2; ++kv) {
-            const uint8_t* pool = kv ? vpool : kpool;
-            unsigned long long* bar = kv ? &s.full_v[st] : &s.full_k[st];
-#pragma unroll
-            for (int pg = 0; pg < 4; ++pg) {
-              if (pg < td.n_pages) {
-                const int r0 = (pg == 0) ? td.row_begin : pg * c.p;
-                const int r1 = (pg == td.n_pages - 1) ? td.row_end : (pg + 1) * c.p;
-                const uint8_t* src = pool + row_offset(c, layer, td.page[pg], cur.h, r0 - pg * c.p);
-                bulk_g2s_hint(&s.kv[st][kv][r0 * kRowBytes], src, (uint32_t)(r1 - r0) * kRowBytes, bar, kv_policy);
-              }
+          for (int pg = 0; pg < 4; ++pg) {
+            if (ti.bytes[pg]) {
+              bulk_g2s_hint(&s.kv[st][0][ti.dst[pg]], kpool + ti.off[pg], ti.bytes[pg], &s.full_k[st], kv_policy);
+              bulk_g2s_hint(&s.kv[st][1][ti.dst[pg]], vpool + ti.off[pg], ti.bytes[pg], &s.full_v[st], kv_policy);
             }
           }
         }
         __syncwarp();
+        if (++st == kStages) {
+          st = 0;
+          ph ^= 1u;
+        }
       }
-      n += (uint32_t)cnt;
-      if (item_done) {
+      // ---- advance, and prepare the next batch while the ring (just filled) drains ----
+      base += cnt;
+      if (base >= seg) {  // item (or this CTA's segment of it) done
+        remaining -= seg;
+        base = 0;
         ++item_no;
-        remaining = nrem;
+        if (remaining > 0) {
+          next_item(s, n_seqs, n_kv, cur);
+          seg = (int)min((long long)s.nt[cur.i], remaining);
+        }
       }
-      cur = ncur;
-      seg = nseg;
-      base = nbase;
-      cnt = ncnt;
-      td = ntd;
+      cnt = remaining > 0 ? min(32, seg - base) : 0;
+      if (lane < cnt) ti = prep(cur, cur.k + base + lane);
     }
     return;
   }
@@ -612,18 +805,33 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 
 }  // namespace
 
-cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
-                            void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
-                            bool pdl, cudaStream_t st, LaunchInfo* info) {
+namespace {
+
+template <bool kStep>
+cudaError_t launch_mma(const CacheView& c, const SeqList& list, const AttnParams& prm_in, int grid, bool pdl,
+                       cudaStream_t st, LaunchInfo* info) {
   static bool attr_set = false;
   const int smem = (int)sizeof(SmemLayout);
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(attn_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(attn_mma_kernel<kStep>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   if (grid > kMaxAttnGrid) grid = kMaxAttnGrid;
-  AttnParams prm;
+  AttnParams prm = prm_in;
+  PdlLaunch l(dim3((unsigned)grid), dim3(kMmaThreads + (kStep ? 32 : 0)), (size_t)smem, st, pdl);
+  info->launches += 1;
+  info->grid = grid;
+  info->smem = smem;
+  return cudaLaunchKernelEx(&l.cfg, attn_mma_kernel<kStep>, c, list, prm);
+}
+
+}  // namespace
+
+cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
+                            void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
+                            bool pdl, cudaStream_t st, LaunchInfo* info) {
+  AttnParams prm{};
   prm.q = reinterpret_cast<const uint16_t*>(q);
   prm.out = reinterpret_cast<uint16_t*>(out);
   prm.lse = lse;
@@ -632,11 +840,25 @@ cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_bas
   prm.layer_begin = layer_begin;
   prm.n_layers_call = layer_end - layer_begin;
   prm.sm_scale = sm_scale;
-  PdlLaunch l(dim3((unsigned)grid), dim3(kMmaThreads), (size_t)smem, st, pdl);
-  info->launches += 1;
-  info->grid = grid;
-  info->smem = smem;
-  return cudaLaunchKernelEx(&l.cfg, attn_mma_kernel, c, list, prm);
+  return launch_mma<false>(c, list, prm, grid, pdl, st, info);
+}
+
+// The whole decode step (append one token per sequence, evict, attend) as ONE launch, all layers.
+cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void* k_new, const void* v_new,
+                            const void* q, void* out, float* lse, float sm_scale, int grid, bool pdl, cudaStream_t st,
+                            LaunchInfo* info) {
+  AttnParams prm{};
+  prm.q = reinterpret_cast<const uint16_t*>(q);
+  prm.out = reinterpret_cast<uint16_t*>(out);
+  prm.lse = lse;
+  prm.k_new = reinterpret_cast<const uint16_t*>(k_new);
+  prm.v_new = reinterpret_cast<const uint16_t*>(v_new);
+  prm.seq_base = 0;
+  prm.n_seqs_total = list.n;
+  prm.layer_begin = 0;
+  prm.n_layers_call = c.n_layers;
+  prm.sm_scale = sm_scale;
+  return launch_mma<true>(c, list, prm, grid, pdl, st, info);
 }
 
 }  // namespace murmur

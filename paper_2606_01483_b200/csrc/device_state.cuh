@@ -22,6 +22,7 @@ constexpr int kTileRows = 64;            // rows of one attention tile (tokens)
 constexpr int kMaxGroup = 8;             // query heads per KV head, padded to the MMA N = 8
 constexpr int kMaxRuns = 6;
 constexpr int kMaxSeqsPerLaunch = 128;
+constexpr int kMaxSeqsAttn = 64;         // sequences per launch of the tensor-core attention kernel (smem tables)
 constexpr int kOStride = 132;            // floats per head row in split-K partials / merge scratch
 constexpr int kPartialFloats = kMaxGroup * kOStride + 2 * kMaxGroup;  // o[8][132] + m[8] + l[8]
 constexpr int kMaxAttnGrid = 1024;       // upper bound on CTAs of the persistent attention kernel
@@ -31,7 +32,23 @@ constexpr int kTimelineWords = 4;        // globaltimer at CTA start, at CTA end
 // ctrl word indices
 enum { kCtrlFreeTop = 0, kCtrlError = 1, kCtrlAppendTicket = 2, kCtrlWords = 8 };
 
-struct SeqDev {  // 128 bytes
+// The maximal intervals of A(t) held in six fixed slots (all indexing static, so the whole thing
+// lives in registers): slot i is a run iff bit i of `mask` is set; merged neighbours are folded
+// into the lowest slot of their group.
+struct Runs6 {
+  int32_t a[6], b[6];
+  uint32_t mask;
+};
+
+// Attention tiles of one sequence, generated from the runs: a tile is <= 64 consecutive rows of
+// one run = 64/p consecutive (live) blocks.  toff[i] = tiles before slot i.
+struct TileGen {
+  Runs6 rr;
+  int32_t toff[6];
+  int32_t n_tiles, n_ret;
+};
+
+struct SeqDev {  // 320 bytes
   int32_t P, S, M, len;
   int32_t w_s, d, k_s, w_o, k_o;
   int32_t active;
@@ -40,8 +57,14 @@ struct SeqDev {  // 128 bytes
   int32_t n_tiles;     // attention tiles (tensor-core path)
   int32_t n_retained;  // |A(t)|
   int32_t runs[kMaxRuns][3];  // first_pos, n_tok, index of first block in live list
+  // Tile tables of the retained set, double-buffered by length parity: tg[x & 1] is the table at
+  // length x iff tg_len[x & 1] == x.  An evict at length L writes the tables for L and L + 1, so
+  // the next decode step (which attends at L + 1) finds its table ready and only copies it.
+  TileGen tg[2];
+  int32_t tg_len[2];
+  int32_t pad[4];
 };
-static_assert(sizeof(SeqDev) == 128, "SeqDev must be 128 bytes");
+static_assert(sizeof(SeqDev) == 320, "SeqDev must be 320 bytes");
 
 struct __align__(16) TileDesc {  // 32 bytes: one <= 64-row tile of one run, same for all layers/heads
   int32_t page[4];     // physical pages of the tile, in order (unused = -1)
@@ -157,6 +180,9 @@ cudaError_t launch_attn_generic(const CacheView& c, const SeqList& list, int seq
 cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                             void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
                             bool pdl, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void* k_new, const void* v_new,
+                            const void* q, void* out, float* lse, float sm_scale, int grid, bool pdl, cudaStream_t st,
+                            LaunchInfo* info);
 cudaError_t launch_expand_retained(const CacheView& c, int seq, int32_t* pos_out_dev, int cap, cudaStream_t st,
                                    LaunchInfo* info);
 cudaError_t launch_gather(const CacheView& c, int seq, const int32_t* positions_dev, int n, int layer_begin,

@@ -50,14 +50,7 @@ __device__ __forceinline__ bool is_dead_block(const DeadRanges& dr, int blk) {
   return (blk >= dr.lo0 && blk < dr.hi0) || (blk >= dr.lo1 && blk < dr.hi1);
 }
 
-// The maximal intervals of A(t) held in six fixed slots (all indexing static, so the whole thing
-// lives in registers): slot i is a run iff bit i of `mask` is set; merged neighbours are folded
-// into the lowest slot of their group.  Same set as retained_runs() of policy_math.cuh.
-struct Runs6 {
-  int32_t a[6], b[6];
-  unsigned mask;
-};
-
+// Runs6 (device_state.cuh) of a sequence: same set as retained_runs() of policy_math.cuh.
 __device__ __forceinline__ Runs6 retained_runs6(const SeqParams& s) {
   const int32_t t = seq_t(s);
   const int32_t l = mm_min(window_start(s, t), s.S);
@@ -96,6 +89,47 @@ __device__ __forceinline__ Runs6 retained_runs6(const SeqParams& s) {
   return r;
 }
 
+__device__ __forceinline__ TileGen make_tilegen(const SeqParams& sp, int p, int plog) {
+  TileGen g;
+  g.rr = retained_runs6(sp);
+  const int ppt = kTileRows >> plog;  // pages per tile (tiles only exist for 16 <= p <= 64)
+  g.n_tiles = 0;
+  g.n_ret = 0;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+    g.toff[i] = g.n_tiles;
+    if (g.rr.mask >> i & 1u) {
+      g.n_ret += g.rr.b[i] - g.rr.a[i];
+      const int fb = g.rr.a[i] >> plog, lb = (g.rr.b[i] - 1) >> plog;
+      g.n_tiles += ((lb - fb + 1) + ppt - 1) / ppt;
+    }
+  }
+  if (p < 16 || p > kTileRows) g.n_tiles = 0;
+  return g;
+}
+
+// Descriptor of tile tix (0 <= tix < n_tiles); page_of(b) maps a logical block to its page.
+template <class Lookup>
+__device__ __forceinline__ TileDesc tile_at(const TileGen& g, int tix, int p, int plog, const Lookup& page_of) {
+  int32_t a = 0, b = 0, t0 = 0;
+#pragma unroll
+  for (int i = 0; i < 6; ++i)
+    if ((g.rr.mask >> i & 1u) && tix >= g.toff[i]) { a = g.rr.a[i]; b = g.rr.b[i]; t0 = g.toff[i]; }
+  const int ppt = kTileRows >> plog;
+  const int j = tix - t0;
+  const int fb = a >> plog, lb = (b - 1) >> plog;
+  const int b0 = fb + j * ppt;
+  const int np = min(ppt, lb - b0 + 1);
+  TileDesc td;
+  td.n_pages = np;
+  td.row_begin = (j == 0) ? (a & (p - 1)) : 0;
+  td.row_end = (b0 + np - 1 == lb) ? (np - 1) * p + ((b - 1) & (p - 1)) + 1 : np * p;
+  td.first_pos = (j == 0) ? a : b0 * p;
+#pragma unroll
+  for (int q = 0; q < 4; ++q) td.page[q] = (q < np) ? page_of(b0 + q) : -1;
+  return td;
+}
+
 // Page of logical block b of a sequence, as the eviction sees it.  The stand-alone kernel reads
 // the block table; the fused step prologue, which runs these tasks BEFORE the append's integer
 // state is committed, substitutes the pages the append is about to map (kv_append.cu).
@@ -128,22 +162,10 @@ __device__ __forceinline__ void evict_task(const CacheView& c, int id, const Seq
   } else {
     // ---- run descriptors: maximal intervals of A(t) + rank of their first block in the live list ----
     SeqDev& sd = c.seqs[id];
-    const Runs6 rr = retained_runs6(sp);
+    const TileGen g = make_tilegen(sp, p, plog);
+    const Runs6& rr = g.rr;
     const int nr = __popc(rr.mask);
-    const int ppt = kTileRows >> plog;  // pages per tile (tiles only exist for 16 <= p <= 64)
-    const bool tiled = (p >= 16 && p <= kTileRows);
-    int n_ret = 0, n_tiles = 0;
-    int toff[6];  // tiles before slot i (static indexing)
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-      toff[i] = n_tiles;
-      if (rr.mask >> i & 1u) {
-        n_ret += rr.b[i] - rr.a[i];
-        const int fb = rr.a[i] >> plog, lb = (rr.b[i] - 1) >> plog;
-        n_tiles += ((lb - fb + 1) + ppt - 1) / ppt;
-      }
-    }
-    if (!tiled) n_tiles = 0;
+    const int n_tiles = g.n_tiles, n_ret = g.n_ret;
     if (lane < nr) {  // lane r writes run r = the r-th set slot
       const int slot = __fns(rr.mask, 0, lane + 1);
       int32_t a = 0, b = 0;
@@ -156,44 +178,34 @@ __device__ __forceinline__ void evict_task(const CacheView& c, int id, const Seq
       sd.runs[lane][1] = b - a;
       sd.runs[lane][2] = live_rank(dr, blk);
     }
-    // ---- attention tiles: <= 64 consecutive rows of one run = 64/p consecutive (live) blocks ----
+    // ---- attention tile list (read by tools; the attention kernel regenerates tiles itself) ----
     TileDesc* tiles = c.tiles + (size_t)id * c.max_blocks;
     for (int tix = lane; tix < n_tiles; tix += 32) {
-      int32_t a = 0, b = 0, t0 = 0;
+      const TileDesc td = tile_at(g, tix, p, plog, page_of);
 #pragma unroll
-      for (int i = 0; i < 6; ++i)
-        if ((rr.mask >> i & 1u) && tix >= toff[i]) { a = rr.a[i]; b = rr.b[i]; t0 = toff[i]; }
-      const int j = tix - t0;
-      const int fb = a >> plog, lb = (b - 1) >> plog;
-      const int b0 = fb + j * ppt;
-      const int np = min(ppt, lb - b0 + 1);
-      TileDesc td;
-      td.n_pages = np;
-      td.row_begin = (j == 0) ? (a & (p - 1)) : 0;
-      td.row_end = (b0 + np - 1 == lb) ? (np - 1) * p + ((b - 1) & (p - 1)) + 1 : np * p;
-      td.first_pos = (j == 0) ? a : b0 * p;
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        td.page[q] = (q < np) ? page_of(b0 + q) : -1;
-        bad |= (q < np) && (td.page[q] < 0);
-      }
+      for (int q = 0; q < 4; ++q) bad |= (q < td.n_pages) && (td.page[q] < 0);
       tiles[tix] = td;
     }
     if (lane == 0) {
       sd.n_runs = nr;
       sd.n_tiles = n_tiles;
       sd.n_retained = n_ret;
+      // tile tables for the attention kernels: this length (unless already there - it may be in
+      // use by concurrent readers, which never read an invalid slot) and the next decode step's
+      SeqParams sp1 = sp;
+      sp1.len += 1;
+      sd.tg[sp1.len & 1] = make_tilegen(sp1, p, plog);
+      sd.tg_len[sp1.len & 1] = sp1.len;
+      if (sd.tg_len[sp.len & 1] != sp.len) {
+        sd.tg[sp.len & 1] = g;
+        __threadfence();  // the table before the length that validates it
+        sd.tg_len[sp.len & 1] = sp.len;
+      }
     }
   }
   if (bad) atomicCAS(&c.ctrl[kCtrlError], 0, 2);
 }
 
-// CTA-wide: product 0.  Counts each sequence's newly dead (still mapped) blocks (unless the caller
-// already has: `counted`), fixes the push
-// order with an exclusive prefix sum in call order, pushes the pages (blocks ascending) and unmaps
-// them.  sp_sh: SeqParams[n] in shared memory with the lengths as of this evict; s_ndead
-// int[kMaxSeqsPerLaunch], s_off int[kMaxSeqsPerLaunch + 1] shared scratch; free_top0 = height of
-// the free stack before this evict.  Must be called by every thread of the CTA.
 // Warp tasks: s_ndead[i] = mapped blocks inside the dead ranges of sequence i at length
 // sp_sh[i].len (+ extra_len[i] if given).
 __device__ __forceinline__ void evict_count(const CacheView& c, const int32_t* ids, int n, const SeqParams* sp_sh,
@@ -212,6 +224,12 @@ __device__ __forceinline__ void evict_count(const CacheView& c, const int32_t* i
   }
 }
 
+// CTA-wide: product 0.  Counts each sequence's newly dead (still mapped) blocks (unless the caller
+// already has: `counted`), fixes the push order with an exclusive prefix sum in call order, pushes
+// the pages (blocks ascending) and unmaps them.  sp_sh: SeqParams[n] in shared memory with the
+// lengths as of this evict; s_ndead int[kMaxSeqsPerLaunch], s_off int[kMaxSeqsPerLaunch + 1] shared
+// scratch; free_top0 = height of the free stack before this evict.  Must be called by every
+// thread of the CTA.
 __device__ __forceinline__ void evict_free(const CacheView& c, const int32_t* ids, int n, const SeqParams* sp_sh,
                                            int free_top0, int* s_ndead, int* s_off, bool counted = false) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
@@ -250,6 +268,34 @@ __device__ __forceinline__ void evict_free(const CacheView& c, const int32_t* id
       }
     }
   }
+}
+
+// Product 0 by ONE warp (the keeper warp of the single-kernel decode step): sequences in call
+// order, so the push offset is a running sum and no CTA-wide synchronisation is needed.
+__device__ __forceinline__ void evict_free_warp(const CacheView& c, const int32_t* ids, int n, const SeqParams* sp_sh,
+                                                int free_top0) {
+  const int lane = threadIdx.x & 31;
+  const unsigned lt_mask = (1u << lane) - 1;
+  int top = free_top0;
+  for (int i = 0; i < n; ++i) {
+    const DeadRanges dr = dead_block_ranges(sp_sh[i], c.p_log2);
+    int32_t* tab = c.block_table + (size_t)ids[i] * c.max_blocks;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int lo = k ? dr.lo1 : dr.lo0, hi = k ? dr.hi1 : dr.hi0;
+      for (int b0 = lo; b0 < hi; b0 += 32) {
+        const int b = b0 + lane;
+        const int pg = (b < hi) ? tab[b] : -1;
+        const unsigned m = __ballot_sync(0xffffffffu, pg >= 0);
+        if (pg >= 0) {
+          c.free_stack[top + __popc(m & lt_mask)] = pg;
+          tab[b] = -1;
+        }
+        top += __popc(m);
+      }
+    }
+  }
+  if (lane == 0) c.ctrl[kCtrlFreeTop] = top;
 }
 
 // The whole eviction in one CTA (stand-alone kernel).

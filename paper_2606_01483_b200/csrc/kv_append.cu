@@ -42,6 +42,7 @@ __global__ void seq_begin_kernel(CacheView c, int seq, SeqParams sp) {
     s.w_s = sp.w_s; s.d = sp.d; s.k_s = sp.k_s; s.w_o = sp.w_o; s.k_o = sp.k_o;
     s.active = 1;
     s.n_live = 0; s.n_runs = 0; s.n_tiles = 0; s.n_retained = 0;
+    s.tg_len[0] = s.tg_len[1] = -1;
   }
 }
 

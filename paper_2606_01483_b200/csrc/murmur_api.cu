@@ -160,7 +160,7 @@ murmur_status_t murmur_cache_create(const murmur_cache_desc_t* d, murmur_cache_t
   c->attn_variant_opt = MURMUR_ATTN_AUTO;
   c->attn_grid_opt = 0;
   c->pdl_opt = 1;
-  c->fuse_step_opt = 1;
+  c->fuse_step_opt = 2;
   std::memset(&c->stats, 0, sizeof c->stats);
   c->last_cuda = cudaSuccess;
   int dev = 0;
@@ -371,9 +371,10 @@ murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, in
   if (variant == MURMUR_ATTN_AUTO) variant = (c->desc.page_size >= 16) ? MURMUR_ATTN_MMA : MURMUR_ATTN_GENERIC;
   if (variant == MURMUR_ATTN_MMA && c->desc.page_size < 16) return MURMUR_ERR_UNSUPPORTED;
   const int grid = c->attn_grid_opt > 0 ? c->attn_grid_opt : c->sm_count;
-  for (int base = 0; base < n_seqs; base += kMaxSeqsPerLaunch) {
+  const int chunk = (variant == MURMUR_ATTN_MMA) ? kMaxSeqsAttn : kMaxSeqsPerLaunch;
+  for (int base = 0; base < n_seqs; base += chunk) {
     SeqList list;
-    list.n = (n_seqs - base) < kMaxSeqsPerLaunch ? (n_seqs - base) : kMaxSeqsPerLaunch;
+    list.n = (n_seqs - base) < chunk ? (n_seqs - base) : chunk;
     for (int i = 0; i < list.n; ++i) list.ids[i] = seq_ids[base + i];
     LaunchInfo li{};
     if (variant == MURMUR_ATTN_MMA) {
@@ -416,6 +417,32 @@ murmur_status_t murmur_decode_step(murmur_cache_t* c, const int32_t* seq_ids, in
   if (st != MURMUR_OK) return st;
   int32_t ones[kMaxSeqsPerLaunch];
   for (int i = 0; i < n_seqs; ++i) ones[i] = 1;
+  int variant = c->attn_variant_opt;
+  if (variant == MURMUR_ATTN_AUTO) variant = (c->desc.page_size >= 16) ? MURMUR_ATTN_MMA : MURMUR_ATTN_GENERIC;
+  if (c->fuse_step_opt >= 2 && variant == MURMUR_ATTN_MMA && c->desc.page_size >= 16 && n_seqs <= kMaxSeqsAttn) {
+    // ONE launch: every CTA derives the post-append state, keeper warps scatter / commit / evict
+    SeqList list;
+    list.n = n_seqs;
+    for (int i = 0; i < n_seqs; ++i) list.ids[i] = seq_ids[i];
+    const int grid = c->attn_grid_opt > 0 ? c->attn_grid_opt : c->sm_count;
+    LaunchInfo li{};
+    MM_CUDA(c, launch_step_mma(c->view, list, k_new, v_new, q, out, lse, sm_scale, grid, c->pdl_opt != 0,
+                               (cudaStream_t)stream, &li));
+    note(c, li);
+    const int32_t p = c->desc.page_size;
+    for (int i = 0; i < n_seqs; ++i) {  // host mirror of the append (validated by check_step) ...
+      HostSeq& hs = c->seqs[seq_ids[i]];
+      c->free_pages -= blocks_for(hs.sp.len + 1, p) - blocks_for(hs.sp.len, p);
+      hs.sp.len += 1;
+    }
+    mirror_evict(c, seq_ids, n_seqs);  // ... and of the eviction
+    c->stats.append_calls += 1;
+    c->stats.attn_calls += 1;
+    c->stats.attn_grid = li.grid;
+    c->stats.attn_smem_bytes = li.smem;
+    c->stats.attn_variant = variant;
+    return MURMUR_OK;
+  }
   const bool fuse = c->fuse_step_opt != 0;  // n_seqs <= 128 (check_step): one append launch
   st = append_impl(c, seq_ids, ones, n_seqs, k_new, v_new, 0, c->desc.n_layers, fuse, stream);
   if (st != MURMUR_OK) return st;
@@ -611,7 +638,8 @@ murmur_status_t murmur_set_option(murmur_cache_t* c, int32_t option, int32_t val
       c->pdl_opt = value != 0;
       return MURMUR_OK;
     case MURMUR_OPT_FUSE_STEP:
-      c->fuse_step_opt = value != 0;
+      if (value < 0 || value > 2) return MURMUR_ERR_INVALID_ARG;
+      c->fuse_step_opt = value;
       return MURMUR_OK;
     default:
       return MURMUR_ERR_INVALID_ARG;

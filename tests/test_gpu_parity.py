@@ -321,9 +321,10 @@ def test_decode_step_host_matches_device_calls(dev):
 
 
 # -------------------------------------------------------------------------------- fused step / PDL
-@pytest.mark.parametrize("pdl,fuse", [(1, 1), (0, 1), (1, 0), (0, 0)])
+@pytest.mark.parametrize("pdl,fuse", [(1, 2), (0, 2), (1, 1), (0, 1), (1, 0), (0, 0)])
 def test_decode_step_fused_prologue_ragged_every_step(dev, pdl, fuse):
-    """murmur_decode_step (append+evict in one launch, attention programmatically dependent) on a
+    """murmur_decode_step (fuse 2: the whole step in one launch; 1: append+evict in one launch, then
+    attention; 0: three launches; each with / without programmatic dependent launch) on a
     ragged page-16 batch whose windows start sliding and whose sequences finish at different steps:
     integer state bit-exact after every step, attention within tolerance, for every option mix."""
     from paper_2606_01483_b200 import MURMUR_OPT_FUSE_STEP, MURMUR_OPT_PDL
