@@ -49,6 +49,10 @@ static_assert(kFragFloats >= kScratchFloats, "the two merge layouts share one bu
 struct __align__(128) SmemLayout {
   uint8_t kv[kStages][2][kTileBytes];
   uint8_t q[2][kQBytes];
+  // step mode: this step's K row and V row of the current item (natural layout).  Processed as a
+  // 16-row tile of which only row 0 is valid; the rows "behind" it are whatever follows in shared
+  // memory (masked), so this must stay in front of a >= 4 KB member.
+  uint8_t newrow[2][2][kRowBytes];
   float scratch[kSliceWarps][kFragFloats];  // group merge (fragment layout), then slice merge (o[8][132], m, l)
   unsigned long long full_k[kStages], full_v[kStages], empty[kStages], q_full[2], q_empty[2];
   int meta[kStages][2];  // row_begin, row_end of the tile in each stage
@@ -60,6 +64,7 @@ struct __align__(128) SmemLayout {
   TileGen tg[kMaxSeqsAttn];      // runs + tile offsets of each sequence (closed form of sp)
   int old_nblk[kMaxSeqsAttn];    // blocks mapped in the block table when the kernel starts
   int newpage[kMaxSeqsAttn];     // step mode: page this step's append maps for the new block, else -1
+  int newatt[kMaxSeqsAttn];      // step mode: 1 if this step's token is in the retained set
   int blk_total;                      // step mode: pages this step's append pops
   int abort;
 };
@@ -284,6 +289,11 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     }
     s.nt[i] = s.tg[i].n_tiles;
 #endif
+    int last_b = 0;
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+      if (s.tg[i].rr.mask >> k & 1u) last_b = max(last_b, s.tg[i].rr.b[k]);
+    s.newatt[i] = (kStep && last_b == sp.len) ? 1 : 0;
   }
   __syncthreads();
   if (warp == 0) {  // prefix sums over <= 64 sequences: tiles, and (step mode) new-block demand
@@ -394,7 +404,6 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       uint32_t dst[4], bytes[4];  // destination offset in the stage buffer, bytes to copy (0 = none)
       int row_begin, row_end;     // valid rows of the tile buffer
       uint32_t tx;                // bytes arriving through bulk copies, per K / V barrier
-      int has_new;                // step mode: the last row is this step's token (not in the pool yet)
     };
     auto prep = [&](const Cursor& cc, int tix) {
       const AttnLookup lk{c.block_table + (size_t)list.ids[cc.i] * c.max_blocks, s.old_nblk[cc.i], s.newpage[cc.i]};
@@ -406,14 +415,10 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       TileIssue ti;
       ti.row_begin = td.row_begin;
       ti.row_end = td.row_end;
-      // step mode: the newest token (position len - 1) is the last row of the item's last tile
-#ifdef MURMUR_EXP_NO_NEWROW
-      ti.has_new = 0 &&
-#else
-      ti.has_new =
-#endif
-          kStep && td.first_pos + (td.row_end - td.row_begin) - 1 == s.sp[cc.i].len - 1;
-      const int row_end_pool = td.row_end - ti.has_new;
+      // step mode: this step's token (if attended) is the last row of the item's last tile; it is not
+      // in the pool yet and is handled apart (newrow), so the tile ends one row earlier
+      const int row_end_pool = td.row_end - ((kStep && s.newatt[cc.i] && tix == s.nt[cc.i] - 1) ? 1 : 0);
+      ti.row_end = row_end_pool;
       ti.tx = (uint32_t)(row_end_pool - td.row_begin) * kRowBytes;
       const int layer = prm.layer_begin + cc.layer;
 #pragma unroll
@@ -436,46 +441,30 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     int item_no = 0;
     TileIssue ti;
     if (lane < cnt) ti = prep(cur, cur.k + lane);
-    uint4 new_row = make_uint4(0u, 0u, 0u, 0u);
-#ifdef MURMUR_EXP_TRACE_FIRST
-    if (lane == 0) trace[2] = globaltimer_ns();
-#endif
     while (remaining > 0) {
       // ---- issue the current batch ----
-      if (base == 0) {  // first batch of an item (or of this CTA's segment of it)
-        if (lane == 0) {  // stage its G query rows
-          const int qb = item_no & 1;
-          mbar_wait(&s.q_empty[qb], ((item_no >> 1) & 1) ^ 1);
-          const size_t row = ((size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i) * c.n_q + (size_t)cur.h * G;
-          mbar_expect_tx(&s.q_full[qb], (uint32_t)(G * kRowBytes));
-          bulk_g2s(&s.q[qb][0], prm.q + row * kHeadDim, (uint32_t)(G * kRowBytes), &s.q_full[qb]);
-        }
-        if (kStep) {
-          // this step's K and V rows of the item, straight from k_new / v_new into registers
-          // (lane = (K|V, 16-byte chunk)); stored into the stage buffer when the last tile is issued
-          const size_t src_row = ((size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i) * n_kv + cur.h;
-          new_row = reinterpret_cast<const uint4*>((lane >> 4) ? prm.v_new : prm.k_new)[src_row * 16 + (lane & 15)];
+      if (base == 0 && lane == 0) {  // first batch of an item (or of this CTA's segment of it)
+        // stage its G query rows and, in step mode, this step's K / V rows of the item when this
+        // CTA's segment ends with the item's last tile (natural layout, straight from k_new / v_new)
+        const int qb = item_no & 1;
+        mbar_wait(&s.q_empty[qb], ((item_no >> 1) & 1) ^ 1);
+        const bool mini = kStep && s.newatt[cur.i] && (cur.k + seg == s.nt[cur.i]);
+        const size_t seq_row = (size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i;
+        mbar_expect_tx(&s.q_full[qb], (uint32_t)((G + (mini ? 2 : 0)) * kRowBytes));
+        bulk_g2s(&s.q[qb][0], prm.q + (seq_row * c.n_q + (size_t)cur.h * G) * kHeadDim, (uint32_t)(G * kRowBytes),
+                 &s.q_full[qb]);
+        if (mini) {
+          const size_t off = (seq_row * n_kv + cur.h) * kHeadDim;
+          bulk_g2s(&s.newrow[qb][0][0], prm.k_new + off, (uint32_t)kRowBytes, &s.q_full[qb]);
+          bulk_g2s(&s.newrow[qb][1][0], prm.v_new + off, (uint32_t)kRowBytes, &s.q_full[qb]);
         }
       }
-      // only the item's last tile can end with this step's token
-      const int j_last = kStep ? (s.nt[cur.i] - 1) - (cur.k + base) : -1;
       for (int j = 0; j < cnt; ++j) {
-        bool has_new = false;
-        if (kStep && j == j_last) {
-          has_new = __shfl_sync(0xffffffffu, ti.has_new, j) != 0;
-          if (has_new) {
-            if (lane == j) mbar_wait(&s.empty[st], ph ^ 1u);
-            __syncwarp();
-            const int r = __shfl_sync(0xffffffffu, ti.row_end, j) - 1;
-            *reinterpret_cast<uint4*>(&s.kv[st][lane >> 4][r * kRowBytes + (((lane & 15) ^ (r & 7)) << 4)]) = new_row;
-            __syncwarp();  // the stores are ordered before lane j's (releasing) arrive below
-          }
-        }
         if (lane == j) {
-          if (!has_new) mbar_wait(&s.empty[st], ph ^ 1u);
+          mbar_wait(&s.empty[st], ph ^ 1u);
           s.meta[st][0] = ti.row_begin;
           s.meta[st][1] = ti.row_end;
-          mbar_expect_tx(&s.full_k[st], ti.tx);  // 0 bytes (a tile that is only the new row) = plain arrive
+          mbar_expect_tx(&s.full_k[st], ti.tx);  // 0 bytes (a tile that held only the new row) = plain arrive
           mbar_expect_tx(&s.full_v[st], ti.tx);
 #pragma unroll
           for (int pg = 0; pg < 4; ++pg) {
@@ -553,24 +542,24 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       }
     }
     __syncwarp();
-    if (lane == 0) mbar_arrive(&s.q_empty[qb]);
+    // step mode: warp 0 also processes this step's token at the end of the item, from the same
+    // double buffer as the queries - it hands the buffer back only then
+    const bool mini = kStep && warp == 0 && s.newatt[cur.i] && (cur.k + seg == nt_i);
+    if (lane == 0 && !mini) mbar_arrive(&s.q_empty[qb]);
 
     float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
     float o[8][4];
 #pragma unroll
     for (int dt = 0; dt < 8; ++dt) o[dt][0] = o[dt][1] = o[dt][2] = o[dt][3] = 0.f;
 
-    for (int tt = (grp + kGroups - (int)(n % kGroups)) % kGroups; tt < seg; tt += kGroups) {
-      const uint32_t nn = n + (uint32_t)tt;
-      const int st = (int)(nn % kStages);
-      const uint32_t ph = (nn / kStages) & 1u;
-      mbar_wait(&s.full_k[st], ph);
-      const int rb = s.meta[st][0], re = s.meta[st][1];
+    // One 16-row slice of a tile whose K / V buffers start at kbase / vbase (shared-memory
+    // addresses of row 0), valid rows [rb, re).  v_ready: barrier the V data arrives on, or null.
+    auto slice = [&](uint32_t kbase, uint32_t vbase, int rb, int re, unsigned long long* v_ready, uint32_t ph) {
       const bool act = (slice0 < re) && (slice0 + 16 > rb);  // warp-uniform: the slice holds valid rows
       uint32_t pb0 = 0u, pb1 = 0u;
       if (act) {
         // ---- S^T[16 x 8] = K Q^T, two independent accumulator chains ----
-        const uint32_t rowaddr = smem_u32(&s.kv[st][0][0]) + k_off;
+        const uint32_t rowaddr = kbase + k_off;
         float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int ks = 0; ks < 8; ks += 2) {
@@ -612,9 +601,9 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         pb1 = movmatrix_t(pack_bf16(p2, p3));
       }
       // ---- O^T[128 x 8] += V^T P^T over this warp's 16 rows ----
-      mbar_wait(&s.full_v[st], ph);
+      if (v_ready != nullptr) mbar_wait(v_ready, ph);
       if (act) {
-        const uint32_t rowaddr = smem_u32(&s.kv[st][1][0]) + v_off;
+        const uint32_t rowaddr = vbase + v_off;
         const bool edge = (slice0 < rb) || (slice0 + 16 > re);
         uint32_t mk01 = 0xffffffffu, mk23 = 0xffffffffu;
         if (edge) {  // rows outside [rb, re) were never copied: zero them in the A fragment
@@ -630,8 +619,21 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
           mma_bf16(o[dt], a, pb0, pb1);
         }
       }
+    };
+
+    for (int tt = (grp + kGroups - (int)(n % kGroups)) % kGroups; tt < seg; tt += kGroups) {
+      const uint32_t nn = n + (uint32_t)tt;
+      const int st = (int)(nn % kStages);
+      const uint32_t ph = (nn / kStages) & 1u;
+      mbar_wait(&s.full_k[st], ph);
+      slice(smem_u32(&s.kv[st][0][0]), smem_u32(&s.kv[st][1][0]), s.meta[st][0], s.meta[st][1], &s.full_v[st], ph);
       __syncwarp();
       if (lane == 0) mbar_arrive(&s.empty[st]);
+    }
+    if (mini) {  // warp 0 (slice0 == 0): a tile whose only valid row, row 0, is this step's token
+      slice(smem_u32(&s.newrow[qb][0][0]), smem_u32(&s.newrow[qb][1][0]), 0, 1, nullptr, 0u);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&s.q_empty[qb]);
     }
     n += (uint32_t)seg;
 
@@ -791,6 +793,14 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     }
     consumer_bar();  // scratch and flag are reused by the next segment
 
+#ifdef MURMUR_EXP_ITEMLOG
+    if (blockIdx.x == 5 && tid == 0 && item_no < 60) {
+      c.timeline[(size_t)(512 + item_no) * kTimelineWords + 0] = globaltimer_ns();
+      c.timeline[(size_t)(512 + item_no) * kTimelineWords + 1] = globaltimer_ns();
+      c.timeline[(size_t)(512 + item_no) * kTimelineWords + 2] = 0;
+      c.timeline[(size_t)(512 + item_no) * kTimelineWords + 3] = seg;
+    }
+#endif
     remaining -= seg;
     pos += seg;
     first_segment = false;
