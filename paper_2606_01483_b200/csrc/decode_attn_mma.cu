@@ -65,6 +65,8 @@ struct __align__(128) SmemLayout {
   int old_nblk[kMaxSeqsAttn];    // blocks mapped in the block table when the kernel starts
   int newpage[kMaxSeqsAttn];     // step mode: page this step's append maps for the new block, else -1
   int newatt[kMaxSeqsAttn];      // step mode: 1 if this step's token is in the retained set
+  int tokpage[kMaxSeqsAttn];     // step mode: page this step's token is written to (read BEFORE the ticket: the
+                                 // eviction of the same step may unmap that very block)
   int blk_total;                      // step mode: pages this step's append pops
   int abort;
 };
@@ -277,6 +279,10 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     s.sp[i] = sp;
     s.old_nblk[i] = old_nblk;
     s.newpage[i] = -1;
+    if (kStep) {
+      const int xb = (sp.len - 1) >> plog;
+      s.tokpage[i] = xb < old_nblk ? c.block_table[(size_t)list.ids[i] * c.max_blocks + xb] : -1;
+    }
     // the tile table at this length was written by the last evict / decode step (SeqDev.tg);
     // generate it here only if it is missing (e.g. a bulk append that was not followed by an evict)
 #ifdef MURMUR_EXP_OLD_SETUP
@@ -316,8 +322,13 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         if (lane == 0) s.abort = 3;
       } else {
 #pragma unroll
-        for (int k = 0; k < 4; ++k)  // pops in call order (C3)
-          if (v[k]) s.newpage[lane * 4 + k] = c.free_stack[free_top - 1 - ex[k]];
+        for (int k = 0; k < 4; ++k) {  // pops in call order (C3)
+          if (v[k]) {
+            const int pg = c.free_stack[free_top - 1 - ex[k]];
+            s.newpage[lane * 4 + k] = pg;
+            s.tokpage[lane * 4 + k] = pg;
+          }
+        }
       }
       if (lane == 0) s.blk_total = blk_all;
     }
@@ -359,8 +370,8 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         const unsigned is_v = u >= per_kv, r = is_v ? u - per_kv : u;
         const unsigned r2 = r / (unsigned)n_kv, h = r - r2 * (unsigned)n_kv;
         const unsigned lc = r2 / (unsigned)n_seqs, i = r2 - lc * (unsigned)n_seqs;
-        const int x = s.sp[i].len - 1, b = x >> plog, slot = x & (p - 1);
-        const int page = b < s.old_nblk[i] ? c.block_table[(size_t)list.ids[i] * c.max_blocks + b] : s.newpage[i];
+        const int slot = (s.sp[i].len - 1) & (p - 1);
+        const int page = s.tokpage[i];
         if (page < 0) {
           atomicCAS(&c.ctrl[kCtrlError], 0, 2);
           continue;
@@ -555,7 +566,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     // One 16-row slice of a tile whose K / V buffers start at kbase / vbase (shared-memory
     // addresses of row 0), valid rows [rb, re).  v_ready: barrier the V data arrives on, or null.
     auto slice = [&](uint32_t kbase, uint32_t vbase, int rb, int re, unsigned long long* v_ready, uint32_t ph) {
-      const bool act = (slice0 < re) && (slice0 + 16 > rb);  // warp-uniform: the slice holds valid rows
+      const bool act = max(slice0, rb) < min(slice0 + 16, re);  // warp-uniform: the slice holds a valid row (a tile may be empty)
       uint32_t pb0 = 0u, pb1 = 0u;
       if (act) {
         // ---- S^T[16 x 8] = K Q^T, two independent accumulator chains ----

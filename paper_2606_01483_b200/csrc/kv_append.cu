@@ -83,12 +83,12 @@ constexpr int kAppendThreads = 256;  // small enough to be co-resident with an a
 // One half-warp moves one 256-byte row (16 lanes x 16 bytes).  Unit u of a call = (K|V, layer, token, head).
 struct RowUnit {
   const uint4* src;
-  int page;              // loaded, not yet consumed: dst() is the first use
-  int layer, head, slot, sub, is_v;
+  int page;               // loaded, not yet consumed: dst() is the first use
+  int is_v;
+  size_t off0;            // byte offset of the destination chunk in a pool, without the page term
   __device__ __forceinline__ uint4* dst(const CacheView& c) const {
-    // pre-swizzled row (see device_state.cuh)
     uint8_t* pool = reinterpret_cast<uint8_t*>(is_v ? c.v_pool : c.k_pool);
-    return reinterpret_cast<uint4*>(pool + row_offset(c, layer, page, head, slot)) + (sub ^ (slot & 7));
+    return reinterpret_cast<uint4*>(pool + off0 + (size_t)page * ((size_t)c.n_kv * c.p * kRowBytes));
   }
 };
 
@@ -124,7 +124,9 @@ __device__ __forceinline__ RowUnit locate_row(const CacheView& c, const AppendLi
   if (b < s_old_nblk[i]) ru.page = c.block_table[(size_t)list.ids[i] * c.max_blocks + b];
   else ru.page = c.free_stack[free_top - 1 - (s_blk_off[i] + (b - s_old_nblk[i]))];
   ru.src = (is_v ? v_new : k_new) + r * 16 + sub;
-  ru.layer = layer; ru.head = head; ru.slot = slot; ru.sub = sub; ru.is_v = is_v;
+  ru.is_v = is_v;
+  // pre-swizzled row (see device_state.cuh): chunk `sub` of slot `slot` sits at position sub ^ (slot & 7)
+  ru.off0 = row_offset(c, layer, 0, head, slot) + (size_t)((sub ^ (slot & 7)) << 4);
   return ru;
 }
 
@@ -269,10 +271,25 @@ append_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Appen
     }
     if (u < units && ru.page >= 0) *ru.dst(c) = val;
   } else {
-    for (long long u = (long long)blockIdx.x * units_per_cta + (tid >> 4); u < units; u += unit_stride) {
-      const RowUnit ru = locate_row(c, list, u, rows_src, total_tokens, layer_begin, n, free_top, sub, k_new, v_new,
-                                    s_tok_off, s_blk_off, s_old_nblk, s_sp);
-      if (ru.page >= 0) *ru.dst(c) = *ru.src; else bad_page = 1;
+    // four rows in flight per half-warp: all page lookups and source loads first, then the stores
+    for (long long u0 = (long long)blockIdx.x * units_per_cta + (tid >> 4); u0 < units; u0 += 4 * unit_stride) {
+      RowUnit ru[4];
+      uint4 val[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const long long u = u0 + k * unit_stride;
+        ru[k].page = -2;  // no row
+        if (u < units) {
+          ru[k] = locate_row(c, list, u, rows_src, total_tokens, layer_begin, n, free_top, sub, k_new, v_new, s_tok_off,
+                             s_blk_off, s_old_nblk, s_sp);
+          val[k] = *ru[k].src;
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        if (ru[k].page >= 0) *ru[k].dst(c) = val[k];
+        else if (ru[k].page == -1) bad_page = 1;
+      }
     }
     if (fuse_evict) fused_evict_tasks(c, list, n, free_top, s_sp, s_blk_off, s_old_nblk);
     bad_page = __syncthreads_or(bad_page);  // every store above has consumed its page id

@@ -355,6 +355,59 @@ def test_decode_step_fused_prologue_ragged_every_step(dev, pdl, fuse):
     a.close()
 
 
+@pytest.mark.parametrize("seed", range(8))
+def test_decode_step_one_launch_random_policies(dev, seed):
+    """The one-launch step on random small cases: page 16/32/64, windows 0 / tiny / larger than the
+    sequence, speech sinks, a second prompt, output window 0 (the new token is appended but not
+    attended), sequences that start without an evict (tile table missing -> generated in the kernel),
+    new pages popped in the same step in which others are freed, reversed call order."""
+    rng = random.Random(900 + seed)
+    p = rng.choice([16, 32, 64])
+    n_seqs = rng.randint(1, 5)
+    seqs = []
+    for _ in range(n_seqs):
+        seqs.append(seq_spec(rng.randint(1, 70), rng.randint(0, 200), rng.randint(3, 70), rng.choice([0, 1, 7, 40, 64, 300]),
+                             rng.choice([0, 1, 5, 33, 100]), M=rng.choice([0, 0, 3]),
+                             delay=rng.choice([0, 1, 6, 20]), n_sink_speech=rng.choice([0, 0, 2, 9]),
+                             n_sink_out=rng.choice([0, 1, 4])))
+    cfg = Config(f"randstep{seed}", 70 + seed, Geometry(n_layers=2), p, tuple(seqs))
+    sbs = _mk(cfg, dev)
+    ids = list(range(n_seqs))
+    sbs.bulk_prefill(ids, 0, evict=bool(seed % 2))
+    active = list(ids)
+    step = 0
+    while active:
+        order = active[::-1] if step % 2 else list(active)
+        q, out, lse = sbs.fused_step(order, want_lse=True)
+        sbs.check_integer_state(active)
+        sbs.check_attention(order, q, out, lse)
+        for i in list(active):
+            if sbs.t_of(i) >= cfg.seqs[i].T:
+                sbs.gpu.seq_end(i)
+                sbs.oracle.seq_end(i)
+                active.remove(i)
+        step += 1
+    assert sbs.gpu.free_stack().tolist() == sbs.oracle.free_stack
+    assert len(sbs.oracle.free_stack) == sbs.oracle.N
+    sbs.close()
+
+
+def test_decode_step_more_than_64_sequences_falls_back(dev):
+    """n_seqs > 64 exceeds the step kernel's tables: murmur_decode_step takes the two-launch form and
+    the attention call is split in chunks; results are the same."""
+    specs = [seq_spec(4, 20 + (i % 7), 6, 16, 8, n_sink_out=1) for i in range(70)]
+    cfg = Config("many", 90, Geometry(n_layers=1), 16, tuple(specs))
+    sbs = _mk(cfg, dev)
+    ids = list(range(70))
+    sbs.bulk_prefill(ids, 1)
+    for _ in range(3):
+        q, out, lse = sbs.fused_step(ids, want_lse=True)
+        sbs.check_integer_state(ids)
+        sbs.check_attention(ids, q, out, lse, seq_subset=[0, 33, 63, 64, 69])
+    assert sbs.gpu.stats()["kernel_launches"] > 0
+    sbs.close()
+
+
 def test_decode_step_back_to_back_without_host_sync(dev):
     """200 fused steps enqueued back to back (PDL chain prologue -> attention -> prologue ...) with
     no host synchronisation in between; the final integer state and every step's output are
