@@ -155,8 +155,8 @@ def pick_workload(name: str):
         return workloads.config3(False), 1030
     if name == "config3b":
         return workloads.config3(True), 1030
-    if name == "config5":
-        return workloads.config5(), None
+    if name == "config5":  # the full-batch point: all 32 sequences active (windows already sliding for most)
+        return workloads.config5(), 700
     if name.startswith("sweep_"):  # sweep_<w_s>_<w_o>
         _, ws, wo = name.split("_")
         return workloads.config4(int(ws), int(wo)), 1100
@@ -275,15 +275,13 @@ def run_murmur(args):
     binding.lib()  # fail loudly if libmurmur.so is missing
 
     cfg, t0 = pick_workload(args.workload)
-    if cfg.config_id == 5:
-        raise SystemExit("config5 (ragged) is benchmarked by bench sweeps in a later round; use config2/3a/3b/sweep_*")
     g = cfg.geom
     K, W = args.steps, max(3, args.warmup)
     Ke, We = args.e2e_steps, 3
     n_steps_total = W + 2 * K + We + Ke + 1
     n_gen = min(n_steps_total, 1100)  # distinct pre-generated step inputs (re-used cyclically beyond that)
-    Tmax = max(s.T for s in cfg.seqs)
-    extra = max(2, t0 + n_steps_total + 2 - Tmax)  # a long --steps run decodes past the config's T
+    Tmin = min(s.T for s in cfg.seqs)
+    extra = max(2, t0 + n_steps_total + 2 - Tmin)  # a long --steps run decodes past the config's T
     B = cfg.batch
     ids = np.arange(B, dtype=np.int32)
 
@@ -509,13 +507,19 @@ def run_murmur(args):
         "metric": METRIC, "value": us_step, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": cfg.name, "batch": B, "n_layers": g.n_layers, "n_q_heads": g.n_q_heads,
-                   "n_kv_heads": g.n_kv_heads, "head_dim": g.head_dim, "page_size": cfg.page_size,
-                   "speech_tokens": cfg.seqs[0].S, "prefix_tokens": cfg.seqs[0].P, "w_speech": cfg.seqs[0].w_speech,
-                   "w_out": cfg.seqs[0].w_out, "delay": cfg.seqs[0].delay, "n_sink_out": cfg.seqs[0].n_sink_out,
-                   "retained_tokens_per_seq": n_ret // B, "t_first_timed": t0 + W + 1,
-                   "l2": "inputs larger than L2 (each step re-reads %.0f MB of K/V)" % (kv_bytes / 1e6),
-                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "config": dict({"workload": cfg.name, "batch": B, "n_layers": g.n_layers, "n_q_heads": g.n_q_heads,
+                        "n_kv_heads": g.n_kv_heads, "head_dim": g.head_dim, "page_size": cfg.page_size,
+                        "retained_tokens_per_seq": n_ret // B, "t_first_timed": t0 + W + 1,
+                        "l2": "inputs larger than L2 (each step re-reads %.0f MB of K/V)" % (kv_bytes / 1e6),
+                        "parallelism": "replicas only" if world > 1 else "single GPU"},
+                       **({"speech_tokens": cfg.seqs[0].S, "prefix_tokens": cfg.seqs[0].P,
+                           "w_speech": cfg.seqs[0].w_speech, "w_out": cfg.seqs[0].w_out, "delay": cfg.seqs[0].delay,
+                           "n_sink_out": cfg.seqs[0].n_sink_out}
+                          if len({(x.S, x.w_speech, x.w_out) for x in cfg.seqs}) == 1 else
+                          {"ragged": True, "speech_tokens": [min(x.S for x in cfg.seqs), max(x.S for x in cfg.seqs)],
+                           "prefix_tokens": cfg.seqs[0].P, "w_speech": sorted({x.w_speech for x in cfg.seqs}),
+                           "w_out": sorted({x.w_out for x in cfg.seqs}), "n_sink_out": cfg.seqs[0].n_sink_out,
+                           "note": "all sequences kept active at a common t (the full-batch point of config 5)"})),
         "tokens_per_s": world * B / (us_step * 1e-6),
         "step_kernel_us": t_stepk, "launches_per_step": launches_per_step_b1,
         "separate_calls": {"append_us": t_app, "evict_us": t_evi, "attn_us": t_att, "attn_median_us": t_att_med,

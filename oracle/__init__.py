@@ -20,6 +20,9 @@ What it computes (PAPER.md = /root/reference/PAPER.md):
 * ``attention``    - Eq. 1: exact max-subtracted softmax attention over
                      the retained set in fp64, GQA head map h -> h // G, and the
                      log-sum-exp merge of partial results.
+* ``sparsity``     - the attention-sparsity profile of PAPER.md:77 / Fig. 5: the
+                     fewest tokens holding 99 % of a head's attention mass, split by region, and
+                     the mass a candidate window policy preserves.
 * ``cost_model``   - Eq. 3 theoretical attention-cost ratio.
 * ``c/``           - a plain C twin of ``attention`` (fp64, optional OpenMP) used for the
                      timed CPU baseline; checked against ``attention`` in tests.

@@ -256,11 +256,21 @@ def test_config5_ragged_two_layers_sequences_finish_at_different_steps(dev):
 
 # -------------------------------------------------------------------------------- full-size, sampled
 def _full_size_steps(sbs, ids, n_steps, sample_layers, seq_subset):
+    """Full-size steps in the launch configuration bench.py times: first as three API calls, then the
+    same number of steps through murmur_decode_step (one launch per step)."""
     for _ in range(n_steps):
         sbs.append_step(ids)
         sbs.evict(ids)
         sbs.check_integer_state(ids)
         q, out, lse = sbs.attend(ids, want_lse=True)
+        assert torch.isfinite(out.float()).all()
+        sbs.check_attention(ids, q, out, lse, layers=sample_layers, seq_subset=seq_subset)
+    launches0 = sbs.gpu.stats()["kernel_launches"]
+    for k in range(n_steps):
+        q, out, lse = sbs.fused_step(ids, want_lse=True)
+        if k == 0:
+            assert sbs.gpu.stats()["kernel_launches"] == launches0 + 1, "murmur_decode_step must be ONE launch"
+        sbs.check_integer_state(ids)
         assert torch.isfinite(out.float()).all()
         sbs.check_attention(ids, q, out, lse, layers=sample_layers, seq_subset=seq_subset)
 
