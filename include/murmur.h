@@ -194,6 +194,35 @@ MURMUR_API murmur_status_t murmur_decode_step_host(murmur_cache_t* cache, const 
                                                    const void* k_new_host, const void* v_new_host,
                                                    const void* q_host, void* out_host, float sm_scale, void* stream);
 
+/* ---- analysis: attention-sparsity profile (Fig. 5 at PAPER.md:85) ----------------- */
+/* Per (layer, sequence, query head), over the RESIDENT positions of the cache (everything not dead;
+ * run the cache with MURMUR_WINDOW_OFF to profile full attention):
+ *   n_*        tokens per region: prompt = both system prompts, speech, text = output tokens
+ *   k_mass     size of the FEWEST-token set whose Eq. 1 weights sum to >= mass_frac of the total
+ *              (weights descending, ties by ascending position); k_prompt/k_speech/k_text = its
+ *              members per region ("kept" of Fig. 5; "evictable" = n_* - k_*)
+ *   mass_*     attention mass per region;  coverage = mass inside the retained set A(t) of the
+ *              candidate policy (what a window policy would preserve at this step) */
+typedef struct {
+  int32_t n_resident, n_prompt, n_speech, n_text;
+  int32_t k_mass, k_prompt, k_speech, k_text;
+  float coverage, mass_prompt, mass_speech, mass_text;
+} murmur_profile_t;
+
+/* Bytes of DEVICE scratch murmur_attn_profile needs for these sequences and layers (0 on bad arguments). */
+MURMUR_API size_t murmur_profile_scratch_bytes(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                               int32_t layer_begin, int32_t layer_end);
+/* q        : DEVICE bf16 [layer_end-layer_begin][n_seqs][n_q_heads][head_dim] (the step's queries)
+ * candidate: HOST policy whose A(t) `coverage` is measured against, or NULL = each sequence's own
+ * mass_frac: in (0, 1], the paper uses 0.99
+ * out      : DEVICE murmur_profile_t [layer_end-layer_begin][n_seqs][n_q_heads]
+ * scratch  : DEVICE, >= murmur_profile_scratch_bytes(); n_seqs <= MURMUR_MAX_SEQS_PER_LAUNCH.
+ * Reads the cache only (any time after an append; no evict needed); softmax in fp32, sums in fp64. */
+MURMUR_API murmur_status_t murmur_attn_profile(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                               const void* q, const murmur_policy_t* candidate, float mass_frac,
+                                               void* out, void* scratch, size_t scratch_bytes, int32_t layer_begin,
+                                               int32_t layer_end, float sm_scale, void* stream);
+
 /* ---- introspection (tests; each call synchronises the stream it is given) ------------------ */
 /* state_out[0..5] = length, t, n_live_blocks, n_runs, n_attn_tiles, n_retained (device values). */
 MURMUR_API murmur_status_t murmur_seq_get_state(murmur_cache_t* cache, int32_t seq, int32_t* state_out, void* stream);

@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = [
     "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
     "murmur_decode_step", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
-    "murmur_debug_attn_timeline", "murmur_debug_step_trace",
+    "murmur_debug_attn_timeline", "murmur_debug_step_trace", "murmur_profile_scratch_bytes", "murmur_attn_profile",
     "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
     "murmur_last_cuda_error", "murmur_version",
 ]
@@ -97,6 +97,9 @@ def lib() -> C.CDLL:
     L.murmur_get_last_error.argtypes = [vp, vp, vp]
     L.murmur_debug_attn_timeline.argtypes = [vp, vp, i32, vp, vp]
     L.murmur_debug_step_trace.argtypes = [vp, vp, vp]
+    L.murmur_profile_scratch_bytes.argtypes = [vp, vp, i32, i32, i32]
+    L.murmur_profile_scratch_bytes.restype = C.c_size_t
+    L.murmur_attn_profile.argtypes = [vp, vp, i32, vp, vp, C.c_float, vp, vp, C.c_size_t, i32, i32, C.c_float, vp]
     L.murmur_set_option.argtypes = [vp, i32, i32]
     L.murmur_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.murmur_reset_stats.argtypes = [vp]
@@ -207,6 +210,30 @@ class MurmurCache:
                                               lse.data_ptr() if lse is not None else None, layer_begin, layer_end,
                                               C.c_float(sm_scale), _stream()))
         return out
+
+    def attn_profile(self, seq_ids, q: torch.Tensor, candidate=None, mass_frac: float = 0.99,
+                     sm_scale: Optional[float] = None, layer_begin: int = 0, layer_end: Optional[int] = None) -> np.ndarray:
+        """Attention-sparsity profile of the step whose queries are q: structured array
+        [layers, n_seqs, n_q] with the fields of murmur_profile_t.  candidate: 5-tuple policy or None."""
+        layer_end = self.n_layers if layer_end is None else layer_end
+        ids = _ids(seq_ids)
+        shape = (layer_end - layer_begin, len(ids), self.n_q, self.d)
+        assert q.dtype == torch.bfloat16 and q.is_cuda and q.is_contiguous() and tuple(q.shape) == shape
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        nbytes = self.L.murmur_profile_scratch_bytes(self.h, ids.ctypes.data, len(ids), layer_begin, layer_end)
+        if nbytes == 0:
+            raise MurmurError("murmur_profile_scratch_bytes: bad arguments")
+        scratch = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        out = torch.zeros(shape[:3] + (12,), dtype=torch.int32, device=self.device)
+        pol = (C.c_int32 * 5)(*candidate) if candidate is not None else None
+        self._check(self.L.murmur_attn_profile(self.h, ids.ctypes.data, len(ids), q.data_ptr(), pol, C.c_float(mass_frac),
+                                               out.data_ptr(), scratch.data_ptr(), nbytes, layer_begin, layer_end,
+                                               C.c_float(sm_scale), _stream()))
+        torch.cuda.synchronize(self.device)
+        dt = np.dtype([(n, np.int32) for n in ("n_resident", "n_prompt", "n_speech", "n_text", "k_mass", "k_prompt",
+                                               "k_speech", "k_text")] +
+                      [(n, np.float32) for n in ("coverage", "mass_prompt", "mass_speech", "mass_text")])
+        return out.cpu().numpy().view(dt).reshape(shape[:3])
 
     def decode_step(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor, out: torch.Tensor,
                     lse: Optional[torch.Tensor] = None, sm_scale: Optional[float] = None):

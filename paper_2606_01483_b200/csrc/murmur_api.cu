@@ -478,6 +478,51 @@ murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_id
   return MURMUR_OK;
 }
 
+// ---- analysis -----------------------------------------------------------------------------------
+static long long profile_stride(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs) {
+  int32_t mx = 1;
+  for (int i = 0; i < n_seqs; ++i) mx = c->seqs[seq_ids[i]].sp.len > mx ? c->seqs[seq_ids[i]].sp.len : mx;
+  return ((long long)mx + 31) / 32 * 32;
+}
+
+size_t murmur_profile_scratch_bytes(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, int32_t layer_begin,
+                                    int32_t layer_end) {
+  if (!c || n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch) return 0;
+  if (check_ids(c, seq_ids, n_seqs) != MURMUR_OK) return 0;
+  if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return 0;
+  return (size_t)(layer_end - layer_begin) * n_seqs * c->desc.n_q_heads * (size_t)profile_stride(c, seq_ids, n_seqs) * 4;
+}
+
+murmur_status_t murmur_attn_profile(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q,
+                                    const murmur_policy_t* cand, float mass_frac, void* out, void* scratch,
+                                    size_t scratch_bytes, int32_t layer_begin, int32_t layer_end, float sm_scale,
+                                    void* stream) {
+  if (!c || !q || !out || !scratch) return MURMUR_ERR_INVALID_ARG;
+  if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs);
+  if (st != MURMUR_OK) return st;
+  if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
+  if (!(sm_scale > 0.f) || !(mass_frac > 0.f) || mass_frac > 1.f) return MURMUR_ERR_INVALID_ARG;
+  if (cand && (cand->w_speech < 0 || cand->delay < 0 || cand->n_sink_speech < 0 || cand->w_out < 0 || cand->n_sink_out < 0))
+    return MURMUR_ERR_INVALID_ARG;
+  for (int i = 0; i < n_seqs; ++i)
+    if (c->seqs[seq_ids[i]].sp.len < 1) return MURMUR_ERR_STATE;
+  if (scratch_bytes < murmur_profile_scratch_bytes(c, seq_ids, n_seqs, layer_begin, layer_end)) return MURMUR_ERR_INVALID_ARG;
+  SeqList list;
+  list.n = n_seqs;
+  for (int i = 0; i < n_seqs; ++i) list.ids[i] = seq_ids[i];
+  SeqParams cs{};
+  if (cand) {
+    cs.w_s = cand->w_speech; cs.d = cand->delay; cs.k_s = cand->n_sink_speech; cs.w_o = cand->w_out; cs.k_o = cand->n_sink_out;
+  }
+  LaunchInfo li{};
+  MM_CUDA(c, launch_attn_profile(c->view, list, 0, n_seqs, q, cand ? &cs : nullptr, mass_frac, out,
+                                 reinterpret_cast<float*>(scratch), profile_stride(c, seq_ids, n_seqs), layer_begin,
+                                 layer_end, sm_scale, (cudaStream_t)stream, &li));
+  note(c, li);
+  return MURMUR_OK;
+}
+
 // ---- introspection ------------------------------------------------------------------------------
 static murmur_status_t check_seq(murmur_cache_t* c, int32_t seq) {
   if (!c) return MURMUR_ERR_INVALID_ARG;
