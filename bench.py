@@ -146,6 +146,23 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
+def max_over_ranks(values, dist, device):
+    """MAX over ranks of a list of floats (every timing is reported as the slowest rank's); identity
+    when dist is None.  Works with any torch.distributed backend (nccl on the GPUs, gloo in the CPU test)."""
+    import torch
+
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.tolist()]
+
+
+def whole_job_tokens_per_s(world: int, batch_per_rank: int, us_step: float) -> float:
+    """Replicas only: every rank decodes its own batch, one token per sequence
+    per step; the job's throughput is all ranks' tokens over the slowest rank's step time."""
+    return world * batch_per_rank / (us_step * 1e-6)
+
+
 def pick_workload(name: str):
     import workloads
 
@@ -451,11 +468,8 @@ def run_murmur(args):
 
     # ---- reduce over ranks ---------------------------------------------------------------------
     us_step = ms_a / K * 1e3
-    vals = torch.tensor([us_step, us_e2e, t_att, t_app, t_evi, t_att_med, t_stepk, t_stepk_med], dtype=torch.float64,
-                        device=dev)
-    if dist is not None:
-        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
-    us_step, us_e2e, t_att, t_app, t_evi, t_att_med, t_stepk, t_stepk_med = [float(x) for x in vals.tolist()]
+    us_step, us_e2e, t_att, t_app, t_evi, t_att_med, t_stepk, t_stepk_med = max_over_ranks(
+        [us_step, us_e2e, t_att, t_app, t_evi, t_att_med, t_stepk, t_stepk_med], dist, dev)
 
     # ---- algorithmic bytes of one attention launch ------------------------------
     # retained tokens per launch: the device's own |A(t)|, mean of the first and last step of region B
@@ -520,7 +534,7 @@ def run_murmur(args):
                            "prefix_tokens": cfg.seqs[0].P, "w_speech": sorted({x.w_speech for x in cfg.seqs}),
                            "w_out": sorted({x.w_out for x in cfg.seqs}), "n_sink_out": cfg.seqs[0].n_sink_out,
                            "note": "all sequences kept active at a common t (the full-batch point of config 5)"})),
-        "tokens_per_s": world * B / (us_step * 1e-6),
+        "tokens_per_s": whole_job_tokens_per_s(world, B, us_step),
         "step_kernel_us": t_stepk, "launches_per_step": launches_per_step_b1,
         "separate_calls": {"append_us": t_app, "evict_us": t_evi, "attn_us": t_att, "attn_median_us": t_att_med,
                            "attn_hbm_gbs": attn_only, "attn_pct_of_measured_peak": 100.0 * attn_only / peak,

@@ -285,16 +285,12 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     }
     // the tile table at this length was written by the last evict / decode step (SeqDev.tg);
     // generate it here only if it is missing (e.g. a bulk append that was not followed by an evict)
-#ifdef MURMUR_EXP_OLD_SETUP
-    s.nt[i] = sd.n_tiles;
-#else
     if (sd.tg_len[sp.len & 1] == sp.len) {
       s.tg[i] = sd.tg[sp.len & 1];
     } else {
       s.tg[i] = make_tilegen(sp, p, plog);
     }
     s.nt[i] = s.tg[i].n_tiles;
-#endif
     int last_b = 0;
 #pragma unroll
     for (int k = 0; k < 6; ++k)
@@ -350,9 +346,6 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     if (lane == 0) last = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
     last = __shfl_sync(0xffffffffu, last, 0);
     // (1) the eviction's table products for the post-append state, spread over the CTAs
-#ifdef MURMUR_EXP_NO_KEEPER
-    if (!last) return;
-#endif
     for (int task = (int)blockIdx.x; task < 2 * n_seqs; task += (int)gridDim.x) {
       const int role = 1 + task / n_seqs, i = task % n_seqs;
       const AttnLookup lk{c.block_table + (size_t)list.ids[i] * c.max_blocks, s.old_nblk[i], s.newpage[i]};
@@ -362,11 +355,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     {
       const int half = lane >> 4, sub = lane & 15;
       const unsigned per_kv = (unsigned)prm.n_layers_call * (unsigned)n_seqs * (unsigned)n_kv;
-#ifdef MURMUR_EXP_NO_SCATTER
-      for (unsigned u = 2u * per_kv; u < 2u * per_kv; u += 2u * gridDim.x) {
-#else
       for (unsigned u = 2u * blockIdx.x + half; u < 2u * per_kv; u += 2u * gridDim.x) {
-#endif
         const unsigned is_v = u >= per_kv, r = is_v ? u - per_kv : u;
         const unsigned r2 = r / (unsigned)n_kv, h = r - r2 * (unsigned)n_kv;
         const unsigned lc = r2 / (unsigned)n_seqs, i = r2 - lc * (unsigned)n_seqs;
@@ -418,11 +407,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     };
     auto prep = [&](const Cursor& cc, int tix) {
       const AttnLookup lk{c.block_table + (size_t)list.ids[cc.i] * c.max_blocks, s.old_nblk[cc.i], s.newpage[cc.i]};
-#ifdef MURMUR_EXP_LOAD_TILES
-      const TileDesc td = kStep ? tile_at(s.tg[cc.i], tix, p, plog, lk) : c.tiles[(size_t)list.ids[cc.i] * c.max_blocks + tix];
-#else
       const TileDesc td = tile_at(s.tg[cc.i], tix, p, plog, lk);
-#endif
       TileIssue ti;
       ti.row_begin = td.row_begin;
       ti.row_end = td.row_end;
@@ -804,14 +789,6 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     }
     consumer_bar();  // scratch and flag are reused by the next segment
 
-#ifdef MURMUR_EXP_ITEMLOG
-    if (blockIdx.x == 5 && tid == 0 && item_no < 60) {
-      c.timeline[(size_t)(512 + item_no) * kTimelineWords + 0] = globaltimer_ns();
-      c.timeline[(size_t)(512 + item_no) * kTimelineWords + 1] = globaltimer_ns();
-      c.timeline[(size_t)(512 + item_no) * kTimelineWords + 2] = 0;
-      c.timeline[(size_t)(512 + item_no) * kTimelineWords + 3] = seg;
-    }
-#endif
     remaining -= seg;
     pos += seg;
     first_segment = false;

@@ -651,11 +651,7 @@ murmur_status_t murmur_get_last_error(murmur_cache_t* c, int32_t* device_err_out
 murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* c, uint64_t* out, int32_t cap_ctas, int32_t* n_out,
                                            void* stream) {
   if (!c || !n_out || cap_ctas < 0 || (cap_ctas > 0 && !out)) return MURMUR_ERR_INVALID_ARG;
-#ifdef MURMUR_EXP_ITEMLOG
-  const int n = 600;
-#else
   const int n = c->stats.attn_variant == MURMUR_ATTN_MMA ? c->stats.attn_grid : 0;
-#endif
   *n_out = n;
   if (n > cap_ctas) return MURMUR_ERR_INVALID_ARG;
   MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
