@@ -174,6 +174,17 @@ MURMUR_API murmur_status_t murmur_decode_attn(murmur_cache_t* cache, const int32
                                               const void* q, void* out, float* lse, int32_t layer_begin,
                                               int32_t layer_end, float sm_scale, void* stream);
 
+/* Per-layer windows (sparsity differs by layer; "particularly in deeper layers"): the same
+ * as murmur_decode_attn, but the attended set of every listed sequence is the A(t) of `window` (HOST)
+ * instead of its own policy's - call it once per group of layers that share a window.  What is RESIDENT
+ * is still decided by each sequence's own policy (murmur_kv_evict), which therefore has to be the
+ * loosest one: `window` may not exceed it in any field (else MURMUR_ERR_INVALID_ARG), so that A_window(t)
+ * never touches an evicted position.  Tensor-core variant only (page_size >= 16). */
+MURMUR_API murmur_status_t murmur_decode_attn_windowed(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                                       const void* q, void* out, float* lse, int32_t layer_begin,
+                                                       int32_t layer_end, float sm_scale,
+                                                       const murmur_policy_t* window, void* stream);
+
 /* One whole decode step from DEVICE buffers: append one token to every listed sequence (all
  * layers) -> evict -> decode_attn, enqueued by ONE host call as ONE launch by default (see
  * MURMUR_OPT_FUSE_STEP; the result is identical for every setting) (PAPER.md:112-116, 136-146, 101-104:

@@ -190,6 +190,8 @@ struct AttnParams {
   float* lse;
   const uint16_t* k_new;  // step mode: [n_layers][n_seqs][n_kv][128] rows of this step's token
   const uint16_t* v_new;
+  int has_window;         // murmur_decode_attn_windowed: attend over the A(t) of THIS policy instead of the sequence's
+  int w_s, d, k_s, w_o, k_o;
   int seq_base, n_seqs_total, layer_begin, n_layers_call;
   float sm_scale;
 };
@@ -285,7 +287,11 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     }
     // the tile table at this length was written by the last evict / decode step (SeqDev.tg);
     // generate it here only if it is missing (e.g. a bulk append that was not followed by an evict)
-    if (sd.tg_len[sp.len & 1] == sp.len) {
+    if (!kStep && prm.has_window) {  // per-call window (e.g. per-layer windows): tables generated here
+      sp.w_s = prm.w_s; sp.d = prm.d; sp.k_s = prm.k_s; sp.w_o = prm.w_o; sp.k_o = prm.k_o;
+      s.sp[i] = sp;
+      s.tg[i] = make_tilegen(sp, p, plog);
+    } else if (sd.tg_len[sp.len & 1] == sp.len) {
       s.tg[i] = sd.tg[sp.len & 1];
     } else {
       s.tg[i] = make_tilegen(sp, p, plog);
@@ -828,8 +834,12 @@ cudaError_t launch_mma(const CacheView& c, const SeqList& list, const AttnParams
 
 cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                             void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
-                            bool pdl, cudaStream_t st, LaunchInfo* info) {
+                            bool pdl, const SeqParams* window, cudaStream_t st, LaunchInfo* info) {
   AttnParams prm{};
+  if (window != nullptr) {
+    prm.has_window = 1;
+    prm.w_s = window->w_s; prm.d = window->d; prm.k_s = window->k_s; prm.w_o = window->w_o; prm.k_o = window->k_o;
+  }
   prm.q = reinterpret_cast<const uint16_t*>(q);
   prm.out = reinterpret_cast<uint16_t*>(out);
   prm.lse = lse;

@@ -179,7 +179,7 @@ cudaError_t launch_attn_generic(const CacheView& c, const SeqList& list, int seq
                                 float sm_scale, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                             void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
-                            bool pdl, cudaStream_t st, LaunchInfo* info);
+                            bool pdl, const SeqParams* window, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void* k_new, const void* v_new,
                             const void* q, void* out, float* lse, float sm_scale, int grid, bool pdl, cudaStream_t st,
                             LaunchInfo* info);

@@ -353,8 +353,11 @@ murmur_status_t murmur_kv_evict(murmur_cache_t* c, const int32_t* seq_ids, int32
   return MURMUR_OK;
 }
 
-murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q, void* out,
-                                   float* lse, int32_t layer_begin, int32_t layer_end, float sm_scale, void* stream) {
+// window == nullptr: each sequence's own policy.  Otherwise the attended set is the A(t) of `window`
+// (same for all listed sequences), which must lie inside what the sequence's own policy keeps resident.
+static murmur_status_t attn_impl(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q, void* out,
+                                 float* lse, int32_t layer_begin, int32_t layer_end, float sm_scale,
+                                 const murmur_policy_t* window, void* stream) {
   if (!c) return MURMUR_ERR_INVALID_ARG;
   murmur_status_t st = check_ids(c, seq_ids, n_seqs);
   if (st != MURMUR_OK) return st;
@@ -362,14 +365,30 @@ murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, in
   if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
   if (n_seqs == 0) return MURMUR_OK;
   if (!q || !out) return MURMUR_ERR_INVALID_ARG;
+  SeqParams win{};
+  if (window) {
+    if (window->w_speech < 0 || window->delay < 0 || window->n_sink_speech < 0 || window->w_out < 0 || window->n_sink_out < 0)
+      return MURMUR_ERR_INVALID_ARG;
+    win.w_s = window->w_speech; win.d = window->delay; win.k_s = window->n_sink_speech;
+    win.w_o = window->w_out; win.k_o = window->n_sink_out;
+  }
   for (int i = 0; i < n_seqs; ++i) {
     const HostSeq& hs = c->seqs[seq_ids[i]];
     if (hs.sp.len < 1 || hs.evict_len != hs.sp.len) return MURMUR_ERR_STATE;
-    if (retained_count(hs.sp) < 1) return MURMUR_ERR_STATE;  // Eq. 1 over an empty set is undefined
+    SeqParams sp = hs.sp;
+    if (window) {
+      // A_window(t) must avoid every position the sequence's own policy has evicted: a window that
+      // trails no further back, a delay no longer, and no more sinks than the base policy's
+      if (win.w_s > sp.w_s || win.d > sp.d || win.k_s > sp.k_s || win.w_o > sp.w_o || win.k_o > sp.k_o)
+        return MURMUR_ERR_INVALID_ARG;
+      sp.w_s = win.w_s; sp.d = win.d; sp.k_s = win.k_s; sp.w_o = win.w_o; sp.k_o = win.k_o;
+    }
+    if (retained_count(sp) < 1) return MURMUR_ERR_STATE;  // Eq. 1 over an empty set is undefined
   }
   int variant = c->attn_variant_opt;
   if (variant == MURMUR_ATTN_AUTO) variant = (c->desc.page_size >= 16) ? MURMUR_ATTN_MMA : MURMUR_ATTN_GENERIC;
   if (variant == MURMUR_ATTN_MMA && c->desc.page_size < 16) return MURMUR_ERR_UNSUPPORTED;
+  if (window && variant != MURMUR_ATTN_MMA) return MURMUR_ERR_UNSUPPORTED;
   const int grid = c->attn_grid_opt > 0 ? c->attn_grid_opt : c->sm_count;
   const int chunk = (variant == MURMUR_ATTN_MMA) ? kMaxSeqsAttn : kMaxSeqsPerLaunch;
   for (int base = 0; base < n_seqs; base += chunk) {
@@ -379,7 +398,7 @@ murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, in
     LaunchInfo li{};
     if (variant == MURMUR_ATTN_MMA) {
       MM_CUDA(c, launch_attn_mma(c->view, list, base, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, grid,
-                                 c->pdl_opt != 0, (cudaStream_t)stream, &li));
+                                 c->pdl_opt != 0, window ? &win : nullptr, (cudaStream_t)stream, &li));
     } else {
       MM_CUDA(c, launch_attn_generic(c->view, list, base, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale,
                                      (cudaStream_t)stream, &li));
@@ -391,6 +410,18 @@ murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, in
   c->stats.attn_variant = variant;
   c->stats.attn_calls += 1;
   return MURMUR_OK;
+}
+
+murmur_status_t murmur_decode_attn(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q, void* out,
+                                   float* lse, int32_t layer_begin, int32_t layer_end, float sm_scale, void* stream) {
+  return attn_impl(c, seq_ids, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, nullptr, stream);
+}
+
+murmur_status_t murmur_decode_attn_windowed(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q,
+                                            void* out, float* lse, int32_t layer_begin, int32_t layer_end,
+                                            float sm_scale, const murmur_policy_t* window, void* stream) {
+  if (!window) return MURMUR_ERR_INVALID_ARG;
+  return attn_impl(c, seq_ids, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, window, stream);
 }
 
 // validates a 1-token-per-sequence append before anything is enqueued (all-or-nothing)

@@ -437,6 +437,56 @@ def test_decode_step_back_to_back_without_host_sync(dev):
     a.close()
 
 
+# -------------------------------------------------------------------------------- per-layer windows
+def test_decode_attn_windowed_per_layer_groups(dev):
+    """murmur_decode_attn_windowed: layers 0-1 attend a tighter window than layers 2-3 while residency
+    follows the sequences' own (loosest) policy; each group is checked against Eq. 1 over the A(t) of
+    ITS window, and a window equal to the base policy reproduces murmur_decode_attn bit for bit."""
+    from oracle import attention as o_attn
+    from oracle import policy as o_policy
+    from paper_2606_01483_b200 import MurmurError
+
+    specs = [seq_spec(9 + i, 150 + 20 * i, 80, 64, 40, delay=32, n_sink_speech=2, n_sink_out=4) for i in range(3)]
+    cfg = Config("winlayers", 95, Geometry(n_layers=4), 16, tuple(specs))
+    sbs = _mk(cfg, dev)
+    ids = [0, 1, 2]
+    sbs.bulk_prefill(ids, 50)
+    tight = (32, 16, 0, 16, 2)
+    base = specs[0].policy_tuple
+    for _ in range(4):
+        sbs.append_step(ids)
+        sbs.evict(ids)
+        sbs.check_integer_state(ids)
+        q = sbs.queries(ids)
+        lse = torch.empty(q.shape[:3], dtype=torch.float32, device=dev)
+        out = torch.empty_like(q)
+        sbs.gpu.decode_attn(ids, q[0:2].contiguous(), out=out[0:2], lse=lse[0:2], sm_scale=sbs.scale, layer_begin=0, layer_end=2, window=tight)
+        sbs.gpu.decode_attn(ids, q[2:4].contiguous(), out=out[2:4], lse=lse[2:4], sm_scale=sbs.scale, layer_begin=2, layer_end=4, window=base)
+        plain = sbs.gpu.decode_attn(ids, q[2:4].contiguous(), sm_scale=sbs.scale, layer_begin=2, layer_end=4)
+        assert torch.equal(plain, out[2:4]), "a window equal to the base policy must reproduce murmur_decode_attn (same split)"
+        got = out.float().cpu().numpy().astype(np.float64)
+        q_bits = workloads.to_bits(q)
+        errs = []
+        for j, i in enumerate(ids):
+            st = sbs.oracle.seqs[i]
+            kb, vb = sbs.kv_by_position(i)
+            for layer in range(4):
+                pol = o_policy.Policy(*(tight if layer < 2 else base))
+                ret = [x for x in o_policy.retained_positions(st.P, st.S, st.M, st.t, pol) if x < st.length]
+                assert set(ret) <= set(sbs.oracle.retained(i)) | set(o_policy.resident_positions(st.P, st.S, st.M, st.t, st.pol))
+                o_ref, lse_ref, _ = o_attn.attend_retained(q_bits[layer, j], kb[layer], vb[layer], ret, sbs.scale)
+                errs.append(np.abs(got[layer, j] - o_ref))
+                assert np.max(np.abs(lse[layer, j].cpu().numpy() - lse_ref)) < 2e-3
+        e = np.stack(errs)
+        assert e.max() <= 2e-2 and e.mean() <= 2e-3
+    # a window that reaches further back than the base policy could touch evicted positions: rejected
+    for bad in ((65, 32, 2, 40, 4), (64, 33, 2, 40, 4), (64, 32, 3, 40, 4), (64, 32, 2, 41, 4), (64, 32, 2, 40, 5)):
+        with pytest.raises(MurmurError):
+            sbs.gpu.decode_attn(ids, q, sm_scale=sbs.scale, window=bad)
+    assert sbs.gpu.last_error() == 0
+    sbs.close()
+
+
 # -------------------------------------------------------------------------------- errors
 def test_error_behaviour_leaves_state_unchanged(dev):
     from paper_2606_01483_b200 import MurmurCache, MurmurError
