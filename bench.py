@@ -430,6 +430,7 @@ def run_murmur(args):
     step_list = sorted(e[0].elapsed_time(e[1]) * 1e3 for e in evs1)
     t_stepk = sum(step_list) / K
     t_stepk_med = step_list[K // 2]
+    stepk_p10, stepk_p90 = step_list[K // 10], step_list[min(K - 1, (9 * K) // 10)]
     t_app = sum(e[0].elapsed_time(e[1]) for e in evs) / Kb2 * 1e3
     t_evi = sum(e[1].elapsed_time(e[2]) for e in evs) / Kb2 * 1e3
     attn_list = sorted(e[2].elapsed_time(e[3]) * 1e3 for e in evs)
@@ -535,7 +536,8 @@ def run_murmur(args):
                            "w_out": sorted({x.w_out for x in cfg.seqs}), "n_sink_out": cfg.seqs[0].n_sink_out,
                            "note": "all sequences kept active at a common t (the full-batch point of config 5)"})),
         "tokens_per_s": whole_job_tokens_per_s(world, B, us_step),
-        "step_kernel_us": t_stepk, "launches_per_step": launches_per_step_b1,
+        "step_kernel_us": t_stepk, "step_kernel_us_p10_p50_p90": [stepk_p10, t_stepk_med, stepk_p90],
+        "launches_per_step": launches_per_step_b1,
         "separate_calls": {"append_us": t_app, "evict_us": t_evi, "attn_us": t_att, "attn_median_us": t_att_med,
                            "attn_hbm_gbs": attn_only, "attn_pct_of_measured_peak": 100.0 * attn_only / peak,
                            "note": "the same step as three API calls, one event pair per call (includes launch gaps)"},
@@ -593,11 +595,16 @@ def oracle_sample(cfg, cache, k_seq0, v_seq0, ids, q_last, scale, t_now, dev, bu
         best = el if best is None else min(best, el)
     n_items = cfg.batch * g.n_layers
     us_step = (best / n_l * n_items + t_policy * cfg.batch) * 1e6
+    # the same oracle on ONE thread, on a slice small enough for ~2 s
+    n_l1 = int(max(1, min(n_l, 2.0 / max(per_layer * used, 1e-5))))
+    tc = time.perf_counter()
+    co.attend(q_bits[:n_l1], k_bits[:n_l1], v_bits[:n_l1], ret, scale, n_threads=1)
+    us_step_1t = ((time.perf_counter() - tc) / n_l1 * n_items + t_policy * cfg.batch) * 1e6
     e = np.abs(got[:n_l] - o_ref)
     parity = {"max_abs": float(e.max()), "mean_abs": float(e.mean()), "tol_max_abs": 2e-2, "tol_mean_abs": 2e-3,
               "compared": f"sequence 0, layers 0..{n_l - 1}, all {g.n_q_heads} heads of the last step (t={t_now}); "
                           "retained set bit-exact"}
-    cpu = {"value": us_step, "unit": UNIT, "cores": int(used), "kind": "oracle",
+    cpu = {"value": us_step, "unit": UNIT, "cores": int(used), "kind": "oracle", "single_thread_value": us_step_1t,
            "sample": f"oracle.policy retained set + plain-C fp64 attention (oracle/c) of sequence 0, layers 0..{n_l - 1} of "
                      f"the last step ({len(ret)} retained tokens), best of runs, scaled x{n_items / n_l:.1f} to the "
                      f"{n_items} (sequence, layer) items of a step; host cores = {os.cpu_count()}"}

@@ -23,6 +23,8 @@ What it computes (PAPER.md = /root/reference/PAPER.md):
 * ``sparsity``     - the attention-sparsity profile of PAPER.md:77 / Fig. 5: the
                      fewest tokens holding 99 % of a head's attention mass, split by region, and
                      the mass a candidate window policy preserves.
+* ``prefill``      - causal self-attention of the prefill tokens: Eq. 1 of each
+                     prefill position over the positions up to and including itself.
 * ``cost_model``   - Eq. 3 theoretical attention-cost ratio.
 * ``c/``           - a plain C twin of ``attention`` (fp64, optional OpenMP) used for the
                      timed CPU baseline; checked against ``attention`` in tests.

@@ -18,7 +18,7 @@ INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libmurmur.so")
 
 SOURCES = ["murmur_api.cu", "kv_append.cu", "kv_evict.cu", "decode_attn_generic.cu", "decode_attn_mma.cu", "attn_profile.cu"]
-HEADERS = ["device_state.cuh", "policy_math.cuh", "evict_body.cuh"]
+HEADERS = ["device_state.cuh", "policy_math.cuh", "evict_body.cuh", "ptx_utils.cuh"]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
