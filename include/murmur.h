@@ -205,6 +205,19 @@ MURMUR_API murmur_status_t murmur_decode_step_host(murmur_cache_t* cache, const 
                                                    const void* k_new_host, const void* v_new_host,
                                                    const void* q_host, void* out_host, float sm_scale, void* stream);
 
+/* ---- prefill ------------------------------------------------------------------------------- */
+/* Causal self-attention of prefill tokens: for the positions x in
+ * [pos_begin, pos_end) of `seq`, out[l][x - pos_begin][h] = Eq. 1 of query q_x over
+ * the cache positions y <= x.  The K/V of positions [0, pos_end) must already be appended for the
+ * given layers and none of them evicted (MURMUR_ERR_STATE otherwise) - call it after the bulk
+ * murmur_kv_append of the chunk and before the first murmur_kv_evict.
+ *   q, out : DEVICE bf16 [layer_end-layer_begin][pos_end-pos_begin][n_q_heads][head_dim]
+ *   lse    : DEVICE fp32 [layer_end-layer_begin][pos_end-pos_begin][n_q_heads] or NULL
+ * page_size >= 16.  First correct path: mma.sync tensor cores (not yet tcgen05). */
+MURMUR_API murmur_status_t murmur_prefill_attn(murmur_cache_t* cache, int32_t seq, int32_t pos_begin, int32_t pos_end,
+                                               const void* q, void* out, float* lse, int32_t layer_begin,
+                                               int32_t layer_end, float sm_scale, void* stream);
+
 /* ---- analysis: attention-sparsity profile (Fig. 5 at PAPER.md:85) ----------------- */
 /* Per (layer, sequence, query head), over the RESIDENT positions of the cache (everything not dead;
  * run the cache with MURMUR_WINDOW_OFF to profile full attention):

@@ -33,7 +33,7 @@ EXPORTED_SYMBOLS = [
     "murmur_decode_step", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
     "murmur_debug_attn_timeline", "murmur_debug_step_trace", "murmur_profile_scratch_bytes", "murmur_attn_profile",
-    "murmur_decode_attn_windowed",
+    "murmur_decode_attn_windowed", "murmur_prefill_attn",
     "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
     "murmur_last_cuda_error", "murmur_version",
 ]
@@ -99,6 +99,7 @@ def lib() -> C.CDLL:
     L.murmur_debug_attn_timeline.argtypes = [vp, vp, i32, vp, vp]
     L.murmur_debug_step_trace.argtypes = [vp, vp, vp]
     L.murmur_decode_attn_windowed.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, C.c_float, vp, vp]
+    L.murmur_prefill_attn.argtypes = [vp, i32, i32, i32, vp, vp, vp, i32, i32, C.c_float, vp]
     L.murmur_profile_scratch_bytes.argtypes = [vp, vp, i32, i32, i32]
     L.murmur_profile_scratch_bytes.restype = C.c_size_t
     L.murmur_attn_profile.argtypes = [vp, vp, i32, vp, vp, C.c_float, vp, vp, C.c_size_t, i32, i32, C.c_float, vp]
@@ -218,6 +219,24 @@ class MurmurCache:
         self._check(self.L.murmur_decode_attn(self.h, ids.ctypes.data, len(ids), q.data_ptr(), out.data_ptr(),
                                               lse.data_ptr() if lse is not None else None, layer_begin, layer_end,
                                               C.c_float(sm_scale), _stream()))
+        return out
+
+    def prefill_attn(self, seq: int, pos_begin: int, pos_end: int, q: torch.Tensor, out: Optional[torch.Tensor] = None,
+                     lse: Optional[torch.Tensor] = None, sm_scale: Optional[float] = None, layer_begin: int = 0,
+                     layer_end: Optional[int] = None) -> torch.Tensor:
+        """Causal attention of the prefill positions [pos_begin, pos_end): q, out [layers, n_tok, n_q, d] bf16."""
+        layer_end = self.n_layers if layer_end is None else layer_end
+        shape = (layer_end - layer_begin, pos_end - pos_begin, self.n_q, self.d)
+        assert q.dtype == torch.bfloat16 and q.is_cuda and q.is_contiguous() and tuple(q.shape) == shape
+        if out is None:
+            out = torch.empty(shape, dtype=torch.bfloat16, device=self.device)
+        assert out.dtype == torch.bfloat16 and out.is_contiguous() and tuple(out.shape) == shape
+        if lse is not None:
+            assert lse.dtype == torch.float32 and lse.is_contiguous() and tuple(lse.shape) == shape[:3]
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        self._check(self.L.murmur_prefill_attn(self.h, seq, pos_begin, pos_end, q.data_ptr(), out.data_ptr(),
+                                               lse.data_ptr() if lse is not None else None, layer_begin, layer_end,
+                                               C.c_float(sm_scale), _stream()))
         return out
 
     def attn_profile(self, seq_ids, q: torch.Tensor, candidate=None, mass_frac: float = 0.99,

@@ -133,6 +133,8 @@ murmur_status_t check_ids(murmur_cache* c, const int32_t* ids, int32_t n) {
 
 extern "C" {
 
+static murmur_status_t check_seq(murmur_cache_t* c, int32_t seq);
+
 size_t murmur_pool_bytes(const murmur_cache_desc_t* d) {
   if (!geometry_ok(d)) return 0;
   return (size_t)d->n_layers * (size_t)d->n_pages * d->n_kv_heads * d->page_size * kRowBytes;
@@ -506,6 +508,26 @@ murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_id
   st = murmur_decode_step(c, seq_ids, n_seqs, dk, dv, dq, dout, nullptr, sm_scale, stream);
   if (st != MURMUR_OK) return st;
   MM_CUDA(c, cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, s));
+  return MURMUR_OK;
+}
+
+// ---- prefill ------------------------------------------------------------------------------------
+murmur_status_t murmur_prefill_attn(murmur_cache_t* c, int32_t seq, int32_t pos_begin, int32_t pos_end, const void* q,
+                                    void* out, float* lse, int32_t layer_begin, int32_t layer_end, float sm_scale,
+                                    void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!q || !out) return MURMUR_ERR_INVALID_ARG;
+  if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
+  if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
+  if (c->desc.page_size < 16) return MURMUR_ERR_UNSUPPORTED;
+  const HostSeq& hs = c->seqs[seq];
+  if (pos_begin < 0 || pos_begin >= pos_end || pos_end > hs.sp.len) return MURMUR_ERR_INVALID_ARG;
+  if (hs.freed_blocks != 0) return MURMUR_ERR_STATE;  // something below pos_end may be gone
+  LaunchInfo li{};
+  MM_CUDA(c, launch_prefill_attn(c->view, seq, pos_begin, pos_end - pos_begin, q, out, lse, layer_begin, layer_end,
+                                 sm_scale, (cudaStream_t)stream, &li));
+  note(c, li);
   return MURMUR_OK;
 }
 

@@ -1,0 +1,120 @@
+"""Parity of murmur_prefill_attn (causal attention of the prefill tokens over the paged cache)
+against oracle/prefill.py on the same seeded inputs; tolerance as for decode (2e-2 / 2e-3)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import workloads
+from oracle import attention as o_attn
+from oracle import prefill as o_pre
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return "cuda:0"
+
+
+def _cache(dev, n_layers, n_tok, page, policy=None, P=8, M=0):
+    from paper_2606_01483_b200 import MURMUR_WINDOW_OFF, MurmurCache
+
+    nb = (n_tok + page - 1) // page + 2
+    c = MurmurCache(n_layers, 28, 4, 128, page, 1, nb, nb + 2, device=dev)
+    c.seq_begin(0, P, n_tok - P - M, M, policy or (MURMUR_WINDOW_OFF, 0, 0, MURMUR_WINDOW_OFF, 0))
+    return c
+
+
+def _rand(shape, seed, dev):
+    g = torch.Generator().manual_seed(seed)
+    return torch.randn(*shape, generator=g).to(torch.bfloat16).to(dev)
+
+
+def _check(out, lse, q, k, v, pos_begin, rows, scale):
+    got = out.float().cpu().numpy().astype(np.float64)
+    qb, kb, vb = workloads.to_bits(q), workloads.to_bits(k), workloads.to_bits(v)
+    errs = []
+    for layer in range(q.shape[0]):
+        if rows is None:
+            o_ref, lse_ref = o_pre.causal_attention(qb[layer], kb[layer], vb[layer], pos_begin, scale)
+            errs.append(np.abs(got[layer] - o_ref))
+            if lse is not None:
+                assert np.max(np.abs(lse[layer].cpu().numpy() - lse_ref)) < 2e-3
+        else:
+            for i in rows:
+                o_ref, lse_ref, _ = o_attn.attend_retained(qb[layer, i], kb[layer], vb[layer], range(pos_begin + i + 1), scale)
+                errs.append(np.abs(got[layer, i] - o_ref))
+                if lse is not None:
+                    assert np.max(np.abs(lse[layer, i].cpu().numpy() - lse_ref)) < 2e-3
+    e = np.concatenate([x.ravel() for x in errs])
+    assert np.isfinite(got).all()
+    assert e.max() <= 2e-2 and e.mean() <= 2e-3, (e.max(), e.mean())
+
+
+@pytest.mark.parametrize("page,n_tok", [(16, 200), (32, 130), (64, 257), (64, 64), (16, 1)])
+def test_prefill_every_row_small(dev, page, n_tok):
+    L = 2
+    c = _cache(dev, L, n_tok, page, P=min(8, n_tok))
+    k, v = _rand((L, n_tok, 4, 128), 1, dev), _rand((L, n_tok, 4, 128), 2, dev)
+    k[:, :4] *= 4  # sink keys
+    q = _rand((L, n_tok, 28, 128), 3, dev)
+    c.kv_append([0], [n_tok], k, v)
+    lse = torch.empty(L, n_tok, 28, dtype=torch.float32, device=dev)
+    out = c.prefill_attn(0, 0, n_tok, q, lse=lse)
+    _check(out, lse, q, k, v, 0, None, 1 / math.sqrt(128))
+    assert c.last_error() == 0
+    c.close()
+
+
+def test_prefill_chunked_unaligned_ranges_and_layer_range(dev):
+    # the chunk is prefilled in two pieces that do not start on a tile boundary; second layer only
+    L, n_tok = 3, 300
+    c = _cache(dev, L, n_tok, 16)
+    k, v = _rand((L, n_tok, 4, 128), 4, dev), _rand((L, n_tok, 4, 128), 5, dev)
+    q = _rand((L, n_tok, 28, 128), 6, dev)
+    c.kv_append([0], [n_tok], k, v)
+    scale = 1 / math.sqrt(128)
+    for a, b in ((0, 37), (37, 300), (101, 102)):
+        out = c.prefill_attn(0, a, b, q[1:2, a:b].contiguous(), layer_begin=1, layer_end=2)
+        _check(out, None, q[1:2, a:b], k[1:2], v[1:2], a, None, scale)
+    c.close()
+
+
+def test_prefill_config2_size_sampled_rows(dev):
+    # one 300 s chunk: 64 prefix + 2250 speech tokens, 2 layers; rows around tile / page boundaries and the end
+    cfg = workloads.config2().with_layers(2)
+    d = workloads.SeqData(cfg, 0, device=dev)
+    k, v = d.prefill_kv()
+    n_tok = k.shape[1]
+    c = _cache(dev, 2, n_tok, 64, P=64)
+    c.kv_append([0], [n_tok], k.contiguous(), v.contiguous())
+    q = _rand((2, n_tok, 28, 128), 7, dev)
+    lse = torch.empty(2, n_tok, 28, dtype=torch.float32, device=dev)
+    out = c.prefill_attn(0, 0, n_tok, q, lse=lse)
+    torch.cuda.synchronize()
+    _check(out, lse, q, k, v, 0, [0, 1, 15, 16, 63, 64, 65, 127, 128, 1000, 2047, 2048, n_tok - 2, n_tok - 1], 1 / math.sqrt(128))
+    c.close()
+
+
+def test_prefill_rejects_evicted_cache_and_bad_ranges(dev):
+    from paper_2606_01483_b200 import MurmurError
+
+    c = _cache(dev, 1, 200, 16, policy=(16, 0, 0, 16, 0), P=8)
+    k = _rand((1, 200, 4, 128), 8, dev)
+    c.kv_append([0], [200], k, k.clone())
+    q = _rand((1, 200, 28, 128), 9, dev)
+    c.prefill_attn(0, 0, 200, q)  # fine before any evict
+    with pytest.raises(MurmurError):
+        c.prefill_attn(0, 0, 201, _rand((1, 201, 28, 128), 9, dev))
+    with pytest.raises(MurmurError):
+        c.prefill_attn(0, 5, 5, q[:, :0].contiguous())
+    kk = _rand((1, 40, 4, 128), 10, dev)
+    c.kv_append([0], [40], kk, kk.clone())  # 40 output tokens: the speech window slides, blocks are freed
+    c.kv_evict([0])
+    with pytest.raises(MurmurError):
+        c.prefill_attn(0, 0, 200, q)
+    c.close()
