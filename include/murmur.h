@@ -205,6 +205,17 @@ MURMUR_API murmur_status_t murmur_decode_step_host(murmur_cache_t* cache, const 
                                                    const void* k_new_host, const void* v_new_host,
                                                    const void* q_host, void* out_host, float sm_scale, void* stream);
 
+/* ---- chunking (host only) ------------------------------------------------------------------ */
+/* Greedy merge of VAD speech segments into chunks of span <= max_len seconds (c = 300 s).
+ *   seg_start, seg_end : HOST float[n_segments], seconds, sorted and non-overlapping
+ *   chunk_first_seg    : HOST int32[cap] out: index of the first segment of each chunk (chunk j covers
+ *                        segments chunk_first_seg[j] .. chunk_first_seg[j+1]-1); may be NULL with cap 0
+ *   *n_chunks_out      : number of chunks (set even when cap is too small -> MURMUR_ERR_INVALID_ARG)
+ * A segment longer than max_len is a chunk by itself.  No GPU work, no handle. */
+MURMUR_API murmur_status_t murmur_chunk_plan(const float* seg_start, const float* seg_end, int32_t n_segments,
+                                             float max_len, int32_t* chunk_first_seg, int32_t cap,
+                                             int32_t* n_chunks_out);
+
 /* ---- prefill ------------------------------------------------------------------------------- */
 /* Causal self-attention of prefill tokens: for the positions x in
  * [pos_begin, pos_end) of `seq`, out[l][x - pos_begin][h] = Eq. 1 of query q_x over

@@ -33,7 +33,7 @@ EXPORTED_SYMBOLS = [
     "murmur_decode_step", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
     "murmur_debug_attn_timeline", "murmur_debug_step_trace", "murmur_profile_scratch_bytes", "murmur_attn_profile",
-    "murmur_decode_attn_windowed", "murmur_prefill_attn",
+    "murmur_decode_attn_windowed", "murmur_prefill_attn", "murmur_chunk_plan",
     "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
     "murmur_last_cuda_error", "murmur_version",
 ]
@@ -99,6 +99,7 @@ def lib() -> C.CDLL:
     L.murmur_debug_attn_timeline.argtypes = [vp, vp, i32, vp, vp]
     L.murmur_debug_step_trace.argtypes = [vp, vp, vp]
     L.murmur_decode_attn_windowed.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, C.c_float, vp, vp]
+    L.murmur_chunk_plan.argtypes = [vp, vp, i32, C.c_float, vp, i32, vp]
     L.murmur_prefill_attn.argtypes = [vp, i32, i32, i32, vp, vp, vp, i32, i32, C.c_float, vp]
     L.murmur_profile_scratch_bytes.argtypes = [vp, vp, i32, i32, i32]
     L.murmur_profile_scratch_bytes.restype = C.c_size_t
@@ -355,6 +356,20 @@ class MurmurCache:
 
     def reset_stats(self):
         self._check(self.L.murmur_reset_stats(self.h))
+
+
+def chunk_plan(segments, max_len: float = 300.0):
+    """Greedy VAD-segment merge (murmur_chunk_plan): list of (start, end) seconds -> list of lists of segment indices."""
+    seg = np.ascontiguousarray(np.asarray(segments, dtype=np.float32).reshape(-1, 2))
+    a, b = np.ascontiguousarray(seg[:, 0]), np.ascontiguousarray(seg[:, 1])
+    first = np.zeros(max(1, len(seg)), dtype=np.int32)
+    n = C.c_int32(0)
+    st = lib().murmur_chunk_plan(a.ctypes.data, b.ctypes.data, len(seg), C.c_float(max_len), first.ctypes.data, len(first),
+                                 C.byref(n))
+    if st != 0:
+        raise MurmurError(f"murmur_chunk_plan: {STATUS_NAMES.get(st, st)}")
+    cuts = list(first[: n.value]) + [len(seg)]
+    return [list(range(cuts[j], cuts[j + 1])) for j in range(n.value)]
 
 
 def version() -> str:

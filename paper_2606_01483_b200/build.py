@@ -17,7 +17,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libmurmur.so")
 
-SOURCES = ["murmur_api.cu", "kv_append.cu", "kv_evict.cu", "decode_attn_generic.cu", "decode_attn_mma.cu", "attn_profile.cu", "prefill_attn.cu"]
+SOURCES = ["murmur_api.cu", "kv_append.cu", "kv_evict.cu", "decode_attn_generic.cu", "decode_attn_mma.cu", "attn_profile.cu", "prefill_attn.cu", "chunk_plan.cu"]
 HEADERS = ["device_state.cuh", "policy_math.cuh", "evict_body.cuh", "ptx_utils.cuh"]
 
 NVCC_FLAGS = [
