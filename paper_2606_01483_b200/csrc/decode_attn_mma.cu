@@ -1,28 +1,35 @@
-// murmur_decode_attn, tensor-core split-K variant for sm_100a.
+// murmur_decode_attn and murmur_decode_step, tensor-core split-K kernel for sm_100a.
 //
 // Eq. 1 for one query token per sequence over the retained set, all layers in
 // ONE persistent launch (the path moves only ~20 MB per layer, so per-layer launches could never
-// reach the HBM roofline - DESIGN.md "Kernels").
+// reach the HBM roofline - DESIGN.md "Kernels").  kStep = true runs the whole decode step (append,
+// evict, attention) in that one launch.
 //
 // Work decomposition
 //   item  = (layer, sequence, KV head): G query heads (<= 8) share every K/V row.
-//   tile  = <= 64 consecutive retained rows of one run (64/p consecutive live pages), built by
-//           murmur_kv_evict; identical for all layers and heads of a sequence.
-//   The flattened tile list (layer, seq, head, tile) is cut into `grid` equal contiguous ranges,
-//   one per CTA (split-K across the retained length whenever a cut falls inside an item).
-// Per CTA: 1 producer warp + 6 consumer warps, a 6-stage ring of (K tile, V tile) buffers
-//   (tile n lives in stage n % 6 and is consumed by warp n % 6, so each stage has one owner).
-//   producer : one lane per tile issues 1-D bulk copies (cp.async.bulk, TMA engine) of each
-//              page's contiguous row range straight into the stage buffer; rows are stored
-//              pre-swizzled in HBM, so the copy needs no tensor map and ldmatrix is
-//              conflict-free.  Bytes copied = retained rows exactly.
-//   consumer : warp w takes every 6th tile.  S^T[64 tok x 8 heads] = K Q^T with mma.sync
-//              m16n8k16 bf16 (tokens are M, the padded head group is N: 7/8 useful), fp32
-//              online softmax in exp2 form, P^T moved to the B-operand layout with movmatrix,
-//              O^T[128 d x 8 heads] += V^T P^T with ldmatrix.trans.
-//   merge    : the six warps' (m, l, O) are merged through shared memory; an item that spans
-//              several CTAs is finished by the LAST contributor (arrival counter): partials go
-//              to a workspace slot, the last one merges them by the log-sum-exp rule.
+//   tile  = <= 64 consecutive retained rows of one run (64/p consecutive live pages), generated
+//           in the kernel from the sequence's tile table (closed form of the policy) plus one
+//           block-table load per page; identical for all layers and heads of a sequence.
+//   The flattened tile list (layer, seq, head, tile) is cut into 2 * grid equal contiguous ranges,
+//   two per CTA (split-K across the retained length whenever a cut falls inside an item).
+// Per CTA: 2 independent halves, each = 1 producer warp + 4 consumer warps + 3 stages of the ring
+//   of (K tile, V tile) buffers, working through its own range - so that one half's end-of-item
+//   merge overlaps the other half's streaming - plus, in step mode, one keeper warp.
+//   producer : lane j prepares tile j of a batch (pool offsets, sizes), one lane at a time issues
+//              1-D bulk copies (cp.async.bulk, TMA engine, L2::evict_first) of each page's
+//              contiguous row range straight into the stage buffer; rows are stored pre-swizzled
+//              in HBM, so the copy needs no tensor map and ldmatrix is conflict-free.  Bytes
+//              copied = retained rows exactly.
+//   consumer : the 4 warps of a half take the 4 16-row slices of each tile.  S^T[16 tok x 8 heads]
+//              = K Q^T with mma.sync m16n8k16 bf16 (tokens are M, the padded head group is N: 7/8
+//              useful), fp32 online softmax in exp2 form, P^T moved to the B-operand layout with
+//              movmatrix, O^T[128 d x 8 heads] += V^T P^T with ldmatrix.trans.
+//   merge    : at the end of an item the 4 warps' (m, l, O^T) are tree-merged in the MMA fragment
+//              layout through shared memory (only the receiving warp waits); the half's first warp
+//              writes the output, or - for an item that spans several ranges - publishes a partial
+//              and, if it is the LAST contributor (arrival counter), merges all of them.
+//   keeper   : step mode only - row scatter k_new/v_new -> pools, the eviction's table products,
+//              and (last CTA through a ticket) the integer commit + freeing of dead pages.
 #include <cuda_bf16.h>
 
 #include "evict_body.cuh"
@@ -33,33 +40,30 @@ namespace {
 
 constexpr int kStages = 6;
 constexpr int kSliceWarps = 4;   // the four 16-row slices of a 64-row tile, one warp each
-constexpr int kGroups = 2;       // warp groups; group g consumes tiles n with n % kGroups == g
+constexpr int kGroups = 2;       // warp groups; each works through its OWN tile range, fed through its own half of the ring
 constexpr int kConsumerWarps = kSliceWarps * kGroups;
-// A stage must always be consumed by the same warps: a warp that waited on a stage it had not seen
-// the previous phase of could pass try_wait.parity one phase early (parity aliasing).
-static_assert(kStages % kGroups == 0, "a stage must belong to exactly one consumer group");
+static_assert(kStages % kGroups == 0, "each group owns kStages / kGroups stages of the ring");
+constexpr int kSub = kStages / kGroups;  // stages per group: group g owns stages g, g + kGroups, ...
 static_assert(kTileRows == kSliceWarps * 16, "one m16 slice per warp");
 constexpr int kConsumerThreads = kConsumerWarps * 32;
-constexpr int kMmaThreads = kConsumerThreads + 32;
+constexpr int kMmaThreads = kConsumerThreads + kGroups * 32;  // + one producer warp per group
 constexpr int kTileBytes = kTileRows * kRowBytes;            // 16 KB per K or V tile
 constexpr int kQBytes = kMaxGroup * kRowBytes;               // 2 KB
-constexpr int kScratchFloats = kMaxGroup * kOStride + 2 * kMaxGroup;  // o[8][132], m[8], l[8]
 constexpr int kFragFloats = 36 * 32;                         // o[32] + m[2] + l[2] per lane, [reg][lane]
-static_assert(kFragFloats >= kScratchFloats, "the two merge layouts share one buffer");
+static_assert(kFragFloats == kPartialFloats, "split-K partials are stored in the fragment layout");
 
 struct __align__(128) SmemLayout {
   uint8_t kv[kStages][2][kTileBytes];
-  uint8_t q[2][kQBytes];
+  uint8_t q[kGroups][2][kQBytes];
   // step mode: this step's K row and V row of the current item (natural layout).  Processed as a
   // 16-row tile of which only row 0 is valid; the rows "behind" it are whatever follows in shared
   // memory (masked), so this must stay in front of a >= 4 KB member.
-  uint8_t newrow[2][2][kRowBytes];
-  float scratch[kSliceWarps][kFragFloats];  // group merge (fragment layout), then slice merge (o[8][132], m, l)
-  unsigned long long full_k[kStages], full_v[kStages], empty[kStages], q_full[2], q_empty[2];
+  uint8_t newrow[kGroups][2][2][kRowBytes];
+  float scratch[kGroups][2][kFragFloats];  // per group: two hand-over buffers of the end-of-item tree merge
+  unsigned long long full_k[kStages], full_v[kStages], empty[kStages], q_full[kGroups][2], q_empty[kGroups][2];
   int meta[kStages][2];  // row_begin, row_end of the tile in each stage
   int nt[kMaxSeqsAttn];
   int pre[kMaxSeqsAttn + 1];
-  int flag;
   // per-sequence state the tiles are generated from (the kernel does not read the evict's tile list)
   SeqParams sp[kMaxSeqsAttn];    // lengths as attended; step mode: AFTER this step's append
   TileGen tg[kMaxSeqsAttn];      // runs + tile offsets of each sequence (closed form of sp)
@@ -73,7 +77,10 @@ struct __align__(128) SmemLayout {
 };
 static_assert(sizeof(SmemLayout) <= 227 * 1024, "shared memory budget");
 
-__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory"); }
+// Named barriers of one consumer group (4 warps): ids 2 + 4 g + k.  sync = wait for `count` threads,
+// arrive = count towards it without waiting.
+__device__ __forceinline__ void group_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void group_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
 // ---- walking the flattened (layer, seq, head, tile) list ---------------------------------------------
 struct Cursor {
@@ -171,15 +178,15 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       mbar_init(&s.full_v[i], 1);
       mbar_init(&s.empty[i], kSliceWarps);
     }
-    for (int i = 0; i < 2; ++i) {
-      mbar_init(&s.q_full[i], 1);
-      mbar_init(&s.q_empty[i], kConsumerWarps);
+    for (int i = 0; i < 2 * kGroups; ++i) {
+      mbar_init(&s.q_full[0][0] + i, 1);
+      mbar_init(&s.q_empty[0][0] + i, kSliceWarps);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     s.abort = 0;
     s.blk_total = 0;
   }
-  for (int i = tid; i < 2 * kQBytes / 4; i += n_threads) reinterpret_cast<uint32_t*>(&s.q[0][0])[i] = 0u;
+  for (int i = tid; i < kGroups * 2 * kQBytes / 4; i += n_threads) reinterpret_cast<uint32_t*>(&s.q[0][0][0])[i] = 0u;
   __syncthreads();
   // Everything above touches only this CTA's shared memory; from here on the kernel reads what
   // earlier kernels of the stream wrote and writes buffers the previous launch may still use.
@@ -267,7 +274,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   const uint8_t* kpool = reinterpret_cast<const uint8_t*>(c.k_pool);
   const uint8_t* vpool = reinterpret_cast<const uint8_t*>(c.v_pool);
 
-  if (kStep && warp == kConsumerWarps + 1) {
+  if (kStep && warp == kConsumerWarps + kGroups) {
     // ===================================== keeper warp =====================================
     // All the old state this CTA needs is in shared memory now: take the ticket first.
     int last = 0;
@@ -311,14 +318,18 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     return;
   }
 
+  // Work split: the flattened (layer, seq, head, tile) list is cut into V equal contiguous ranges,
+  // two per CTA - one per consumer group (split-K wherever a cut falls inside an item).  The two
+  // groups of a CTA work through their ranges independently, each fed through its own half of the
+  // ring: while one group is in its end-of-item merge (~2 us, no tiles consumed) the other keeps
+  // streaming, so the merges no longer stall the CTA's share of HBM.
   const long long total = (long long)prm.n_layers_call * n_kv * s.pre[n_seqs];
-  const long long geff = total < (long long)gridDim.x ? total : (long long)gridDim.x;
-  const long long cta = blockIdx.x;
-  if (cta >= geff) return;
-  const long long lo = cta * total / geff, hi = (cta + 1) * total / geff;
-
-  if (warp == kConsumerWarps) {
-    // =================================== producer warp ===================================
+  const long long V = min(total, (long long)kGroups * gridDim.x);
+  if ((long long)kGroups * blockIdx.x >= V) return;
+  auto range_lo = [&](long long v) { return v * total / V; };
+  if (warp >= kConsumerWarps) {
+    // ================================ producer warps (one per group) ================================
+    const int gg = warp - kConsumerWarps;
     // Walks its tile range in batches of <= 32 tiles of one item; lane j owns tile j of the batch.
     // Everything a tile's copies need (pool offsets, sizes, destination rows) is computed by all
     // lanes in parallel, right after the previous batch has been issued (the ring is full then, so
@@ -356,34 +367,40 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       }
       return ti;
     };
+    // This producer warp feeds consumer group gg: it walks the group's range in batches of <= 32
+    // tiles of one item; lane j of the warp holds the prepared copies of tile j of the batch.
+    const long long v = (long long)kGroups * blockIdx.x + gg;
+    if (v >= V) return;
+    const long long lo = range_lo(v), hi = range_lo(v + 1);
     Cursor cur = locate(s, n_seqs, n_kv, lo);
     long long remaining = hi - lo;  // tiles left, counted from the start of the current item's segment
     int seg = (int)min((long long)(s.nt[cur.i] - cur.k), remaining);
     int base = 0, cnt = min(32, seg);
-    int st = 0;          // ring stage of the next tile
+    int sub = 0;         // position of the next tile in the group's kSub stages
     uint32_t ph = 0;     // its phase parity
     int item_no = 0;
     TileIssue ti;
     if (lane < cnt) ti = prep(cur, cur.k + lane);
     while (remaining > 0) {
       // ---- issue the current batch ----
-      if (base == 0 && lane == 0) {  // first batch of an item (or of this CTA's segment of it)
+      if (base == 0 && lane == 0) {  // first batch of an item (or of this range's segment of it)
         // stage its G query rows and, in step mode, this step's K / V rows of the item when this
-        // CTA's segment ends with the item's last tile (natural layout, straight from k_new / v_new)
+        // segment ends with the item's last tile (natural layout, straight from k_new / v_new)
         const int qb = item_no & 1;
-        mbar_wait(&s.q_empty[qb], ((item_no >> 1) & 1) ^ 1);
+        mbar_wait(&s.q_empty[gg][qb], ((item_no >> 1) & 1) ^ 1);
         const bool mini = kStep && s.newatt[cur.i] && (cur.k + seg == s.nt[cur.i]);
         const size_t seq_row = (size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i;
-        mbar_expect_tx(&s.q_full[qb], (uint32_t)((G + (mini ? 2 : 0)) * kRowBytes));
-        bulk_g2s(&s.q[qb][0], prm.q + (seq_row * c.n_q + (size_t)cur.h * G) * kHeadDim, (uint32_t)(G * kRowBytes),
-                 &s.q_full[qb]);
+        mbar_expect_tx(&s.q_full[gg][qb], (uint32_t)((G + (mini ? 2 : 0)) * kRowBytes));
+        bulk_g2s(&s.q[gg][qb][0], prm.q + (seq_row * c.n_q + (size_t)cur.h * G) * kHeadDim, (uint32_t)(G * kRowBytes),
+                 &s.q_full[gg][qb]);
         if (mini) {
           const size_t off = (seq_row * n_kv + cur.h) * kHeadDim;
-          bulk_g2s(&s.newrow[qb][0][0], prm.k_new + off, (uint32_t)kRowBytes, &s.q_full[qb]);
-          bulk_g2s(&s.newrow[qb][1][0], prm.v_new + off, (uint32_t)kRowBytes, &s.q_full[qb]);
+          bulk_g2s(&s.newrow[gg][qb][0][0], prm.k_new + off, (uint32_t)kRowBytes, &s.q_full[gg][qb]);
+          bulk_g2s(&s.newrow[gg][qb][1][0], prm.v_new + off, (uint32_t)kRowBytes, &s.q_full[gg][qb]);
         }
       }
       for (int j = 0; j < cnt; ++j) {
+        const int st = kGroups * sub + gg;
         if (lane == j) {
           mbar_wait(&s.empty[st], ph ^ 1u);
           s.meta[st][0] = ti.row_begin;
@@ -399,14 +416,14 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
           }
         }
         __syncwarp();
-        if (++st == kStages) {
-          st = 0;
+        if (++sub == kSub) {
+          sub = 0;
           ph ^= 1u;
         }
       }
       // ---- advance, and prepare the next batch while the ring (just filled) drains ----
       base += cnt;
-      if (base >= seg) {  // item (or this CTA's segment of it) done
+      if (base >= seg) {  // item (or this range's segment of it) done
         remaining -= seg;
         base = 0;
         ++item_no;
@@ -441,10 +458,15 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   const uint32_t k_off = (uint32_t)(slice0 + lm_row) * kRowBytes;
   const uint32_t v_off = (uint32_t)(slice0 + lv_row) * kRowBytes;
 
+  // this group's tile range
+  const long long vrange = (long long)kGroups * blockIdx.x + grp;
+  if (vrange >= V) return;
+  const long long lo = range_lo(vrange), hi = range_lo(vrange + 1);
+  const int bar0 = 2 + 4 * grp;  // this group's named barriers
   Cursor cur = locate(s, n_seqs, n_kv, lo);
   long long remaining = hi - lo;
   long long pos = lo;
-  uint32_t n = 0;
+  uint32_t n = 0;  // tiles of this group's stream consumed so far
   int item_no = 0;
   bool first_segment = true;
 
@@ -455,10 +477,10 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 
     // ---- this item's query fragments (B operand of S^T = K Q^T) ----
     const int qb = item_no & 1;
-    mbar_wait(&s.q_full[qb], (item_no >> 1) & 1);
+    mbar_wait(&s.q_full[grp][qb], (item_no >> 1) & 1);
     uint32_t qf[8][2];
     {
-      const uint8_t* qs = &s.q[qb][0] + lrow * kRowBytes + lcol * 2;
+      const uint8_t* qs = &s.q[grp][qb][0] + lrow * kRowBytes + lcol * 2;
 #pragma unroll
       for (int ks = 0; ks < 8; ++ks) {
         qf[ks][0] = *reinterpret_cast<const uint32_t*>(qs + ks * 32);
@@ -466,10 +488,10 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       }
     }
     __syncwarp();
-    // step mode: warp 0 also processes this step's token at the end of the item, from the same
-    // double buffer as the queries - it hands the buffer back only then
-    const bool mini = kStep && warp == 0 && s.newatt[cur.i] && (cur.k + seg == nt_i);
-    if (lane == 0 && !mini) mbar_arrive(&s.q_empty[qb]);
+    // step mode: the group's first warp also processes this step's token at the end of the item, from
+    // the same double buffer as the queries - it hands the buffer back only then
+    const bool mini = kStep && w4 == 0 && s.newatt[cur.i] && (cur.k + seg == nt_i);
+    if (lane == 0 && !mini) mbar_arrive(&s.q_empty[grp][qb]);
 
     float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
     float o[8][4];
@@ -545,177 +567,139 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       }
     };
 
-    for (int tt = (grp + kGroups - (int)(n % kGroups)) % kGroups; tt < seg; tt += kGroups) {
+    for (int tt = 0; tt < seg; ++tt) {
       const uint32_t nn = n + (uint32_t)tt;
-      const int st = (int)(nn % kStages);
-      const uint32_t ph = (nn / kStages) & 1u;
+      const int st = kGroups * (int)(nn % kSub) + grp;
+      const uint32_t ph = (nn / kSub) & 1u;
       mbar_wait(&s.full_k[st], ph);
       slice(smem_u32(&s.kv[st][0][0]), smem_u32(&s.kv[st][1][0]), s.meta[st][0], s.meta[st][1], &s.full_v[st], ph);
       __syncwarp();
       if (lane == 0) mbar_arrive(&s.empty[st]);
     }
-    if (mini) {  // warp 0 (slice0 == 0): a tile whose only valid row, row 0, is this step's token
-      slice(smem_u32(&s.newrow[qb][0][0]), smem_u32(&s.newrow[qb][1][0]), 0, 1, nullptr, 0u);
+    if (mini) {  // first warp of the group (slice0 == 0): a tile whose only valid row, row 0, is this step's token
+      slice(smem_u32(&s.newrow[grp][qb][0][0]), smem_u32(&s.newrow[grp][qb][1][0]), 0, 1, nullptr, 0u);
       __syncwarp();
-      if (lane == 0) mbar_arrive(&s.q_empty[qb]);
+      if (lane == 0) mbar_arrive(&s.q_empty[grp][qb]);
     }
     n += (uint32_t)seg;
 
-    // ---- merge 1: groups 1.. hand their state to group 0 (same fragment layout, lane for lane) ----
-#pragma unroll
-    for (int r = 1; r < kGroups; ++r) {
-      float* fs = s.scratch[w4];
-      if (grp == r) {
-#pragma unroll
-        for (int dt = 0; dt < 8; ++dt) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) fs[(dt * 4 + e) * 32 + lane] = o[dt][e];
-        }
-        fs[32 * 32 + lane] = m0;
-        fs[33 * 32 + lane] = m1;
-        fs[34 * 32 + lane] = l0;
-        fs[35 * 32 + lane] = l1;
-      }
-      consumer_bar();
-      if (grp == 0) {
-        const float mo0 = fs[32 * 32 + lane], mo1 = fs[33 * 32 + lane];
-        const float mn0 = fmaxf(m0, mo0), mn1 = fmaxf(m1, mo1);
-        const float fa0 = (m0 == -INFINITY) ? 0.f : ex2((m0 - mn0) * c2);
-        const float fa1 = (m1 == -INFINITY) ? 0.f : ex2((m1 - mn1) * c2);
-        const float fb0 = (mo0 == -INFINITY) ? 0.f : ex2((mo0 - mn0) * c2);
-        const float fb1 = (mo1 == -INFINITY) ? 0.f : ex2((mo1 - mn1) * c2);
-        l0 = l0 * fa0 + fs[34 * 32 + lane] * fb0;
-        l1 = l1 * fa1 + fs[35 * 32 + lane] * fb1;
-#pragma unroll
-        for (int dt = 0; dt < 8; ++dt) {
-          o[dt][0] = o[dt][0] * fa0 + fs[(dt * 4 + 0) * 32 + lane] * fb0;
-          o[dt][1] = o[dt][1] * fa1 + fs[(dt * 4 + 1) * 32 + lane] * fb1;
-          o[dt][2] = o[dt][2] * fa0 + fs[(dt * 4 + 2) * 32 + lane] * fb0;
-          o[dt][3] = o[dt][3] * fa1 + fs[(dt * 4 + 3) * 32 + lane] * fb1;
-        }
-        m0 = mn0;
-        m1 = mn1;
-      }
-      consumer_bar();
-    }
-
-    // ---- merge 2: the four row slices of group 0, through shared memory in [head][d] layout ----
-    if (grp == 0) {
-#pragma unroll
-      for (int sh = 4; sh <= 16; sh <<= 1) {
-        l0 += __shfl_xor_sync(0xffffffffu, l0, sh);
-        l1 += __shfl_xor_sync(0xffffffffu, l1, sh);
-      }
-      float* my_scratch = s.scratch[w4];
+    // ---- end of the item (or of this range's segment of it): tree merge of the group's four row
+    // slices in the MMA fragment layout (lane for lane, no transposition): warps 2, 3 hand their
+    // (m, l, O^T) to warps 0, 1, then warp 1 to warp 0.  Only the receiving side waits; a warp that
+    // has handed over goes straight on to the next item.
+    auto put = [&](float* fs) {
 #pragma unroll
       for (int dt = 0; dt < 8; ++dt) {
-        const int d = dt * 16 + lrow;
-        my_scratch[lcol * kOStride + d] = o[dt][0];
-        my_scratch[(lcol + 1) * kOStride + d] = o[dt][1];
-        my_scratch[lcol * kOStride + d + 8] = o[dt][2];
-        my_scratch[(lcol + 1) * kOStride + d + 8] = o[dt][3];
-      }
-      if (lrow == 0) {
-        my_scratch[kMaxGroup * kOStride + lcol] = m0;
-        my_scratch[kMaxGroup * kOStride + lcol + 1] = m1;
-        my_scratch[kMaxGroup * kOStride + kMaxGroup + lcol] = l0;
-        my_scratch[kMaxGroup * kOStride + kMaxGroup + lcol + 1] = l1;
-      }
-    }
-    consumer_bar();
-
-    const int layer_c = cur.layer;
-    const size_t out_row0 = ((size_t)layer_c * prm.n_seqs_total + prm.seq_base + cur.i) * c.n_q + (size_t)cur.h * G;
-    // thread `tid` < 128 owns column d = tid of every head; the other consumer threads only sync
-    const bool owner = tid < kHeadDim;
-    const int col = owner ? tid : 0;
-    float accv[kMaxGroup], Mh[kMaxGroup], Lh[kMaxGroup];
-    if (owner) {
 #pragma unroll
-      for (int h = 0; h < kMaxGroup; ++h) {
-        float M = -INFINITY;
-#pragma unroll
-        for (int w = 0; w < kSliceWarps; ++w) M = fmaxf(M, s.scratch[w][kMaxGroup * kOStride + h]);
-        float L = 0.f, acc = 0.f;
-#pragma unroll
-        for (int w = 0; w < kSliceWarps; ++w) {
-          const float mw = s.scratch[w][kMaxGroup * kOStride + h];
-          const float f = (mw == -INFINITY) ? 0.f : ex2((mw - M) * c2);
-          L += s.scratch[w][kMaxGroup * kOStride + kMaxGroup + h] * f;
-          acc += s.scratch[w][h * kOStride + col] * f;
-        }
-        accv[h] = acc; Mh[h] = M; Lh[h] = L;
+        for (int e = 0; e < 4; ++e) fs[(dt * 4 + e) * 32 + lane] = o[dt][e];
       }
-    }
-
-    if (complete) {
+      fs[32 * 32 + lane] = m0;
+      fs[33 * 32 + lane] = m1;
+      fs[34 * 32 + lane] = l0;
+      fs[35 * 32 + lane] = l1;
+    };
+    // (m, l, O) <- LSE-merge of itself and the fragment at fs (shared or global memory)
+    auto take = [&](const float* fs, bool global) {
+      auto ld = [&](int r) { return global ? __ldcg(fs + r * 32 + lane) : fs[r * 32 + lane]; };
+      const float mo0 = ld(32), mo1 = ld(33);
+      const float mn0 = fmaxf(m0, mo0), mn1 = fmaxf(m1, mo1);
+      const float fa0 = (m0 == -INFINITY) ? 0.f : ex2((m0 - mn0) * c2);
+      const float fa1 = (m1 == -INFINITY) ? 0.f : ex2((m1 - mn1) * c2);
+      const float fb0 = (mo0 == -INFINITY) ? 0.f : ex2((mo0 - mn0) * c2);
+      const float fb1 = (mo1 == -INFINITY) ? 0.f : ex2((mo1 - mn1) * c2);
+      l0 = l0 * fa0 + ld(34) * fb0;
+      l1 = l1 * fa1 + ld(35) * fb1;
 #pragma unroll
-      for (int h = 0; h < kMaxGroup; ++h) {
-        if (h < G && owner) {
-          prm.out[(out_row0 + h) * kHeadDim + tid] = __bfloat16_as_ushort(__float2bfloat16_rn(accv[h] / Lh[h]));
-          if (prm.lse != nullptr && tid == 0) prm.lse[out_row0 + h] = Mh[h] * prm.sm_scale + __logf(Lh[h]);
-        }
+      for (int dt = 0; dt < 8; ++dt) {
+        o[dt][0] = o[dt][0] * fa0 + ld(dt * 4 + 0) * fb0;
+        o[dt][1] = o[dt][1] * fa1 + ld(dt * 4 + 1) * fb1;
+        o[dt][2] = o[dt][2] * fa0 + ld(dt * 4 + 2) * fb0;
+        o[dt][3] = o[dt][3] * fa1 + ld(dt * 4 + 3) * fb1;
       }
+      m0 = mn0;
+      m1 = mn1;
+    };
+    // all four warps have finished the item's tiles; the hand-over buffers of the previous item are free
+    group_sync(bar0 + 0, kSliceWarps * 32);
+    if (w4 >= 2) {
+      put(s.scratch[grp][w4 - 2]);
+      group_arrive(bar0 + 1, kSliceWarps * 32);
     } else {
-      // split item: publish this CTA's partial; the last contributor merges all of them.
-      const long long item_lo = pos - cur.k;
-      const long long c_first = ((item_lo + 1) * geff - 1) / total;
-      const long long c_last = ((item_lo + nt_i) * geff - 1) / total;
-      const int slot = 2 * (int)cta + (first_segment ? 0 : 1);
-      float* part = c.partials + (size_t)slot * kPartialFloats;
-      if (owner) {
-#pragma unroll
-        for (int h = 0; h < kMaxGroup; ++h) part[h * kOStride + tid] = accv[h];
-      }
-      if (tid == 0) {
-#pragma unroll
-        for (int h = 0; h < kMaxGroup; ++h) {
-          part[kMaxGroup * kOStride + h] = Mh[h];
-          part[kMaxGroup * kOStride + kMaxGroup + h] = Lh[h];
-        }
-      }
-      __threadfence();
-      consumer_bar();
-      int* counter = c.item_counters + ((size_t)layer_c * n_seqs + cur.i) * n_kv + cur.h;
-      if (tid == 0) {
-        __threadfence();  // release: every thread's partial (ordered by the barrier) before the ticket
-        const int old = atomicAdd(counter, 1);
-        s.flag = (old == (int)(c_last - c_first));
-      }
-      consumer_bar();
-      if (s.flag && owner) {
-        __threadfence();
-        float M[kMaxGroup], L[kMaxGroup], acc[kMaxGroup];
-#pragma unroll
-        for (int h = 0; h < kMaxGroup; ++h) { M[h] = -INFINITY; L[h] = 0.f; acc[h] = 0.f; }
-        for (long long cc = c_first; cc <= c_last; ++cc) {
-          const long long lo_cc = cc * total / geff;
-          const int sl = 2 * (int)cc + ((cc == c_first && lo_cc < item_lo) ? 1 : 0);
-          const float* pp = c.partials + (size_t)sl * kPartialFloats;
-#pragma unroll
-          for (int h = 0; h < kMaxGroup; ++h) {
-            const float mw = __ldcg(pp + kMaxGroup * kOStride + h);
-            const float lw = __ldcg(pp + kMaxGroup * kOStride + kMaxGroup + h);
-            const float ow = __ldcg(pp + h * kOStride + tid);
-            const float Mn = fmaxf(M[h], mw);
-            const float fa = (M[h] == -INFINITY) ? 0.f : ex2((M[h] - Mn) * c2);
-            const float fb = (mw == -INFINITY) ? 0.f : ex2((mw - Mn) * c2);
-            L[h] = L[h] * fa + lw * fb;
-            acc[h] = acc[h] * fa + ow * fb;
-            M[h] = Mn;
-          }
-        }
-#pragma unroll
-        for (int h = 0; h < kMaxGroup; ++h) {
-          if (h < G) {
-            prm.out[(out_row0 + h) * kHeadDim + tid] = __bfloat16_as_ushort(__float2bfloat16_rn(acc[h] / L[h]));
-            if (prm.lse != nullptr && tid == 0) prm.lse[out_row0 + h] = M[h] * prm.sm_scale + __logf(L[h]);
-          }
-        }
-        if (tid == 0) *counter = 0;  // self-resetting for the next launch
+      group_sync(bar0 + 1, kSliceWarps * 32);
+      take(s.scratch[grp][w4], false);
+      if (w4 == 1) {
+        put(s.scratch[grp][1]);  // warp 1 has just read this buffer itself
+        group_arrive(bar0 + 2, 2 * 32);
+      } else {
+        group_sync(bar0 + 2, 2 * 32);
+        take(s.scratch[grp][1], false);
       }
     }
-    consumer_bar();  // scratch and flag are reused by the next segment
+
+    if (w4 == 0) {
+      // ---- the group's first warp finishes the item: output, or split-K partial ----
+      const int layer_c = cur.layer;
+      const size_t out_row0 = ((size_t)layer_c * prm.n_seqs_total + prm.seq_base + cur.i) * c.n_q + (size_t)cur.h * G;
+      // lane (lrow, lcol) holds O^T[d][head] for d = 16 dt + lrow (+ 8), head = lcol (+ 1)
+      auto write_out = [&]() {
+        float t0 = l0, t1 = l1;  // l is still split over the 8 row groups (lrow) of the fragment
+#pragma unroll
+        for (int sh = 4; sh <= 16; sh <<= 1) {
+          t0 += __shfl_xor_sync(0xffffffffu, t0, sh);
+          t1 += __shfl_xor_sync(0xffffffffu, t1, sh);
+        }
+        const float i0 = 1.f / t0, i1 = 1.f / t1;
+        uint16_t* o0 = prm.out + (out_row0 + lcol) * kHeadDim;
+        uint16_t* o1 = o0 + kHeadDim;
+#pragma unroll
+        for (int dt = 0; dt < 8; ++dt) {
+          const int d = dt * 16 + lrow;
+          if (lcol < G) {
+            o0[d] = __bfloat16_as_ushort(__float2bfloat16_rn(o[dt][0] * i0));
+            o0[d + 8] = __bfloat16_as_ushort(__float2bfloat16_rn(o[dt][2] * i0));
+          }
+          if (lcol + 1 < G) {
+            o1[d] = __bfloat16_as_ushort(__float2bfloat16_rn(o[dt][1] * i1));
+            o1[d + 8] = __bfloat16_as_ushort(__float2bfloat16_rn(o[dt][3] * i1));
+          }
+        }
+        if (prm.lse != nullptr && lrow == 0) {
+          if (lcol < G) prm.lse[out_row0 + lcol] = m0 * prm.sm_scale + __logf(t0);
+          if (lcol + 1 < G) prm.lse[out_row0 + lcol + 1] = m1 * prm.sm_scale + __logf(t1);
+        }
+      };
+      if (complete) {
+        write_out();
+      } else {
+        // split item: publish this range's partial (fragment layout); the last contributor merges all.
+        // Contributors = the ranges v_first..v_last that intersect the item.
+        const long long item_lo = pos - cur.k;
+        const long long v_first = ((item_lo + 1) * V - 1) / total;
+        const long long v_last = ((item_lo + nt_i) * V - 1) / total;
+        float* part = c.partials + (size_t)(2 * vrange + (first_segment ? 0 : 1)) * kPartialFloats;
+        put(part);
+        __threadfence();  // release: the partial before the ticket
+        __syncwarp();
+        int* counter = c.item_counters + ((size_t)layer_c * n_seqs + cur.i) * n_kv + cur.h;
+        int last = 0;
+        if (lane == 0) last = (atomicAdd(counter, 1) == (int)(v_last - v_first));
+        last = __shfl_sync(0xffffffffu, last, 0);
+        if (last) {
+          __threadfence();
+          m0 = m1 = -INFINITY;
+          l0 = l1 = 0.f;
+#pragma unroll
+          for (int dt = 0; dt < 8; ++dt) o[dt][0] = o[dt][1] = o[dt][2] = o[dt][3] = 0.f;
+          for (long long vv = v_first; vv <= v_last; ++vv) {
+            // a contributor used its second slot for this item iff its range starts before the item
+            const int sl = 2 * (int)vv + ((range_lo(vv) < item_lo) ? 1 : 0);
+            take(c.partials + (size_t)sl * kPartialFloats, true);
+          }
+          write_out();
+          if (lane == 0) *counter = 0;  // self-resetting for the next launch
+        }
+      }
+    }
 
     remaining -= seg;
     pos += seg;
@@ -723,9 +707,9 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     ++item_no;
     next_item(s, n_seqs, n_kv, cur);
   }
-  if (tid == 0) {
-    trace[1] = globaltimer_ns();
-    trace[3] = (unsigned long long)(hi - lo);
+  if (w4 == 0 && lane == 0) {
+    atomicMax(&trace[1], globaltimer_ns());
+    atomicAdd(&trace[3], (unsigned long long)(hi - lo));
   }
 }
 

@@ -22,9 +22,9 @@ constexpr int kTileRows = 64;            // rows of one attention tile (tokens)
 constexpr int kMaxGroup = 8;             // query heads per KV head, padded to the MMA N = 8
 constexpr int kMaxRuns = 6;
 constexpr int kMaxSeqsPerLaunch = 128;
-constexpr int kMaxSeqsAttn = 64;         // sequences per launch of the tensor-core attention kernel (smem tables)
+constexpr int kMaxSeqsAttn = 32;         // sequences per launch of the tensor-core attention kernel (smem tables)
 constexpr int kOStride = 132;            // floats per head row in split-K partials / merge scratch
-constexpr int kPartialFloats = kMaxGroup * kOStride + 2 * kMaxGroup;  // o[8][132] + m[8] + l[8]
+constexpr int kPartialFloats = 36 * 32;   // split-K partial in MMA fragment layout: o[32] + m[2] + l[2] per lane, [reg][lane]
 constexpr int kMaxAttnGrid = 1024;       // upper bound on CTAs of the persistent attention kernel
 constexpr int kStepTraceWords = 16;      // globaltimer stamps of the step prologue (after the per-CTA entries)
 constexpr int kTimelineWords = 4;        // globaltimer at CTA start, at CTA end, SM id, tiles processed
@@ -88,7 +88,7 @@ struct CacheView {
   int32_t* free_stack;   // [n_pages]
   int32_t* ctrl;         // [kCtrlWords]
   int32_t* item_counters;  // [n_layers][max_seqs][n_kv] split-K arrival counters (self-resetting)
-  float* partials;       // [2 * kMaxAttnGrid][kPartialFloats]
+  float* partials;       // [4 * kMaxAttnGrid][kPartialFloats]: two slots per tile range, two ranges per CTA
   unsigned long long* timeline;  // [kMaxAttnGrid][kTimelineWords] per-CTA trace of the last attention launch
 };
 

@@ -66,7 +66,7 @@ Carve carve(const murmur_cache_desc_t* d) {
   c.free_stack = take((size_t)d->n_pages * 4);
   c.ctrl = take(kCtrlWords * 4);
   c.counters = take((size_t)d->n_layers * kMaxSeqsPerLaunch * d->n_kv_heads * 4);
-  c.partials = take((size_t)2 * kMaxAttnGrid * kPartialFloats * 4);
+  c.partials = take((size_t)4 * kMaxAttnGrid * kPartialFloats * 4);
   c.timeline = take(((size_t)kMaxAttnGrid * kTimelineWords + kStepTraceWords) * 8);
   c.stage_seqs = d->max_seqs < kMaxSeqsPerLaunch ? d->max_seqs : kMaxSeqsPerLaunch;
   const size_t kv_b = (size_t)d->n_layers * c.stage_seqs * d->n_kv_heads * kRowBytes;
