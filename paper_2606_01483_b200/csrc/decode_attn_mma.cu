@@ -87,17 +87,22 @@ struct Cursor {
   int layer, i, h, k;  // layer index inside the call, index into the sequence list, KV head, tile
 };
 
-__device__ __forceinline__ Cursor locate(const SmemLayout& s, int n_seqs, int n_kv, long long x) {
-  const long long per_layer = (long long)n_kv * s.pre[n_seqs];
+// 32-bit arithmetic throughout: this runs once per range on the kernel's start-up path, where a
+// 64-bit division costs ~0.2 us (the launcher rejects problems with >= 2^31 tiles).
+__device__ __forceinline__ Cursor locate(const SmemLayout& s, int n_seqs, int n_kv, long long x64) {
+  const unsigned x = (unsigned)x64;
+  const unsigned per_layer = (unsigned)n_kv * (unsigned)s.pre[n_seqs];
   Cursor c;
-  c.layer = (int)(x / per_layer);
-  long long rem = x - (long long)c.layer * per_layer;
+  const unsigned layer = x / per_layer;
+  unsigned rem = x - layer * per_layer;
   int i = 0;
-  while (i + 1 < n_seqs && (long long)n_kv * s.pre[i + 1] <= rem) ++i;
-  rem -= (long long)n_kv * s.pre[i];
+  while (i + 1 < n_seqs && (unsigned)n_kv * (unsigned)s.pre[i + 1] <= rem) ++i;
+  rem -= (unsigned)n_kv * (unsigned)s.pre[i];
+  const unsigned h = rem / (unsigned)s.nt[i];
+  c.layer = (int)layer;
   c.i = i;
-  c.h = (int)(rem / s.nt[i]);
-  c.k = (int)(rem - (long long)c.h * s.nt[i]);
+  c.h = (int)h;
+  c.k = (int)(rem - h * (unsigned)s.nt[i]);
   return c;
 }
 
@@ -134,23 +139,18 @@ struct AttnLookup {
 };
 
 // Exclusive scan over <= 128 values held 4 per lane by one warp; returns the grand total.
-__device__ __forceinline__ int warp_scan4(const int (&v)[4], int (&excl)[4], int lane) {
-  int sum = 0;
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    excl[k] = sum;
-    sum += v[k];
-  }
-  int inc = sum;
+// Exclusive scan over <= 32 values, one per lane; returns the grand total.
+__device__ __forceinline__ int warp_scan(int v, int& excl, int lane) {
+  int inc = v;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
     const int t = __shfl_up_sync(0xffffffffu, inc, o);
     if (lane >= o) inc += t;
   }
-#pragma unroll
-  for (int k = 0; k < 4; ++k) excl[k] += inc - sum;
+  excl = inc - v;
   return __shfl_sync(0xffffffffu, inc, 31);
 }
+static_assert(kMaxSeqsAttn <= 32, "one sequence per lane in the set-up scans");
 
 // kStep = false: murmur_decode_attn (the cache is as murmur_kv_evict left it).
 // kStep = true : the whole decode step in this one launch (murmur_decode_step): every CTA derives
@@ -233,33 +233,20 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     s.newatt[i] = (kStep && last_b == sp.len) ? 1 : 0;
   }
   __syncthreads();
-  if (warp == 0) {  // prefix sums over <= 64 sequences: tiles, and (step mode) new-block demand
-    int v[4], ex[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) v[k] = (lane * 4 + k < n_seqs) ? s.nt[lane * 4 + k] : 0;
-    const int tiles_all = warp_scan4(v, ex, lane);
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (lane * 4 + k < n_seqs) s.pre[lane * 4 + k] = ex[k];
+  if (warp == 0) {  // prefix sums over <= 32 sequences: tiles, and (step mode) new-block demand
+    int ex;
+    const int tiles_all = warp_scan(lane < n_seqs ? s.nt[lane] : 0, ex, lane);
+    if (lane < n_seqs) s.pre[lane] = ex;
     if (lane == 0) s.pre[n_seqs] = tiles_all;
     if (kStep) {
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const int i = lane * 4 + k;
-        v[k] = (i < n_seqs && ((s.sp[i].len + p - 1) >> plog) > s.old_nblk[i]) ? 1 : 0;
-      }
-      const int blk_all = warp_scan4(v, ex, lane);
+      const int need = (lane < n_seqs && ((s.sp[lane].len + p - 1) >> plog) > s.old_nblk[lane]) ? 1 : 0;
+      const int blk_all = warp_scan(need, ex, lane);
       if (blk_all > free_top) {  // cannot happen after the host-side check; all CTAs agree
         if (lane == 0) s.abort = 3;
-      } else {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {  // pops in call order (C3)
-          if (v[k]) {
-            const int pg = c.free_stack[free_top - 1 - ex[k]];
-            s.newpage[lane * 4 + k] = pg;
-            s.tokpage[lane * 4 + k] = pg;
-          }
-        }
+      } else if (need) {  // pops in call order (C3)
+        const int pg = c.free_stack[free_top - 1 - ex];
+        s.newpage[lane] = pg;
+        s.tokpage[lane] = pg;
       }
       if (lane == 0) s.blk_total = blk_all;
     }
@@ -324,9 +311,15 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   // ring: while one group is in its end-of-item merge (~2 us, no tiles consumed) the other keeps
   // streaming, so the merges no longer stall the CTA's share of HBM.
   const long long total = (long long)prm.n_layers_call * n_kv * s.pre[n_seqs];
+  if (total > 0x7fffffffLL) {  // the range arithmetic below is 32-bit (2^31 tiles = 64 TB of K/V per launch)
+    if (tid == 0) atomicCAS(&c.ctrl[kCtrlError], 0, 5);
+    return;
+  }
   const long long V = min(total, (long long)kGroups * gridDim.x);
   if ((long long)kGroups * blockIdx.x >= V) return;
-  auto range_lo = [&](long long v) { return v * total / V; };
+  // range v = [v total / V, (v + 1) total / V), in 32-bit arithmetic (v r < V^2 <= 2^22)
+  const unsigned rq = (unsigned)total / (unsigned)V, rr = (unsigned)total - rq * (unsigned)V;
+  auto range_lo = [&](long long v) { return (long long)((unsigned)v * rq + ((unsigned)v * rr) / (unsigned)V); };
   if (warp >= kConsumerWarps) {
     // ================================ producer warps (one per group) ================================
     const int gg = warp - kConsumerWarps;
@@ -674,6 +667,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         // split item: publish this range's partial (fragment layout); the last contributor merges all.
         // Contributors = the ranges v_first..v_last that intersect the item.
         const long long item_lo = pos - cur.k;
+        // range containing tile x = floor(((x + 1) V - 1) / total)
         const long long v_first = ((item_lo + 1) * V - 1) / total;
         const long long v_last = ((item_lo + nt_i) * V - 1) / total;
         float* part = c.partials + (size_t)(2 * vrange + (first_segment ? 0 : 1)) * kPartialFloats;
