@@ -402,8 +402,8 @@ def test_decode_step_one_launch_random_policies(dev, seed):
     sbs.close()
 
 
-def test_decode_step_more_than_64_sequences_falls_back(dev):
-    """n_seqs > 64 exceeds the step kernel's tables: murmur_decode_step takes the two-launch form and
+def test_decode_step_more_than_32_sequences_falls_back(dev):
+    """n_seqs > 32 exceeds the step kernel's per-sequence tables (kMaxSeqsAttn): murmur_decode_step takes the two-launch form and
     the attention call is split in chunks; results are the same."""
     specs = [seq_spec(4, 20 + (i % 7), 6, 16, 8, n_sink_out=1) for i in range(70)]
     cfg = Config("many", 90, Geometry(n_layers=1), 16, tuple(specs))
