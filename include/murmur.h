@@ -201,7 +201,8 @@ MURMUR_API murmur_status_t murmur_decode_step(murmur_cache_t* cache, const int32
  * (HOST, pinned or pageable, layouts as above with 1 token per sequence and all layers) to
  * device staging, runs append -> evict -> decode_attn, copies out (HOST bf16
  * [n_layers][n_seqs][n_q_heads][head_dim]) back, all on `stream`; returns after enqueueing
- * (synchronise the stream before reading out_host).  n_seqs <= MURMUR_MAX_SEQS_PER_LAUNCH. */
+ * (synchronise the stream before reading out_host).  n_seqs <= MURMUR_MAX_SEQS_PER_LAUNCH.  If the three
+ * input buffers are packed back to back (k_new, then v_new, then q) they are moved with one copy. */
 MURMUR_API murmur_status_t murmur_decode_step_host(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
                                                    const void* k_new_host, const void* v_new_host,
                                                    const void* q_host, void* out_host, float sm_scale, void* stream);

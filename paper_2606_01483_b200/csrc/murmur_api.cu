@@ -502,9 +502,17 @@ murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_id
   uint8_t* dv = c->ws + c->cv.stage_v;
   uint8_t* dq = c->ws + c->cv.stage_q;
   uint8_t* dout = c->ws + c->cv.stage_out;
-  MM_CUDA(c, cudaMemcpyAsync(dk, k_new_host, kv_b, cudaMemcpyHostToDevice, s));
-  MM_CUDA(c, cudaMemcpyAsync(dv, v_new_host, kv_b, cudaMemcpyHostToDevice, s));
-  MM_CUDA(c, cudaMemcpyAsync(dq, q_host, q_b, cudaMemcpyHostToDevice, s));
+  const uint8_t* hk = reinterpret_cast<const uint8_t*>(k_new_host);
+  const uint8_t* hv = reinterpret_cast<const uint8_t*>(v_new_host);
+  const uint8_t* hq = reinterpret_cast<const uint8_t*>(q_host);
+  if (hv == hk + kv_b && hq == hv + kv_b && dv == dk + kv_b && dq == dv + kv_b) {
+    // k, v, q packed back to back on the host (and in the staging area): one copy instead of three
+    MM_CUDA(c, cudaMemcpyAsync(dk, hk, 2 * kv_b + q_b, cudaMemcpyHostToDevice, s));
+  } else {
+    MM_CUDA(c, cudaMemcpyAsync(dk, hk, kv_b, cudaMemcpyHostToDevice, s));
+    MM_CUDA(c, cudaMemcpyAsync(dv, hv, kv_b, cudaMemcpyHostToDevice, s));
+    MM_CUDA(c, cudaMemcpyAsync(dq, hq, q_b, cudaMemcpyHostToDevice, s));
+  }
   st = murmur_decode_step(c, seq_ids, n_seqs, dk, dv, dq, dout, nullptr, sm_scale, stream);
   if (st != MURMUR_OK) return st;
   MM_CUDA(c, cudaMemcpyAsync(out_host, dout, q_b, cudaMemcpyDeviceToHost, s));

@@ -318,7 +318,14 @@ def test_decode_step_host_matches_device_calls(dev):
         u = a.t_of(0)
         k, v = a.data[0].out_kv(u, u + 1)
         q = a.data[0].q_step(u + 1).unsqueeze(1).contiguous()
-        kh, vh, qh = k.cpu().pin_memory(), v.cpu().pin_memory(), q.cpu().pin_memory()
+        if u % 2:  # packed back to back in one pinned block: moved with a single host-to-device copy
+            hb = torch.empty(2 * k.numel() + q.numel(), dtype=torch.bfloat16).pin_memory()
+            hb[: k.numel()] = k.reshape(-1).cpu()
+            hb[k.numel(): 2 * k.numel()] = v.reshape(-1).cpu()
+            hb[2 * k.numel():] = q.reshape(-1).cpu()
+            kh, vh, qh = hb[: k.numel()].view(k.shape), hb[k.numel(): 2 * k.numel()].view(v.shape), hb[2 * k.numel():].view(q.shape)
+        else:
+            kh, vh, qh = k.cpu().pin_memory(), v.cpu().pin_memory(), q.cpu().pin_memory()
         oh = torch.empty(q.shape, dtype=torch.bfloat16).pin_memory()
         a.gpu.decode_step_host([0], kh, vh, qh, oh)
         torch.cuda.synchronize()
