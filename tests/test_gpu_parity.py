@@ -444,6 +444,25 @@ def test_decode_step_back_to_back_without_host_sync(dev):
     a.close()
 
 
+def test_decode_step_soak_small_pages_many_allocations(dev):
+    """600 one-launch steps enqueued without host synchronisation on a page-16 cache with small
+    windows: every sequence allocates a page every 16 steps while others are freed in the same launch
+    (the free stack is reused continuously).  Integer state and outputs are checked at three points."""
+    specs = [seq_spec(5 + i, 90 + 11 * i, 700, 64, 48, delay=10 + i, n_sink_speech=i % 2, n_sink_out=3) for i in range(6)]
+    cfg = Config("soak", 97, Geometry(n_layers=3), 16, tuple(specs))
+    sbs = _mk(cfg, dev, n_pages=6 * 16 + 40)  # far fewer pages than an un-evicted run needs: reuse is mandatory
+    ids = list(range(6))
+    sbs.bulk_prefill(ids, 1)
+    for k in range(600):
+        order = ids[::-1] if k % 3 == 0 else ids
+        q, out, lse = sbs.fused_step(order, want_lse=True)
+        if k in (199, 399, 599):
+            sbs.check_integer_state(ids)
+            sbs.check_attention(order, q, out, lse)
+    assert sbs.gpu.last_error() == 0
+    sbs.close()
+
+
 # -------------------------------------------------------------------------------- per-layer windows
 def test_decode_attn_windowed_per_layer_groups(dev):
     """murmur_decode_attn_windowed: layers 0-1 attend a tighter window than layers 2-3 while residency
