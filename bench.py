@@ -295,7 +295,7 @@ def run_murmur(args):
     g = cfg.geom
     K, W = args.steps, max(3, args.warmup)
     Ke, We = args.e2e_steps, 3
-    n_steps_total = W + 2 * K + We + Ke + 1
+    n_steps_total = W + 2 * K + We + Ke + 1 + (56 if args.per_layer else 0)
     n_gen = min(n_steps_total, 1100)  # distinct pre-generated step inputs (re-used cyclically beyond that)
     Tmin = min(s.T for s in cfg.seqs)
     extra = max(2, t0 + n_steps_total + 2 - Tmin)  # a long --steps run decodes past the config's T
@@ -437,6 +437,34 @@ def run_murmur(args):
     t_att = sum(attn_list) / Kb2
     t_att_med = attn_list[Kb2 // 2]
 
+    # ---- optional region P: the step as a per-layer engine would issue it -------------------------
+    # (layer l's K/V exist only when layer l runs: append(layer l) + attention(layer l), 28 times,
+    # with the eviction right after the first layer's append has reserved the slots)
+    us_per_layer_mode = None
+    if args.per_layer:
+        Kp = min(K, 50)
+        L = g.n_layers
+
+        def layer_step(s_idx):
+            for l in range(L):
+                cache.kv_append(ids, ones, k_all[s_idx][l:l + 1], v_all[s_idx][l:l + 1], layer_begin=l, layer_end=l + 1)
+                if l == 0:
+                    cache.kv_evict(ids)
+                cache.decode_attn(ids, q_all[s_idx][l:l + 1], out=out[l:l + 1], sm_scale=scale, layer_begin=l, layer_end=l + 1)
+
+        for _ in range(3):
+            layer_step(step_no[0] % n_gen)
+            step_no[0] += 1
+        barrier()
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        for _ in range(Kp):
+            layer_step(step_no[0] % n_gen)
+            step_no[0] += 1
+        p1.record(stream)
+        barrier()
+        us_per_layer_mode = p0.elapsed_time(p1) / Kp * 1e3
+
     # ---- region C: end to end from pinned host buffers -------------------------------------------
     s0 = step_no[0]
     sel = torch.arange(s0, s0 + We + Ke, device=dev) % n_gen
@@ -547,6 +575,7 @@ def run_murmur(args):
         "separate_calls": {"append_us": t_app, "evict_us": t_evi, "attn_us": t_att, "attn_median_us": t_att_med,
                            "attn_hbm_gbs": attn_only, "attn_pct_of_measured_peak": 100.0 * attn_only / peak,
                            "note": "the same step as three API calls, one event pair per call (includes launch gaps)"},
+        "per_layer_mode_us": us_per_layer_mode,
         "attn_us": t_att, "append_us": t_app, "evict_us": t_evi,
         "attn_hbm_gbs": attn_only, "attn_pct_of_measured_peak": 100.0 * attn_only / peak,
         "step_hbm_gbs": alg_bytes / (us_step * 1e-6) / 1e9,
@@ -629,6 +658,8 @@ def main():
     ap.add_argument("--variant", default="", choices=["", "generic", "mma"])
     ap.add_argument("--grid", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--per-layer", action="store_true",
+                    help="also time the step issued layer by layer (append(l) + attention(l) x 28, 57 launches)")
     ap.add_argument("--no-pdl", action="store_true", help="A/B: launch the step's kernels without programmatic dependent launch")
     ap.add_argument("--fuse", type=int, default=-1, help="A/B: MURMUR_OPT_FUSE_STEP value (2 = one launch per step, default)")
     ap.add_argument("--no-fuse", action="store_true", help="A/B: murmur_decode_step as three launches (append, evict, attention)")
