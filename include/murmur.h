@@ -283,19 +283,22 @@ MURMUR_API murmur_status_t murmur_kv_gather(murmur_cache_t* cache, int32_t seq, 
 /* Device error word: 0 or the first MURMUR_ERR_* a kernel detected since creation. */
 MURMUR_API murmur_status_t murmur_get_last_error(murmur_cache_t* cache, int32_t* device_err_out, void* stream);
 
-/* Per-CTA trace of the LAST tensor-core attention launch (profiling aid): out is HOST
- * uint64[n][4] = {globaltimer ns when the CTA started its work, at CTA end, SM id, tiles processed}; *n_out = CTAs
- * of that launch (0 if the last launch was the generic variant). */
-MURMUR_API murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* cache, uint64_t* out, int32_t cap_ctas,
-                                                      int32_t* n_out, void* stream);
-
-/* globaltimer stamps (ns) of the LAST step prologue (profiling aid), HOST uint64[16]:
+#ifdef MURMUR_TRACE
+/* Profiling builds only (library compiled with -DMURMUR_TRACE: `python -m paper_2606_01483_b200.build --trace`);
+ * the production kernels carry no time stamps and the production library does not export these. */
+#define MURMUR_TRACE_API MURMUR_API
+/* Per-CTA trace of the LAST tensor-core attention launch: out is HOST uint64[n][4] = {globaltimer ns when
+ * the CTA started its work, at CTA end, SM id, tiles processed}; *n_out = CTAs of that launch (0 if the
+ * last launch was the generic variant). */
+MURMUR_TRACE_API murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* cache, uint64_t* out, int32_t cap_ctas,
+                                                            int32_t* n_out, void* stream);
+/* globaltimer stamps (ns) of the LAST step prologue, HOST uint64[16]:
  * [0] append kernel start (CTA 0, after its dependency wait)  [1] last append CTA through the ticket
  * [2] integer state committed  [3] eviction body start  [4] eviction body end;  the last CTA's own
  * phases: [5] after its dependency wait [6] old state loaded [7] prefix sums done [8] row loads
- * issued [9] eviction tasks done [10] page ids consumed [11] its block index; rest unused.
- * Same clock as murmur_debug_attn_timeline. */
-MURMUR_API murmur_status_t murmur_debug_step_trace(murmur_cache_t* cache, uint64_t* out16, void* stream);
+ * issued [9] eviction tasks done [10] page ids consumed [11] its block index; rest unused. */
+MURMUR_TRACE_API murmur_status_t murmur_debug_step_trace(murmur_cache_t* cache, uint64_t* out16, void* stream);
+#endif
 
 /* ---- options / stats --------------------------------------------------------------------- */
 MURMUR_API murmur_status_t murmur_set_option(murmur_cache_t* cache, int32_t option, int32_t value);

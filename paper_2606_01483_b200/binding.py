@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = [
     "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
     "murmur_decode_step", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
-    "murmur_debug_attn_timeline", "murmur_debug_step_trace", "murmur_profile_scratch_bytes", "murmur_attn_profile",
+    "murmur_profile_scratch_bytes", "murmur_attn_profile",
     "murmur_decode_attn_windowed", "murmur_prefill_attn", "murmur_chunk_plan",
     "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
     "murmur_last_cuda_error", "murmur_version",
@@ -96,8 +96,9 @@ def lib() -> C.CDLL:
     L.murmur_kv_get_free_stack.argtypes = [vp, vp, i64, vp, vp]
     L.murmur_kv_gather.argtypes = [vp, i32, vp, i32, i32, i32, vp, vp, vp]
     L.murmur_get_last_error.argtypes = [vp, vp, vp]
-    L.murmur_debug_attn_timeline.argtypes = [vp, vp, i32, vp, vp]
-    L.murmur_debug_step_trace.argtypes = [vp, vp, vp]
+    if hasattr(L, "murmur_debug_attn_timeline"):  # profiling builds only (-DMURMUR_TRACE)
+        L.murmur_debug_attn_timeline.argtypes = [vp, vp, i32, vp, vp]
+        L.murmur_debug_step_trace.argtypes = [vp, vp, vp]
     L.murmur_decode_attn_windowed.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, C.c_float, vp, vp]
     L.murmur_chunk_plan.argtypes = [vp, vp, i32, C.c_float, vp, i32, vp]
     L.murmur_prefill_attn.argtypes = [vp, i32, i32, i32, vp, vp, vp, i32, i32, C.c_float, vp]
@@ -251,7 +252,7 @@ class MurmurCache:
         sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
         nbytes = self.L.murmur_profile_scratch_bytes(self.h, ids.ctypes.data, len(ids), layer_begin, layer_end)
         if nbytes == 0:
-            raise MurmurError("murmur_profile_scratch_bytes: bad arguments")
+            raise MurmurError(1, "murmur_profile_scratch_bytes: bad arguments")
         scratch = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         out = torch.zeros(shape[:3] + (12,), dtype=torch.int32, device=self.device)
         pol = (C.c_int32 * 5)(*candidate) if candidate is not None else None
@@ -334,7 +335,10 @@ class MurmurCache:
         return e.value
 
     def attn_timeline(self) -> np.ndarray:
-        """uint64 [n_ctas, 4] = (start ns, end ns, SM id, tiles) of the last tensor-core attention launch."""
+        """uint64 [n_ctas, 4] = (start ns, end ns, SM id, tiles) of the last tensor-core attention launch.
+        Needs a profiling build of the library (python -m paper_2606_01483_b200.build --trace)."""
+        if not hasattr(self.L, "murmur_debug_attn_timeline"):
+            raise MurmurError(5, "library built without MURMUR_TRACE")
         a = np.zeros((1024, 4), dtype=np.uint64)
         n = C.c_int32(0)
         self._check(self.L.murmur_debug_attn_timeline(self.h, a.ctypes.data, 1024, C.byref(n), _stream()))
@@ -342,6 +346,8 @@ class MurmurCache:
 
     def step_trace(self) -> np.ndarray:
         """uint64 [16]: globaltimer stamps of the last step prologue (see murmur_debug_step_trace)."""
+        if not hasattr(self.L, "murmur_debug_step_trace"):
+            raise MurmurError(5, "library built without MURMUR_TRACE")
         a = np.zeros(16, dtype=np.uint64)
         self._check(self.L.murmur_debug_step_trace(self.h, a.ctypes.data, _stream()))
         return a
@@ -367,7 +373,7 @@ def chunk_plan(segments, max_len: float = 300.0):
     st = lib().murmur_chunk_plan(a.ctypes.data, b.ctypes.data, len(seg), C.c_float(max_len), first.ctypes.data, len(first),
                                  C.byref(n))
     if st != 0:
-        raise MurmurError(f"murmur_chunk_plan: {STATUS_NAMES.get(st, st)}")
+        raise MurmurError(st, "murmur_chunk_plan")
     cuts = list(first[: n.value]) + [len(seg)]
     return [list(range(cuts[j], cuts[j + 1])) for j in range(n.value)]
 

@@ -168,7 +168,9 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   const int n_threads = kMmaThreads + (kStep ? 32 : 0);
   const int n_seqs = list.n, n_kv = c.n_kv, G = c.group;
   const int p = c.p, plog = c.p_log2;
+#ifdef MURMUR_TRACE
   unsigned long long* trace = c.timeline + (size_t)blockIdx.x * kTimelineWords;
+#endif
   pdl_launch_dependents();
 
   // ---- setup: barriers, zeroed padding rows of the Q buffers ---------------------------------------
@@ -191,12 +193,14 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   // Everything above touches only this CTA's shared memory; from here on the kernel reads what
   // earlier kernels of the stream wrote and writes buffers the previous launch may still use.
   pdl_wait();
+#ifdef MURMUR_TRACE
   if (tid == 0) {
     trace[0] = globaltimer_ns();
     trace[1] = 0ull;
     trace[2] = smid();
     trace[3] = 0ull;
   }
+#endif
   // ---- per-sequence state: policy + length -> tile count; step mode: the length after this step ----
   const int free_top = kStep ? c.ctrl[kCtrlFreeTop] : 0;
   for (int i = tid; i < n_seqs; i += n_threads) {
@@ -220,7 +224,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       sp.w_s = prm.w_s; sp.d = prm.d; sp.k_s = prm.k_s; sp.w_o = prm.w_o; sp.k_o = prm.k_o;
       s.sp[i] = sp;
       s.tg[i] = make_tilegen(sp, p, plog);
-    } else if (sd.tg_len[sp.len & 1] == sp.len) {
+    } else if (ld_acquire(&sd.tg_len[sp.len & 1]) == sp.len) {  // the length validates the table stored before it
       s.tg[i] = sd.tg[sp.len & 1];
     } else {
       s.tg[i] = make_tilegen(sp, p, plog);
@@ -701,10 +705,12 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     ++item_no;
     next_item(s, n_seqs, n_kv, cur);
   }
+#ifdef MURMUR_TRACE
   if (w4 == 0 && lane == 0) {
     atomicMax(&trace[1], globaltimer_ns());
     atomicAdd(&trace[3], (unsigned long long)(hi - lo));
   }
+#endif
 }
 
 }  // namespace
@@ -714,13 +720,9 @@ namespace {
 template <bool kStep>
 cudaError_t launch_mma(const CacheView& c, const SeqList& list, const AttnParams& prm_in, int grid, bool pdl,
                        cudaStream_t st, LaunchInfo* info) {
-  static bool attr_set = false;
   const int smem = (int)sizeof(SmemLayout);
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(attn_mma_kernel<kStep>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  cudaError_t ea = opt_in_smem_once(kStep ? kSmemStep : kSmemAttn, reinterpret_cast<const void*>(attn_mma_kernel<kStep>), smem);
+  if (ea != cudaSuccess) return ea;
   if (grid > kMaxAttnGrid) grid = kMaxAttnGrid;
   AttnParams prm = prm_in;
   PdlLaunch l(dim3((unsigned)grid), dim3(kMmaThreads + (kStep ? 32 : 0)), (size_t)smem, st, pdl);

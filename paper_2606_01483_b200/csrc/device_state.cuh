@@ -103,8 +103,13 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
 // 2 commit done   3 evict body start   4 evict body end
 // 5.. the last CTA's own phases: 5 after its dependency wait, 6 old state loaded, 7 prefix sums
 // done, 8 row loads issued, 9 eviction tasks done, 10 page ids consumed, 11 block index
+// Compiled in only with -DMURMUR_TRACE (profiling builds): the production kernels carry no stamps.
 __device__ __forceinline__ void step_stamp(const CacheView& c, int k) {
+#ifdef MURMUR_TRACE
   c.timeline[(size_t)kMaxAttnGrid * kTimelineWords + k] = globaltimer_ns();
+#else
+  (void)c; (void)k;
+#endif
 }
 #endif
 
@@ -139,6 +144,12 @@ __device__ __forceinline__ SeqParams load_params(const SeqDev& s) {
 // and flushed, so the ordering is that of ordinary stream serialisation; only launch latency and
 // kernel prologues overlap.  Both are no-ops when the kernel was launched without the attribute.
 #ifdef __CUDACC__
+// Acquire load (gpu scope): pairs with the writer's __threadfence() before it publishes a flag / length.
+__device__ __forceinline__ int32_t ld_acquire(const int32_t* p) {
+  int32_t v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 #endif
@@ -159,6 +170,12 @@ struct PdlLaunch {
     cfg.numAttrs = 1;
   }
 };
+
+// Opt a kernel in to `smem` bytes of dynamic shared memory, once per (kernel, device): the attribute is
+// per device, and handles on several GPUs may live in one process (any host thread).  Defined in
+// murmur_api.cu; `slot` identifies the kernel.
+enum SmemKernel { kSmemAttn = 0, kSmemStep, kSmemPrefill, kSmemPrefillUmma, kSmemIndexed, kSmemKernels };
+cudaError_t opt_in_smem_once(int slot, const void* func, int smem);
 
 // ---- host launchers (one per .cu) ------------------------------------------------------------
 struct LaunchInfo {

@@ -194,7 +194,10 @@ __device__ __forceinline__ void evict_task(const CacheView& c, int id, const Seq
       // use by concurrent readers, which never read an invalid slot) and the next decode step's
       SeqParams sp1 = sp;
       sp1.len += 1;
+      sd.tg_len[sp1.len & 1] = -1;  // invalidate, then the table, then the length that validates it
+      __threadfence();
       sd.tg[sp1.len & 1] = make_tilegen(sp1, p, plog);
+      __threadfence();
       sd.tg_len[sp1.len & 1] = sp1.len;
       if (sd.tg_len[sp.len & 1] != sp.len) {
         sd.tg[sp.len & 1] = g;
@@ -207,18 +210,22 @@ __device__ __forceinline__ void evict_task(const CacheView& c, int id, const Seq
 }
 
 // Warp tasks: s_ndead[i] = mapped blocks inside the dead ranges of sequence i at length
-// sp_sh[i].len (+ extra_len[i] if given).
+// sp_sh[i].len (+ extra_len[i] if given).  With old_nblk (the fused append+evict prologue, which
+// counts BEFORE the append's commit) the blocks [old_nblk[i], blocks at that length) count as mapped:
+// the commit maps them before evict_free pushes (a block can be mapped and dead in the same step
+// only when p == 1 and w_out == 0).
 __device__ __forceinline__ void evict_count(const CacheView& c, const int32_t* ids, int n, const SeqParams* sp_sh,
-                                            const int32_t* extra_len, int* s_ndead) {
+                                            const int32_t* extra_len, int* s_ndead, const int* old_nblk = nullptr) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   for (int i = warp; i < n; i += n_warps) {
     SeqParams sp = sp_sh[i];
     if (extra_len != nullptr) sp.len += extra_len[i];
     const DeadRanges dr = dead_block_ranges(sp, c.p_log2);
     const int32_t* tab = c.block_table + (size_t)ids[i] * c.max_blocks;
+    const int tab_end = old_nblk != nullptr ? old_nblk[i] : 0x7fffffff;  // blocks from here on: mapped by the pending commit
     int cnt = 0;
-    for (int b = dr.lo0 + lane; b < dr.hi0; b += 32) cnt += (tab[b] >= 0);
-    for (int b = dr.lo1 + lane; b < dr.hi1; b += 32) cnt += (tab[b] >= 0);
+    for (int b = dr.lo0 + lane; b < dr.hi0; b += 32) cnt += (b >= tab_end) || (tab[b] >= 0);
+    for (int b = dr.lo1 + lane; b < dr.hi1; b += 32) cnt += (b >= tab_end) || (tab[b] >= 0);
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     if (lane == 0) s_ndead[i] = cnt;
   }

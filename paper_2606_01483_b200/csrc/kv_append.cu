@@ -92,10 +92,15 @@ struct RowUnit {
   }
 };
 
+// page: >= 0 the row's physical page; kRowBad = a position that should be mapped is not (device error);
+// kRowSkip = nothing to store (no row, or - write-only calls - a position the eviction has already freed).
+constexpr int kRowBad = -1, kRowSkip = -2;
+
 __device__ __forceinline__ RowUnit locate_row(const CacheView& c, const AppendList& list, long long u, long long rows_src,
                                               int total_tokens, int layer_begin, int n, int free_top, int sub,
                                               const uint4* k_new, const uint4* v_new, const int* s_tok_off,
-                                              const int* s_blk_off, const int* s_old_nblk, const SeqParams* s_sp) {
+                                              const int* s_blk_off, const int* s_old_nblk, const SeqParams* s_sp,
+                                              bool reserve) {
   const int is_v = u >= rows_src;
   const long long r = is_v ? u - rows_src : u;
   int head, tau, layer;
@@ -121,8 +126,25 @@ __device__ __forceinline__ RowUnit locate_row(const CacheView& c, const AppendLi
   const int b = x >> c.p_log2;
   const int slot = x & (c.p - 1);
   RowUnit ru;
-  if (b < s_old_nblk[i]) ru.page = c.block_table[(size_t)list.ids[i] * c.max_blocks + b];
-  else ru.page = c.free_stack[free_top - 1 - (s_blk_off[i] + (b - s_old_nblk[i]))];
+  if (b < s_old_nblk[i]) {
+    ru.page = c.block_table[(size_t)list.ids[i] * c.max_blocks + b];
+    if (!reserve && ru.page < 0) {
+      // write-only call (layer_begin > 0): the slot was reserved by the layer-0 call, and an evict may
+      // have run since.  A position that evict freed is dead for good - its row is not stored; any
+      // other unmapped position is an error.
+      SeqParams cur = s_sp[i];
+      cur.len += list.n_tok[i];
+      Interval dv[2];
+      const int nd = dead_intervals(cur, dv);
+      bool dead = false;
+      for (int k = 0; k < nd; ++k) dead |= (x >= dv[k].a && x < dv[k].b);
+      ru.page = dead ? kRowSkip : kRowBad;
+    }
+  } else if (reserve) {
+    ru.page = c.free_stack[free_top - 1 - (s_blk_off[i] + (b - s_old_nblk[i]))];
+  } else {
+    ru.page = kRowBad;  // never read the free stack without having reserved
+  }
   ru.src = (is_v ? v_new : k_new) + r * 16 + sub;
   ru.is_v = is_v;
   // pre-swizzled row (see device_state.cuh): chunk `sub` of slot `slot` sits at position sub ^ (slot & 7)
@@ -171,7 +193,9 @@ append_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Appen
   pdl_launch_dependents();
   pdl_wait();  // the previous kernel may still be reading the tables this one rewrites
   if (blockIdx.x == 0 && tid == 0) step_stamp(c, 0);
+#ifdef MURMUR_TRACE
   const unsigned long long t_wait = globaltimer_ns();
+#endif
   const int free_top = c.ctrl[kCtrlFreeTop];
 
   // Phase A: per-sequence old fill level and new-block demand (same result in every CTA).
@@ -181,10 +205,15 @@ append_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Appen
     if (!reserve) sp.len -= list.n_tok[i];
     if (!s.active || sp.len < 0) set_error(c, 2);
     s_sp[i] = sp;
-    s_old_nblk[i] = (max(sp.len, 0) + c.p - 1) >> c.p_log2;
+    // reserve: blocks mapped before this call.  Write-only call: every target block was mapped by the
+    // reserving call, so ALL lookups go through the table (blocks at the current length).
+    const int len_tab = reserve ? max(sp.len, 0) : max(sp.len, 0) + list.n_tok[i];
+    s_old_nblk[i] = (len_tab + c.p - 1) >> c.p_log2;
   }
   __syncthreads();
+#ifdef MURMUR_TRACE
   const unsigned long long t_ld = globaltimer_ns();
+#endif
   if (tid < 32) {  // exclusive prefix sums over <= 128 sequences, in call order: 4 per lane + warp scan
     int tok4[4], blk4[4], tok = 0, blk = 0, bad = 0;
 #pragma unroll
@@ -229,7 +258,9 @@ append_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Appen
   }
   __syncthreads();
   if (!s_flag) return;
+#ifdef MURMUR_TRACE
   const unsigned long long t_a = globaltimer_ns();
+#endif
 
   // Phase B: scatter rows.  The integer state may be committed as soon as every CTA has READ what
   // it needs of the old state (page ids); the rows themselves only have to land before the kernel
@@ -243,28 +274,33 @@ append_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Appen
   const long long unit_stride = (long long)gridDim.x * units_per_cta;
   const bool one_pass = units <= unit_stride;
   int bad_page = 0;
+#ifdef MURMUR_TRACE
   unsigned long long t_b = 0, t_l = 0, t_t = 0;
+#define MM_STAMP(v) v = globaltimer_ns()
+#else
+#define MM_STAMP(v)
+#endif
   if (one_pass) {
     const long long u = (long long)blockIdx.x * units_per_cta + (tid >> 4);
     RowUnit ru;
-    ru.page = 0;
+    ru.page = kRowSkip;
     uint4 val = make_uint4(0u, 0u, 0u, 0u);
     if (u < units) {
       ru = locate_row(c, list, u, rows_src, total_tokens, layer_begin, n, free_top, sub, k_new, v_new, s_tok_off,
-                      s_blk_off, s_old_nblk, s_sp);
+                      s_blk_off, s_old_nblk, s_sp, reserve != 0);
       val = *ru.src;
     }
-    t_l = globaltimer_ns();
+    MM_STAMP(t_l);
     if (fuse_evict) {
       fused_evict_tasks(c, list, n, free_top, s_sp, s_blk_off, s_old_nblk);
       // every CTA also counts the blocks the eviction will free (the dead ranges at the new
       // lengths; nothing remaps them before the ticket), so that the last CTA can push at once
-      evict_count(c, list.ids, n, s_sp, list.n_tok, s_ndead);
+      evict_count(c, list.ids, n, s_sp, list.n_tok, s_ndead, s_old_nblk);
     }
-    t_t = globaltimer_ns();
+    MM_STAMP(t_t);
     // the barrier consumes every thread's page id: all of this CTA's reads of the old state are done
-    bad_page = __syncthreads_or(ru.page < 0);
-    t_b = globaltimer_ns();
+    bad_page = __syncthreads_or(ru.page == kRowBad);
+    MM_STAMP(t_b);
     if (reserve) {
       if (tid == 0) s_flag = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
       __syncthreads();
@@ -278,17 +314,17 @@ append_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Appen
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const long long u = u0 + k * unit_stride;
-        ru[k].page = -2;  // no row
+        ru[k].page = kRowSkip;  // no row
         if (u < units) {
           ru[k] = locate_row(c, list, u, rows_src, total_tokens, layer_begin, n, free_top, sub, k_new, v_new, s_tok_off,
-                             s_blk_off, s_old_nblk, s_sp);
+                             s_blk_off, s_old_nblk, s_sp, reserve != 0);
           val[k] = *ru[k].src;
         }
       }
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         if (ru[k].page >= 0) *ru[k].dst(c) = val[k];
-        else if (ru[k].page == -1) bad_page = 1;
+        else if (ru[k].page == kRowBad) bad_page = 1;
       }
     }
     if (fuse_evict) fused_evict_tasks(c, list, n, free_top, s_sp, s_blk_off, s_old_nblk);
@@ -300,10 +336,12 @@ append_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Appen
   }
   if (bad_page && tid == 0) set_error(c, 2);
   if (!reserve || !s_flag) return;
+#ifdef MURMUR_TRACE
   if (tid == 0) {
     unsigned long long* tr = c.timeline + (size_t)kMaxAttnGrid * kTimelineWords;
     tr[5] = t_wait; tr[6] = t_ld; tr[7] = t_a; tr[8] = t_l; tr[9] = t_t; tr[10] = t_b; tr[11] = blockIdx.x;
   }
+#endif
 
   // Phase C: the last CTA through the ticket commits the new integer state.
   if (tid == 0) step_stamp(c, 1);

@@ -7,6 +7,7 @@
 // reading device memory.  Every state transition itself runs in the kernels.
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -15,6 +16,21 @@
 #include "device_state.cuh"
 
 using namespace murmur;
+
+namespace murmur {
+cudaError_t opt_in_smem_once(int slot, const void* func, int smem) {
+  constexpr int kMaxDevices = 64;
+  static std::atomic<bool> done[kSmemKernels][kMaxDevices];  // zero-initialised; setting twice is harmless
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const bool tracked = slot >= 0 && slot < kSmemKernels && dev >= 0 && dev < kMaxDevices;
+  if (tracked && done[slot][dev].load(std::memory_order_acquire)) return cudaSuccess;
+  e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess && tracked) done[slot][dev].store(true, std::memory_order_release);
+  return e;
+}
+}  // namespace murmur
 
 namespace {
 
@@ -709,6 +725,7 @@ murmur_status_t murmur_get_last_error(murmur_cache_t* c, int32_t* device_err_out
   return MURMUR_OK;
 }
 
+#ifdef MURMUR_TRACE
 murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* c, uint64_t* out, int32_t cap_ctas, int32_t* n_out,
                                            void* stream) {
   if (!c || !n_out || cap_ctas < 0 || (cap_ctas > 0 && !out)) return MURMUR_ERR_INVALID_ARG;
@@ -728,6 +745,7 @@ murmur_status_t murmur_debug_step_trace(murmur_cache_t* c, uint64_t* out16, void
                         cudaMemcpyDeviceToHost));
   return MURMUR_OK;
 }
+#endif  // MURMUR_TRACE
 
 murmur_status_t murmur_set_option(murmur_cache_t* c, int32_t option, int32_t value) {
   if (!c) return MURMUR_ERR_INVALID_ARG;

@@ -247,13 +247,9 @@ prefill_attn_kernel(const __grid_constant__ CacheView c, const __grid_constant__
 cudaError_t launch_prefill_attn(const CacheView& c, int seq, int pos_begin, int n_tok, const void* q, void* out,
                                 float* lse, int layer_begin, int layer_end, float sm_scale, cudaStream_t st,
                                 LaunchInfo* info) {
-  static bool attr_set = false;
   const int smem = (int)sizeof(PfSmem);
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(prefill_attn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  cudaError_t ea = opt_in_smem_once(kSmemPrefill, reinterpret_cast<const void*>(prefill_attn_kernel), smem);
+  if (ea != cudaSuccess) return ea;
   PfParams prm{};
   prm.q = reinterpret_cast<const uint16_t*>(q);
   prm.out = reinterpret_cast<uint16_t*>(out);

@@ -32,9 +32,36 @@ def out_to_f64(out_bf16: torch.Tensor) -> np.ndarray:
     return o_attn.bf16_bits_to_f64(workloads.to_bits(out_bf16))
 
 
+class RowStore:
+    """K (or V) rows of one sequence by absolute position, uint16 [L, n_pos, n_kv, d], grown in place
+    (the full-size cases hold ~100 MB per sequence: no re-concatenation per step)."""
+
+    def __init__(self):
+        self.buf: Optional[np.ndarray] = None
+        self.n = 0
+
+    def append(self, bits: np.ndarray):
+        n_new = bits.shape[1]
+        if self.buf is None or self.n + n_new > self.buf.shape[1]:
+            cap = self.n + n_new + max(64, (self.n + n_new) // 4)
+            nb = np.empty((bits.shape[0], cap) + bits.shape[2:], dtype=np.uint16)
+            if self.buf is not None:
+                nb[:, : self.n] = self.buf[:, : self.n]
+            self.buf = nb
+        self.buf[:, self.n: self.n + n_new] = bits
+        self.n += n_new
+
+    def rows(self) -> np.ndarray:
+        return self.buf[:, : self.n]
+
+
 class SideBySide:
     def __init__(self, cfg: workloads.Config, device="cuda:0", n_pages: Optional[int] = None, max_seqs: Optional[int] = None,
-                 extra_tokens: int = 0, variant: Optional[int] = None, grid: Optional[int] = None, use_c_oracle: bool = False):
+                 extra_tokens: int = 0, variant: Optional[int] = None, grid: Optional[int] = None, use_c_oracle: bool = False,
+                 data: Optional[list] = None, bulk_bits: Optional[dict] = None):
+        """data: SeqData list shared between cases that use the same seeded values (the config-4 sweep);
+        bulk_bits: {(seq, n_tokens): (k_bits, v_bits)} host copies of bulk appends, filled and re-used
+        across such cases (saves the device-to-host copy of ~2 GB per case)."""
         from paper_2606_01483_b200 import MurmurCache, binding
 
         self.cfg = cfg
@@ -51,10 +78,11 @@ class SideBySide:
         if grid is not None:
             self.gpu.set_option(binding.MURMUR_OPT_ATTN_GRID, grid)
         self.oracle = o_cache.OraclePagedCache(n_pages, cfg.page_size, max_seqs, max_blocks)
-        self.data = [workloads.SeqData(cfg, i, device=device) for i in range(cfg.batch)]
+        self.data = data if data is not None else [workloads.SeqData(cfg, i, device=device) for i in range(cfg.batch)]
+        self.bulk_bits = bulk_bits
         # oracle-side K/V by absolute position: uint16 [L, n_pos, n_kv, d] per sequence
-        self.k_store: Dict[int, List[np.ndarray]] = {i: [] for i in range(cfg.batch)}
-        self.v_store: Dict[int, List[np.ndarray]] = {i: [] for i in range(cfg.batch)}
+        self.k_store: Dict[int, RowStore] = {i: RowStore() for i in range(cfg.batch)}
+        self.v_store: Dict[int, RowStore] = {i: RowStore() for i in range(cfg.batch)}
         self.scale = 1.0 / math.sqrt(g.head_dim)
         self.use_c_oracle = use_c_oracle
         self.max_abs_seen = 0.0
@@ -65,14 +93,18 @@ class SideBySide:
 
     # ---- helpers ---------------------------------------------------------------------------
     def _store(self, i: int, k: torch.Tensor, v: torch.Tensor):
-        self.k_store[i].append(workloads.to_bits(k))
-        self.v_store[i].append(workloads.to_bits(v))
+        key = (i, k.shape[1])
+        if self.bulk_bits is not None and k.shape[1] > 64:
+            if key not in self.bulk_bits:
+                self.bulk_bits[key] = (workloads.to_bits(k), workloads.to_bits(v))
+            kb, vb = self.bulk_bits[key]
+        else:
+            kb, vb = workloads.to_bits(k), workloads.to_bits(v)
+        self.k_store[i].append(kb)
+        self.v_store[i].append(vb)
 
     def kv_by_position(self, i: int):
-        if len(self.k_store[i]) > 1:
-            self.k_store[i] = [np.concatenate(self.k_store[i], axis=1)]
-            self.v_store[i] = [np.concatenate(self.v_store[i], axis=1)]
-        return self.k_store[i][0], self.v_store[i][0]
+        return self.k_store[i].rows(), self.v_store[i].rows()
 
     def t_of(self, i: int) -> int:
         return self.oracle.seqs[i].t
@@ -138,6 +170,34 @@ class SideBySide:
         self.gpu.decode_step(seq_ids, k_new, v_new, q, out, lse, self.scale)
         return q, out, lse
 
+    def per_layer_step(self, seq_ids: Sequence[int], want_lse: bool = False):
+        """One decode step issued the way an engine that produces layer l's K/V at layer l would:
+        append(layer 0) reserves the slots, evict, attention(layer 0); then for every further layer
+        append(layer l) only writes rows, attention(layer l).  The oracle side does append -> evict.
+        Returns (q, out, lse) over all layers."""
+        ks, vs = [], []
+        for i in seq_ids:
+            u = self.t_of(i)
+            k, v = self.data[i].out_kv(u, u + 1)
+            ks.append(k)
+            vs.append(v)
+            self._store(i, k, v)
+        k_new = torch.cat(ks, dim=1).contiguous()  # [L, n_seqs, kv, d]
+        v_new = torch.cat(vs, dim=1).contiguous()
+        ones = [1] * len(seq_ids)
+        self.oracle.append(seq_ids, ones)
+        self.oracle.evict(seq_ids)
+        q = self.queries(seq_ids)
+        out = torch.empty_like(q)
+        lse = torch.empty(q.shape[:3], dtype=torch.float32, device=self.device) if want_lse else None
+        for l in range(q.shape[0]):
+            self.gpu.kv_append(seq_ids, ones, k_new[l:l + 1].contiguous(), v_new[l:l + 1].contiguous(), layer_begin=l, layer_end=l + 1)
+            if l == 0:
+                self.gpu.kv_evict(seq_ids)
+            self.gpu.decode_attn(seq_ids, q[l:l + 1].contiguous(), out=out[l:l + 1], lse=lse[l:l + 1] if want_lse else None,
+                                 sm_scale=self.scale, layer_begin=l, layer_end=l + 1)
+        return q, out, lse
+
     def queries(self, seq_ids: Sequence[int]) -> torch.Tensor:
         """[L, n_seqs, n_q, d]: query of each sequence's newest output token."""
         qs = [self.data[i].q_step(max(1, self.t_of(i))) for i in seq_ids]
@@ -170,8 +230,10 @@ class SideBySide:
         assert self.gpu.last_error() == 0
         assert self.gpu.stats()["free_pages"] == len(self.oracle.free_stack), "host mirror of free pages is off"
 
-    def check_gather(self, i: int, layers: Sequence[int] = (0,)):
-        """Rows gathered through the GPU's tables == the rows handed to append (bit-exact)."""
+    def check_gather(self, i: int, layers: Optional[Sequence[int]] = (0,)):
+        """Rows gathered through the GPU's tables == the rows handed to append (bit-exact); layers=None: all."""
+        if layers is None:
+            layers = range(self.cfg.geom.n_layers)
         res = sorted(o_policy.resident_positions(*self._regions(i), self.t_of(i), self.oracle.seqs[i].pol))
         res = [x for x in res if x < self.oracle.seqs[i].length]
         kb, vb = self.kv_by_position(i)
@@ -189,8 +251,12 @@ class SideBySide:
         return o_attn.attend_retained(q_bits_layer, kb[layer], vb[layer], self.oracle.retained(i), self.scale)
 
     def check_attention(self, seq_ids: Sequence[int], q: torch.Tensor, out: torch.Tensor, lse: Optional[torch.Tensor] = None,
-                        layers: Optional[Sequence[int]] = None, seq_subset: Optional[Sequence[int]] = None):
-        """Compares out[l, j] with the fp64 oracle for the chosen layers / sequences."""
+                        layers: Optional[Sequence[int]] = None, seq_subset: Optional[Sequence[int]] = None,
+                        retained: Optional[Dict[int, Sequence[int]]] = None):
+        """Compares out[l, j] with the fp64 oracle for the chosen layers / sequences (default: all of
+        them).  retained: the oracle's retained sets as recorded at the step `out` belongs to, when that
+        is not the oracle's current step (outputs of earlier steps checked after the fact)."""
+        ret_of = (lambda i: retained[i]) if retained is not None else self.oracle.retained
         L = q.shape[0]
         layers = range(L) if layers is None else layers
         got = out_to_f64(out)
@@ -205,14 +271,17 @@ class SideBySide:
 
                 kb, vb = self.kv_by_position(i)
                 ls = list(layers)
-                o_all, lse_all, _ = oc.load().attend(q_bits[ls][:, j], kb[ls], vb[ls], self.oracle.retained(i), self.scale)
+                full = ls == list(range(kb.shape[0]))
+                o_all, lse_all, _ = oc.load().attend(q_bits[ls][:, j], kb if full else kb[ls], vb if full else vb[ls],
+                                                     ret_of(i), self.scale)
                 for a, layer in enumerate(ls):
                     errs.append(np.abs(got[layer, j] - o_all[a]))
                     if lse_np is not None:
                         assert np.max(np.abs(lse_np[layer, j] - lse_all[a])) < 2e-3
             else:
                 for layer in layers:
-                    o_ref, lse_ref, _ = self.oracle_attend(i, q_bits[layer, j], layer)
+                    kb, vb = self.kv_by_position(i)
+                    o_ref, lse_ref, _ = o_attn.attend_retained(q_bits[layer, j], kb[layer], vb[layer], ret_of(i), self.scale)
                     errs.append(np.abs(got[layer, j] - o_ref))
                     if lse_np is not None:
                         assert np.max(np.abs(lse_np[layer, j] - lse_ref)) < 2e-3, "lse mismatch"

@@ -2,9 +2,10 @@
 
 Integer state (retained sets, compacted page tables, run descriptors, free stack) must be
 bit-exact; attention within max-abs 2e-2 / mean-abs 2e-3 (BASELINE.json north_star).
-Small and reduced-layer cases compare every element; the full-size cases (configs 2, 3, 5 at
-28 layers, in the launch configuration bench.py times) compare all integer state and
-sampled (sequence, layer) attention outputs the oracle computes one by one.
+Small and reduced-layer cases compare every element.  The full-size cases (configs 2, 3, 5 and all
+15 points of config 4 at 28 layers, in the launch configuration bench.py times) compare all integer
+state and, for the one-launch steps, EVERY (sequence, layer, head) of the output with the plain-C
+fp64 oracle; the three-call steps before them compare sampled (sequence, layer) items.
 """
 import math
 import random
@@ -225,6 +226,39 @@ def test_config4_sweep_points_two_layers(dev, ws, wo):
     sbs.close()
 
 
+# -------------------------------------------------------------------------------- config 4 (sweep), full size
+_SWEEP_SHARED = {}
+
+
+@pytest.mark.parametrize("ws,wo", workloads.config4_points())
+def test_config4_all_sweep_points_full_size(dev, ws, wo):
+    """Every point of the window sweep at 28 layers x 12 sequences: one step as three API calls and one
+    one-launch step, each with bit-exact integer state and EVERY (sequence, layer, head) of the output
+    compared with the fp64 oracle.  The seeded values are the same at every point (only the windows
+    change), so the generators and the host copy of the bulk append are shared between the points."""
+    cfg = workloads.config4(ws, wo)
+    if "data" not in _SWEEP_SHARED:
+        _SWEEP_SHARED["data"] = [workloads.SeqData(cfg, i, device=dev) for i in range(cfg.batch)]
+        _SWEEP_SHARED["bulk"] = {}
+    sbs = _mk(cfg, dev, use_c_oracle=True, data=_SWEEP_SHARED["data"], bulk_bits=_SWEEP_SHARED["bulk"])
+    ids = list(range(cfg.batch))
+    sbs.bulk_prefill(ids, 1100)
+    sbs.check_integer_state(ids)
+    sbs.append_step(ids)
+    sbs.evict(ids)
+    sbs.check_integer_state(ids)
+    q, out, lse = sbs.attend(ids, want_lse=True)
+    sbs.check_attention(ids, q, out, lse)
+    n0 = sbs.gpu.stats()["kernel_launches"]
+    q, out, lse = sbs.fused_step(ids, want_lse=True)
+    assert sbs.gpu.stats()["kernel_launches"] == n0 + 1
+    sbs.check_integer_state(ids)
+    sbs.check_attention(ids, q, out, lse)
+    want = 64 + min(ws, 2250) + 4 + min(wo, sbs.t_of(0) - 4)
+    assert all(sbs.gpu.seq_state(i)["n_retained"] == want for i in ids)
+    sbs.close()
+
+
 # -------------------------------------------------------------------------------- config 5 (ragged), reduced
 def test_config5_ragged_two_layers_sequences_finish_at_different_steps(dev):
     full = workloads.config5()
@@ -256,8 +290,9 @@ def test_config5_ragged_two_layers_sequences_finish_at_different_steps(dev):
 
 # -------------------------------------------------------------------------------- full-size, sampled
 def _full_size_steps(sbs, ids, n_steps, sample_layers, seq_subset):
-    """Full-size steps in the launch configuration bench.py times: first as three API calls, then the
-    same number of steps through murmur_decode_step (one launch per step)."""
+    """Full-size steps in the launch configuration bench.py times: first as three API calls (sampled
+    items compared), then the same number of steps through murmur_decode_step (one launch per step),
+    of which EVERY (sequence, layer, head) is compared with the fp64 oracle."""
     for _ in range(n_steps):
         sbs.append_step(ids)
         sbs.evict(ids)
@@ -272,10 +307,10 @@ def _full_size_steps(sbs, ids, n_steps, sample_layers, seq_subset):
             assert sbs.gpu.stats()["kernel_launches"] == launches0 + 1, "murmur_decode_step must be ONE launch"
         sbs.check_integer_state(ids)
         assert torch.isfinite(out.float()).all()
-        sbs.check_attention(ids, q, out, lse, layers=sample_layers, seq_subset=seq_subset)
+        sbs.check_attention(ids, q, out, lse)  # full tensor: all sequences, layers and heads
 
 
-def test_config2_full_size_28_layers_sampled(dev):
+def test_config2_full_size_28_layers_full_tensor(dev):
     cfg = workloads.config2()
     sbs = _mk(cfg, dev, use_c_oracle=True)
     ids = list(range(12))
@@ -287,25 +322,25 @@ def test_config2_full_size_28_layers_sampled(dev):
 
 
 @pytest.mark.parametrize("evicted", [False, True])
-def test_config3_full_size_28_layers_sampled(dev, evicted):
+def test_config3_full_size_28_layers_full_tensor(dev, evicted):
     cfg = workloads.config3(evicted)
     sbs = _mk(cfg, dev, use_c_oracle=True)
     sbs.bulk_prefill([0], 1030)  # past d = 1024 and k_o + w_o = 516
     sbs.check_integer_state([0])
-    _full_size_steps(sbs, [0], 2, sample_layers=[0, 27], seq_subset=[0])
+    _full_size_steps(sbs, [0], 3, sample_layers=[0, 27], seq_subset=[0])
     want = (64 + 27000 + sbs.t_of(0)) if not evicted else (64 + 2048 + 4 + 512)
     assert sbs.gpu.seq_state(0)["n_retained"] == want
     sbs.close()
 
 
-def test_config5_full_size_28_layers_sampled(dev):
+def test_config5_full_size_28_layers_full_tensor(dev):
     cfg = workloads.config5()
-    sbs = _mk(cfg, dev, use_c_oracle=True)
+    sbs = _mk(cfg, dev, use_c_oracle=True, extra_tokens=8)
     ids = list(range(32))
     for i in ids:
         sbs.bulk_prefill([i], min(cfg.seqs[i].T - 2, 1200))
     sbs.check_integer_state(ids)
-    _full_size_steps(sbs, ids, 2, sample_layers=[5, 27], seq_subset=[0, 9, 31])
+    _full_size_steps(sbs, ids, 3, sample_layers=[5, 27], seq_subset=[0, 9, 31])
     sbs.close()
 
 
@@ -426,21 +461,27 @@ def test_decode_step_more_than_32_sequences_falls_back(dev):
 
 
 def test_decode_step_back_to_back_without_host_sync(dev):
-    """200 fused steps enqueued back to back (PDL chain prologue -> attention -> prologue ...) with
-    no host synchronisation in between; the final integer state and every step's output are
-    checked afterwards (a missing griddepcontrol.wait would corrupt tables or outputs)."""
+    """200 fused steps enqueued back to back (PDL chain: each launch's set-up overlaps its predecessor)
+    with no host synchronisation in between.  Afterwards the final integer state is checked, and the
+    outputs of eight sampled steps (first, around the window edges t = 256 / 260, middle, last) are
+    compared with the oracle over the retained sets recorded at those steps (a missing
+    griddepcontrol.wait would corrupt tables or outputs)."""
     cfg = workloads.config2().with_layers(2)
     a = _mk(cfg, dev)
     ids = list(range(cfg.batch))
     a.bulk_prefill(ids, 250)
-    outs = []
-    for _ in range(200):
-        outs.append(a.fused_step(ids))
+    sampled = {0, 1, 5, 6, 9, 10, 100, 199}  # steps 5 / 9 are t = 256 (= d) and t = 260 (= k_o + w_o)
+    outs, rets = {}, {}
+    for k in range(200):
+        q, out, lse = a.fused_step(ids, want_lse=True)
+        if k in sampled:
+            outs[k] = (q, out, lse)
+            rets[k] = {i: list(a.oracle.retained(i)) for i in ids}
     torch.cuda.synchronize()
     a.check_integer_state(ids)
-    # replay the oracle for sampled steps: retained sets are positional, so they can be recomputed
-    q, out, _ = outs[-1]
-    a.check_attention(ids, q, out, seq_subset=[0, 5, 11])
+    for k in sorted(sampled):
+        q, out, lse = outs[k]
+        a.check_attention(ids, q, out, lse, retained=rets[k])
     a.close()
 
 
@@ -462,6 +503,116 @@ def test_decode_step_soak_small_pages_many_allocations(dev):
     assert sbs.gpu.last_error() == 0
     sbs.close()
 
+
+
+# -------------------------------------------------------------------------------- per-layer engine mode
+def _ragged16_specs_with_w_out_0():
+    """Ragged page-16 batch; the last sequence has w_out = 0: its newest token is dead as soon as it is
+    appended, so the step that completes a block frees the very block the token was written to."""
+    specs = [seq_spec(8, 70 + 9 * i, 40 + 7 * i, 32 if i % 2 else 48, 16 if i % 3 else 32, n_sink_out=2 + i % 3)
+             for i in range(4)]
+    specs.append(seq_spec(5, 60, 45, 32, 0, n_sink_out=1))
+    return specs
+
+
+def test_per_layer_mode_append_write_only_layers(dev):
+    """The reserve-once / write-per-layer append (murmur_kv_append with layer_begin > 0) as an engine
+    issues it - append(0), evict, attn(0), then append(l), attn(l) for every further layer - on a ragged
+    page-16 batch over more than two pages of tokens: integer state bit-exact after every step, the rows
+    of ALL layers gathered back bit-exact (a row written to the wrong page shows up here), attention of
+    every layer within tolerance.  Includes a w_out = 0 sequence (the evict after layer 0 frees the block
+    the newest token lives in; the later layers' rows for it are dropped, not an error)."""
+    specs = _ragged16_specs_with_w_out_0()
+    cfg = workloads.config5().with_seqs(specs).with_layers(3)
+    a = _mk(cfg, dev)
+    active = list(range(cfg.batch))
+    a.bulk_prefill(active, 1)
+    a.check_integer_state(active)
+    step = 0
+    while active:
+        order = active[::-1] if step % 2 else list(active)
+        q, out, lse = a.per_layer_step(order, want_lse=True)
+        a.check_integer_state(active)
+        a.check_attention(order, q, out, lse)
+        if step % 5 == 0 or any((a.oracle.seqs[i].length % 16) in (0, 1) for i in active):
+            for i in active:
+                a.check_gather(i, layers=None)
+        done = [i for i in active if a.t_of(i) >= cfg.seqs[i].T]
+        for i in done:
+            a.gpu.seq_end(i)
+            a.oracle.seq_end(i)
+        active = [i for i in active if i not in done]
+        step += 1
+    assert step == max(s.T for s in specs) - 1 and step > 2 * 16
+    assert list(a.gpu.free_stack()) == a.oracle.free_stack
+    assert a.gpu.last_error() == 0
+    a.close()
+
+
+@pytest.mark.parametrize("mode", ["one_launch", "two_launches", "three_calls", "per_layer"])
+def test_evict_unmaps_the_block_of_the_newest_token(dev, mode):
+    """w_out = 0 with page 16: at every step whose token completes a block of dead outputs, the same
+    step's eviction frees the block that token was just written to.  Every form of the step must leave
+    identical integer state (the page goes back on the stack in the same step) and attend without it."""
+    from paper_2606_01483_b200 import MURMUR_OPT_FUSE_STEP
+
+    specs = [seq_spec(5, 60, 50, 32, 0, n_sink_out=1), seq_spec(3, 29, 50, 16, 0, n_sink_out=0, delay=4),
+             seq_spec(16, 48, 50, 64, 8, n_sink_out=2)]
+    cfg = Config("unmap", 91, Geometry(n_layers=2), 16, tuple(specs))
+    a = _mk(cfg, dev)
+    if mode == "two_launches":
+        a.gpu.set_option(MURMUR_OPT_FUSE_STEP, 1)
+    ids = [0, 1, 2]
+    a.bulk_prefill(ids, 1)
+    freed_same_step = 0
+    for step in range(48):
+        n_free0 = len(a.oracle.free_stack)
+        if mode in ("one_launch", "two_launches"):
+            q, out, lse = a.fused_step(ids, want_lse=True)
+        elif mode == "per_layer":
+            q, out, lse = a.per_layer_step(ids, want_lse=True)
+        else:
+            a.append_step(ids)
+            a.evict(ids)
+            q, out, lse = a.attend(ids, want_lse=True)
+        a.check_integer_state(ids)
+        a.check_attention(ids, q, out, lse)
+        for i in (0, 1):  # the block of the newest token is gone whenever it was completed by this step
+            st = a.oracle.seqs[i]
+            if st.length % 16 == 0 and (st.length - 1) // 16 not in a.oracle.live_blocks(i):
+                freed_same_step += 1
+        if step % 7 == 0:
+            for i in ids:
+                a.check_gather(i, layers=None)
+        assert len(a.oracle.free_stack) >= n_free0 - 3
+    assert freed_same_step >= 4, "the case this test is named for never happened"
+    assert a.gpu.last_error() == 0
+    a.close()
+
+
+def test_bulk_append_130_sequences_two_layers(dev):
+    """More sequences than one append launch takes (128): the call is split, and with several layers
+    every chunk is issued layer by layer - only the first layer's launch reserves, the others write
+    through the block table.  Rows of both layers gathered back bit-exact; then three decode steps."""
+    specs = [seq_spec(3, 10 + (i % 5), 8, 8, 4, n_sink_out=1) for i in range(130)]
+    cfg = Config("many130", 92, Geometry(n_layers=2), 16, tuple(specs))
+    sbs = _mk(cfg, dev)
+    ids = list(range(130))
+    sbs.bulk_prefill(ids, 2, evict=False)  # ONE call, 130 sequences x (prefill + 2) tokens
+    for i in (0, 1, 63, 127, 128, 129):
+        sbs.check_gather(i, layers=None)
+    sbs.evict(ids)
+    sbs.check_integer_state(ids)
+    for _ in range(3):
+        sbs.append_step(ids)
+        sbs.evict(ids)
+        sbs.check_integer_state(ids)
+        q, out, lse = sbs.attend(ids, want_lse=True)
+        sbs.check_attention(ids, q, out, lse, seq_subset=[0, 31, 32, 127, 128, 129])
+    for i in (0, 64, 128, 129):
+        sbs.check_gather(i, layers=None)
+    assert sbs.gpu.last_error() == 0
+    sbs.close()
 
 # -------------------------------------------------------------------------------- per-layer windows
 def test_decode_attn_windowed_per_layer_groups(dev):
