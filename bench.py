@@ -5,21 +5,30 @@
 
 A *step* is one pass of the whole hot path over one batch of synthetic input:
 ``murmur_decode_step`` = append one token per sequence (all 28 layers) -> evict -> decode attention
-(all 28 layers), ONE kernel launch per step by default (MURMUR_OPT_FUSE_STEP; --fuse 1 / 0 give the
-two- and three-launch forms).  Prints ONE JSON line (rank 0).
+(all 28 layers), ONE kernel launch per step.  Prints ONE JSON line (rank 0).
 
 Timed regions (CUDA events on the stream the kernels are launched on, W >= 3 warm-up steps,
 barrier + synchronize on both sides, max over ranks):
-  A  K consecutive steps, inputs resident in HBM                          -> value, ms_per_step
-  B  K more steps with one event pair around every launch                 -> roofline (the fused
-     step kernel's average launch duration); then <= 100 steps as three separate API calls
-     (append, evict, attention) with one event pair each                  -> per-stage breakdown
+  A  K consecutive steps, inputs resident in HBM                          -> value, ms_per_step, roofline
+  B  K more steps with one event pair around every launch                 -> isolated launch duration;
+     then <= 100 steps as three separate API calls (append, evict, attention), one event pair each
+  P  <= 50 steps issued layer by layer from C (murmur_decode_step_chunked, 28 launches per step)
+                                                                         -> per_layer_mode_us
   C  K_e steps through murmur_decode_step_host from pinned HOST buffers, stream-synchronised
      every step (the caller reads `out`)                                  -> e2e
 Every step re-reads ~575 MB of retained K/V (>> 126 MB L2), so inputs are larger than L2 and no
 explicit flush is needed; t advances every step, so windows slide and pages are freed/reused.
-After the timed regions rank 0 (N = 1) times the fp64 CPU oracle on a bounded sample of the last
-step and compares the GPU output of that step against it (cpu_baseline + parity keys).
+
+Checks against the oracle (rank 0, N = 1; all outside the timed regions; SURVEY.md 8(d) "Protocol"):
+  parity    the outputs the TIMED launches produced - region A's last `out` (murmur_decode_step) and
+            region C's last host `out` (murmur_decode_step_host) - compared with the fp64 oracle for
+            every (sequence, layer, head); integer state of every sequence after region A bit-exact
+  replay    region A re-run on a second cache from the same seeded inputs, integer state compared
+            with the oracle at EVERY step; its last output must equal region A's bit for bit
+  protocol  the whole decode t = 1..T on a third cache; full-tensor attention check at the steps
+            {1, 2, k_o+w_o, k_o+w_o+1, d, d+1, d+2, T/2, T-1, T}, retained sets at those steps
+  cpu_baseline  the same oracle (policy + plain-C fp64 attention) timed on the host cores
+  other_workloads  configs 3a, 3b, 5 and two sweep points: us/step, roofline fraction, clocks, oracle check
 
 Multi-GPU: the path has no exchange step: "replicas only".  Under torchrun every
 rank runs an independent replica of the workload on its own GPU; time = max over ranks.
@@ -30,6 +39,7 @@ attention) on the host cores, each step a bounded sample of the same workload.
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import math
 import os
@@ -45,21 +55,34 @@ METRIC = "decode-attn us/step (whole step: append+evict+attn), 12x300s chunks, e
 UNIT = "us/step"
 BYTES_PER_TOKEN_LAYER = 4 * 128 * 2 * 2  # 4 KV heads x 128 x bf16 x {K, V}
 HBM_FALLBACK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+OTHER_WORKLOADS = ["config3a", "config3b", "config5", "sweep_128_64", "sweep_2250_1024"]
+# sources whose change invalidates an ncu traffic capture of the step kernel (profiles/traffic.md)
+KERNEL_SOURCES = ["decode_attn_mma.cu", "evict_body.cuh", "device_state.cuh", "policy_math.cuh", "ptx_utils.cuh"]
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE attention launch from the committed
-# `ncu --set full` capture (profiles/), keyed by workload; None until a capture exists.
-NCU_TRAFFIC_BYTES = {}
-try:
-    with open(os.path.join(ROOT, "profiles", "traffic.md")) as _f:
-        for _ln in _f:
-            if _ln.startswith("| `") and _ln.count("|") >= 4:
-                _c = [x.strip() for x in _ln.strip().strip("|").split("|")]
-                try:
-                    NCU_TRAFFIC_BYTES[_c[0].strip("`")] = float(_c[1])
-                except ValueError:
-                    pass
-except OSError:
-    pass
+
+def kernel_source_hash() -> str:
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2606_01483_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic_bytes(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the committed
+    `ncu --set full` capture (profiles/traffic.md), or None when there is no capture for this workload or
+    the kernel sources have changed since it was taken (the row carries their hash)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.md")) as f:
+            for ln in f:
+                if not (ln.startswith("| `") and ln.count("|") >= 5):
+                    continue
+                c = [x.strip() for x in ln.strip().strip("|").split("|")]
+                if c[0].strip("`") == workload and c[2].strip("`") == kernel_source_hash():
+                    return float(c[1])
+    except (OSError, ValueError, IndexError):
+        pass
+    return None
 
 
 # ------------------------------------------------------------------------------------------------
@@ -100,7 +123,7 @@ REASON_BITS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_pow
 class ClockSampler:
     def __init__(self, dev_index: int):
         self.path = f"/tmp/murmur_clocks_{os.getpid()}.txt"
-        self.windows = []
+        self.windows = {}
         self.proc = None
         try:
             self.proc = subprocess.Popen([sys.executable, "-c", SAMPLER_SRC, str(dev_index), self.path],
@@ -108,12 +131,13 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
-    def window(self, t0: float, t1: float):
-        self.windows.append((t0, t1))
+    def window(self, t0: float, t1: float, tag: str = "main"):
+        self.windows.setdefault(tag, []).append((t0, t1))
 
     def finish(self) -> dict:
+        """{tag: summary of the samples that fell inside that tag's timed regions}."""
         if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "sampler unavailable"}
+            return {}
         time.sleep(0.02)
         self.proc.terminate()
         try:
@@ -132,17 +156,21 @@ class ClockSampler:
             os.unlink(self.path)
         except OSError:
             pass
-        under = [r for r in rows if any(a <= r[0] <= b for a, b in self.windows)]
-        if not under:
-            return {"sm_mhz": None, "sm_max_mhz": rows[0][2] if rows else None, "reasons": [],
-                    "samples": 0, "note": "no sample fell inside a timed region"}
-        sms = sorted(r[1] for r in under)
-        mask = 0
-        for r in under:
-            mask |= r[3]
-        reasons = [name for bit, name in REASON_BITS.items() if mask & bit and name != "gpu_idle"]
-        return {"sm_mhz": sms[len(sms) // 2], "sm_min_mhz": sms[0], "sm_max_mhz": under[0][2], "reasons": reasons,
-                "samples": len(under), "power_w_max": max(r[4] for r in under), "how": "NVML polled every ~4 ms"}
+        out = {}
+        for tag, wins in self.windows.items():
+            under = [r for r in rows if any(a <= r[0] <= b for a, b in wins)]
+            if not under:
+                out[tag] = {"sm_mhz": None, "sm_max_mhz": rows[0][2] if rows else None, "reasons": [], "samples": 0,
+                            "note": "no sample fell inside a timed region"}
+                continue
+            sms = sorted(r[1] for r in under)
+            mask = 0
+            for r in under:
+                mask |= r[3]
+            reasons = [name for bit, name in REASON_BITS.items() if mask & bit and name != "gpu_idle"]
+            out[tag] = {"sm_mhz": sms[len(sms) // 2], "sm_min_mhz": sms[0], "sm_max_mhz": under[0][2], "reasons": reasons,
+                        "samples": len(under), "power_w_max": max(r[4] for r in under), "how": "NVML polled every ~4 ms"}
+        return out
 
 
 # ------------------------------------------------------------------------------------------------
@@ -180,6 +208,24 @@ def pick_workload(name: str):
     raise SystemExit(f"unknown workload {name}")
 
 
+def config_keys(cfg, world: int = 1) -> dict:
+    """The workload description both arms print under `config` (same keys, same values)."""
+    g = cfg.geom
+    d = {"workload": cfg.name, "batch": cfg.batch, "n_layers": g.n_layers, "n_q_heads": g.n_q_heads,
+         "n_kv_heads": g.n_kv_heads, "head_dim": g.head_dim, "page_size": cfg.page_size,
+         "parallelism": "replicas only" if world > 1 else "single GPU"}
+    s0 = cfg.seqs[0]
+    if len({(x.S, x.w_speech, x.w_out) for x in cfg.seqs}) == 1:
+        d.update({"speech_tokens": s0.S, "prefix_tokens": s0.P, "w_speech": s0.w_speech, "w_out": s0.w_out,
+                  "delay": s0.delay, "n_sink_out": s0.n_sink_out})
+    else:
+        d.update({"ragged": True, "speech_tokens": [min(x.S for x in cfg.seqs), max(x.S for x in cfg.seqs)],
+                  "prefix_tokens": s0.P, "w_speech": sorted({x.w_speech for x in cfg.seqs}),
+                  "w_out": sorted({x.w_out for x in cfg.seqs}), "n_sink_out": s0.n_sink_out,
+                  "note": "all sequences kept active at a common t (the full-batch point of config 5)"})
+    return d
+
+
 def load_peak():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -197,7 +243,6 @@ def run_reference(args):
     if rank != 0:
         return 0
     import numpy as np
-    import torch
 
     import workloads
     from oracle import c as oracle_c
@@ -205,8 +250,6 @@ def run_reference(args):
     from oracle import policy as o_policy
 
     cfg, t0 = pick_workload(args.workload)
-    if t0 is None:
-        t0 = 200
     g = cfg.geom
     co = oracle_c.load()
     K, W = args.steps, args.warmup
@@ -214,7 +257,6 @@ def run_reference(args):
     budget_s = float(args.ref_budget_s)
     # data of sequence 0 only (the sample never leaves it): CPU generator, same recipe
     sd = workloads.SeqData(cfg, 0, device="cpu")
-    spec = cfg.seqs[0]
     kp, vp = sd.prefill_kv()
     ko, vo = sd.out_kv(0, t0 + K + W + 2)
     k_bits = np.concatenate([workloads.to_bits(kp), workloads.to_bits(ko)], axis=1)
@@ -249,15 +291,16 @@ def run_reference(args):
         used = step(n_sample)
     el = time.perf_counter() - t_start
     us_step = el / K * (n_items_step / n_sample) * 1e6
-    sample = (f"per step: integer bookkeeping of all {cfg.batch} sequences + fp64 attention of sequence 0, layers "
-              f"0..{n_sample - 1} (all 28 q heads), scaled x{n_items_step / n_sample:.1f} to the "
-              f"{n_items_step} (sequence, layer) items of a step")
+    sample = (f"per step: Python integer bookkeeping (oracle.paged_cache append + evict) of all {cfg.batch} sequences "
+              f"+ fp64 attention of sequence 0, layers 0..{n_sample - 1} (all 28 q heads); the whole time is scaled "
+              f"x{n_items_step / n_sample:.1f} to the {n_items_step} (sequence, layer) items of a step - so, unlike the CUDA "
+              f"arm's cpu_baseline key (policy + attention only), this value includes the Python bookkeeping")
     line = {
         "impl": "reference", "metric": METRIC, "value": us_step, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
         "warmup": W, "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "batch": cfg.batch, "n_layers": g.n_layers, "page_size": cfg.page_size,
-                   "what": "fp64 CPU oracle (oracle/), bounded sample per step"},
+        "config": config_keys(cfg, int(os.environ.get("WORLD_SIZE", "1"))),
+        "what": "fp64 CPU oracle (oracle/), bounded sample per step",
         "cpu_baseline": {"value": us_step, "unit": UNIT, "cores": int(used), "kind": "oracle", "sample": sample},
         "e2e": {"value": us_step, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -269,12 +312,225 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------------
+class Workbench:
+    """One cache filled by a bulk append to t = t0 plus pre-generated step inputs resident in HBM."""
+
+    def __init__(self, cfg, t0: int, n_steps: int, dev, n_gen_cap: int = 1100):
+        import numpy as np
+        import torch
+
+        import workloads
+        from paper_2606_01483_b200 import MurmurCache
+
+        self.cfg, self.t0, self.dev = cfg, t0, dev
+        g = cfg.geom
+        self.B = cfg.batch
+        self.n_gen = max(1, min(n_steps, n_gen_cap))  # distinct step inputs (re-used cyclically beyond that)
+        Tmin = min(s.T for s in cfg.seqs)
+        extra = max(2, t0 + n_steps + 2 - Tmin)  # a long run decodes past the config's T
+        self.ids = np.arange(self.B, dtype=np.int32)
+        self.n_pages = workloads.unevicted_blocks(cfg, extra) + 2
+        self.max_blocks = workloads.max_blocks_per_seq(cfg, extra) + 1
+        self.cache = MurmurCache(g.n_layers, g.n_q_heads, g.n_kv_heads, g.head_dim, cfg.page_size, self.B,
+                                 self.max_blocks, self.n_pages, device=dev)
+        self.data = [workloads.SeqData(cfg, i, device=dev) for i in range(self.B)]
+        k_steps, v_steps, q_steps = [], [], []
+        for i, s in enumerate(cfg.seqs):
+            self.cache.seq_begin(i, s.P, s.S, s.M, s.policy_tuple)
+            k, v = self._bulk(i)
+            if k.shape[1]:
+                self.cache.kv_append([i], [k.shape[1]], k, v)
+            del k, v
+            ks, vs = self.data[i].out_kv(t0, t0 + self.n_gen)  # [L, steps, kv, d]
+            k_steps.append(ks)
+            v_steps.append(vs)
+            q_steps.append(self.data[i].q_steps(t0 + 1, t0 + self.n_gen + 1))  # [steps, L, n_q, d]
+        self.cache.kv_evict(self.ids)
+        self.k_all = torch.stack(k_steps, dim=2).permute(1, 0, 2, 3, 4).contiguous()  # [steps, L, B, kv, d]
+        self.v_all = torch.stack(v_steps, dim=2).permute(1, 0, 2, 3, 4).contiguous()
+        self.q_all = torch.stack(q_steps, dim=2).contiguous()  # [steps, L, B, n_q, d]
+        self.out = torch.empty_like(self.q_all[0])
+        self.scale = 1.0 / math.sqrt(g.head_dim)
+        self.step_no = 0
+
+    def _bulk(self, i: int):
+        import torch
+
+        kp, vp = self.data[i].prefill_kv()
+        ko, vo = self.data[i].out_kv(0, self.t0)
+        return torch.cat([kp, ko], dim=1).contiguous(), torch.cat([vp, vo], dim=1).contiguous()
+
+    def inputs(self, s: int):
+        j = s % self.n_gen
+        return self.k_all[j], self.v_all[j], self.q_all[j]
+
+    def step(self, out=None, lse=None):
+        k, v, q = self.inputs(self.step_no)
+        self.cache.decode_step(self.ids, k, v, q, self.out if out is None else out, lse, self.scale)
+        self.step_no += 1
+
+    def n_retained(self) -> int:
+        return sum(self.cache.seq_state(i)["n_retained"] for i in range(self.B))
+
+    def host_kv(self, i: int, n_steps_done: int):
+        """uint16 [L, n_pos, kv, d] bit patterns of every row appended to sequence i so far, by position."""
+        import torch
+
+        import workloads
+
+        k, v = self._bulk(i)
+        if n_steps_done:
+            order = torch.arange(n_steps_done, device=self.dev) % self.n_gen
+            k = torch.cat([k, self.k_all[order][:, :, i].permute(1, 0, 2, 3)], dim=1)
+            v = torch.cat([v, self.v_all[order][:, :, i].permute(1, 0, 2, 3)], dim=1)
+        return workloads.to_bits(k), workloads.to_bits(v)
+
+    def close(self):
+        self.cache.close()
+
+
+class Shadow:
+    """The oracle's integer bookkeeping (oracle.paged_cache) advanced beside a Workbench."""
+
+    def __init__(self, wb: Workbench):
+        from oracle import paged_cache as o_cache
+        from oracle import policy as o_policy
+
+        cfg = wb.cfg
+        self.ids = list(range(cfg.batch))
+        self.oc = o_cache.OraclePagedCache(wb.n_pages, cfg.page_size, cfg.batch, wb.max_blocks)
+        for i, s in enumerate(cfg.seqs):
+            self.oc.seq_begin(i, s.P, s.S, s.M, o_policy.Policy(*s.policy_tuple))
+            n = s.P + s.S + s.M + wb.t0
+            if n:
+                self.oc.append([i], [n])  # same call pattern as Workbench: one bulk append per sequence
+        self.oc.evict(self.ids)
+
+    def advance(self, n: int = 1):
+        for _ in range(n):
+            self.oc.append(self.ids, [1] * len(self.ids))
+            self.oc.evict(self.ids)
+
+    def retained(self) -> dict:
+        return {i: list(self.oc.retained(i)) for i in self.ids}
+
+    def check(self, cache) -> None:
+        """Integer state of every sequence, bit-exact: length, t, retained set, compacted page table,
+        run descriptors; the free stack; the device error word; the host mirror of the free count."""
+        import numpy as np
+
+        for i in self.ids:
+            st = cache.seq_state(i)
+            o = self.oc.seqs[i]
+            assert st["length"] == o.length and st["t"] == o.t, (i, st, o.length, o.t)
+            assert np.array_equal(cache.retained(i), np.asarray(self.oc.retained(i), dtype=np.int32)), f"retained set, seq {i}"
+            pages, blocks = cache.page_list(i)
+            assert list(blocks) == self.oc.live_blocks(i), f"live blocks, seq {i}"
+            assert list(pages) == self.oc.live_pages(i), f"live pages, seq {i}"
+            assert cache.runs(i) == self.oc.runs(i), f"runs, seq {i}"
+        assert list(cache.free_stack()) == self.oc.free_stack, "free stack"
+        assert cache.last_error() == 0
+        assert cache.stats()["free_pages"] == len(self.oc.free_stack)
+
+
+def oracle_compare(wb: Workbench, host_kv: dict, q, out, retained: dict, n_threads: int = 0):
+    """out [L, B, n_q, d] (bf16 tensor, device or host) vs Eq. 1 over `retained` in fp64 (plain-C oracle),
+    every (sequence, layer, head).  Returns (parity dict, oracle attention seconds, threads used)."""
+    import numpy as np
+
+    import workloads
+    from oracle import attention as o_attn
+    from oracle import c as oracle_c
+
+    co = oracle_c.load()
+    got = o_attn.bf16_bits_to_f64(workloads.to_bits(out))
+    q_bits = workloads.to_bits(q)
+    mx, sm, n, secs, used = 0.0, 0.0, 0, 0.0, 1
+    assert np.all(np.isfinite(got))
+    for i in range(wb.B):
+        kb, vb = host_kv[i]
+        tc = time.perf_counter()
+        o_ref, _, used = co.attend(q_bits[:, i], kb, vb, retained[i], wb.scale, n_threads=n_threads)
+        secs += time.perf_counter() - tc
+        e = np.abs(got[:, i] - o_ref)
+        mx = max(mx, float(e.max()))
+        sm += float(e.sum())
+        n += e.size
+    return {"max_abs": mx, "mean_abs": sm / n, "tol_max_abs": 2e-2, "tol_mean_abs": 2e-3,
+            "ok": bool(mx <= 2e-2 and sm / n <= 2e-3), "items": f"{wb.B} sequences x {q.shape[0]} layers x {q.shape[2]} heads"}, secs, used
+
+
+def timed_steps(wb: Workbench, K: int, barrier, stream, torch):
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0 = time.time()
+    e0.record(stream)
+    for _ in range(K):
+        wb.step()
+    e1.record(stream)
+    barrier()
+    return e0.elapsed_time(e1) / K * 1e3, (w0, time.time())
+
+
+def spin_up(wb: Workbench, torch, seconds: float = 0.25):
+    """Untimed, state not advanced: repeat attention on the current state until the clocks are up."""
+    t_spin = time.perf_counter()
+    while time.perf_counter() - t_spin < seconds:
+        for _ in range(20):
+            wb.cache.decode_attn(wb.ids, wb.q_all[0], out=wb.out, sm_scale=wb.scale)
+        torch.cuda.synchronize(wb.dev)
+
+
+def alg_bytes_of(cfg, n_ret_total: int) -> int:
+    g = cfg.geom
+    return n_ret_total * BYTES_PER_TOKEN_LAYER * g.n_layers + 2 * g.n_layers * cfg.batch * g.n_q_heads * g.head_dim * 2
+
+
+def run_other_workload(name: str, dev, sampler, peak: float, check: bool, torch) -> dict:
+    """One of the other BASELINE.json configurations: 5 warm-up + 50 timed one-launch steps, roofline
+    fraction, and the oracle check of the last timed output (every sequence, layer, head)."""
+    cfg, t0 = pick_workload(name)
+    K, W = 50, 5
+    wb = Workbench(cfg, t0, W + K + 2, dev)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+
+    spin_up(wb, torch, 0.1)
+    for _ in range(W):
+        wb.step()
+    n0 = wb.n_retained()
+    us, win = timed_steps(wb, K, barrier, stream, torch)
+    if sampler:
+        sampler.window(win[0], win[1], name)
+    n_ret = (n0 + wb.n_retained()) // 2
+    ab = alg_bytes_of(cfg, n_ret)
+    gbs = ab / (us * 1e-6) / 1e9
+    res = {"workload": cfg.name, "us_per_step": us, "steps": K, "retained_tokens_per_seq": n_ret // cfg.batch,
+           "algorithmic_bytes_per_step": ab, "achieved_gbs": gbs, "frac": gbs / peak, "frac_of_nominal_8000": gbs / 8000.0,
+           "tokens_per_s": cfg.batch / (us * 1e-6), "launches_per_step": 1}
+    if check:
+        sh = Shadow(wb)
+        sh.advance(W + K)
+        sh.check(wb.cache)
+        hk = {i: wb.host_kv(i, W + K) for i in range(cfg.batch)}
+        par, _, _ = oracle_compare(wb, hk, wb.inputs(W + K - 1)[2], wb.out, sh.retained())
+        par["compared"] = "output of the LAST TIMED murmur_decode_step launch; integer state of every sequence bit-exact"
+        res["parity"] = par
+        del hk
+    res["device_error_word"] = wb.cache.last_error()
+    wb.close()
+    del wb
+    torch.cuda.empty_cache()
+    return res
+
+
 def run_murmur(args):
     import numpy as np
     import torch
 
-    import workloads
-    from paper_2606_01483_b200 import MurmurCache, binding
+    from paper_2606_01483_b200 import binding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -295,55 +551,14 @@ def run_murmur(args):
     g = cfg.geom
     K, W = args.steps, max(3, args.warmup)
     Ke, We = args.e2e_steps, 3
-    n_steps_total = W + 2 * K + We + Ke + 1 + (56 if args.per_layer else 0)
-    n_gen = min(n_steps_total, 1100)  # distinct pre-generated step inputs (re-used cyclically beyond that)
-    Tmin = min(s.T for s in cfg.seqs)
-    extra = max(2, t0 + n_steps_total + 2 - Tmin)  # a long --steps run decodes past the config's T
+    Kb2, Kp = min(K, 100), min(K, 50)
+    n_steps_total = W + 2 * K + Kb2 + 3 + Kp + We + Ke + 1
     B = cfg.batch
-    ids = np.arange(B, dtype=np.int32)
-
-    cache = MurmurCache(g.n_layers, g.n_q_heads, g.n_kv_heads, g.head_dim, cfg.page_size, B,
-                        workloads.max_blocks_per_seq(cfg, extra) + 1, workloads.unevicted_blocks(cfg, extra) + 2,
-                        device=dev)
-    if args.variant:
-        cache.set_option(binding.MURMUR_OPT_ATTN_VARIANT, {"generic": 1, "mma": 2}[args.variant])
-    if args.grid:
-        cache.set_option(binding.MURMUR_OPT_ATTN_GRID, args.grid)
-    if args.no_pdl:
-        cache.set_option(binding.MURMUR_OPT_PDL, 0)
-    if args.no_fuse:
-        cache.set_option(binding.MURMUR_OPT_FUSE_STEP, 0)
-    elif args.fuse >= 0:
-        cache.set_option(binding.MURMUR_OPT_FUSE_STEP, args.fuse)
-    data = [workloads.SeqData(cfg, i, device=dev) for i in range(B)]
-    k_steps, v_steps, q_steps = [], [], []
-    for i, s in enumerate(cfg.seqs):
-        cache.seq_begin(i, s.P, s.S, s.M, s.policy_tuple)
-        kp, vp = data[i].prefill_kv()
-        ko, vo = data[i].out_kv(0, t0)
-        k = torch.cat([kp, ko], dim=1).contiguous()
-        v = torch.cat([vp, vo], dim=1).contiguous()
-        cache.kv_append([i], [k.shape[1]], k, v)
-        del k, v, kp, vp
-        ks, vs = data[i].out_kv(t0, t0 + n_gen)  # [L, steps, kv, d]
-        k_steps.append(ks)
-        v_steps.append(vs)
-        q_steps.append(data[i].q_steps(t0 + 1, t0 + n_gen + 1))  # [steps, L, n_q, d]
-    cache.kv_evict(ids)
-    k_all = torch.stack(k_steps, dim=2).permute(1, 0, 2, 3, 4).contiguous()  # [steps, L, B, kv, d]
-    v_all = torch.stack(v_steps, dim=2).permute(1, 0, 2, 3, 4).contiguous()
-    q_all = torch.stack(q_steps, dim=2).contiguous()  # [steps, L, B, n_q, d]
-    del k_steps, v_steps, q_steps
-    out = torch.empty_like(q_all[0])
-    scale = 1.0 / math.sqrt(g.head_dim)
+    check = rank == 0 and world == 1 and not args.no_cpu_baseline
+    wb = Workbench(cfg, t0, n_steps_total, dev)
+    cache, ids, scale = wb.cache, wb.ids, wb.scale
     stream = torch.cuda.current_stream()
-    step_no = [0]
-
-    def one_step():
-        s = step_no[0]
-        j = s % n_gen
-        cache.decode_step(ids, k_all[j], v_all[j], q_all[j], out, None, scale)
-        step_no[0] = s + 1
+    peak, peak_src = load_peak()
 
     def barrier():
         if dist is not None:
@@ -351,52 +566,32 @@ def run_murmur(args):
         torch.cuda.synchronize(dev)
 
     sampler = ClockSampler(local_rank) if rank == 0 else None
-
-    # spin the clocks up (untimed, state not advanced): repeat attention on the current state
-    t_spin = time.perf_counter()
-    while time.perf_counter() - t_spin < 0.25:
-        for _ in range(20):
-            cache.decode_attn(ids, q_all[0], out=out, sm_scale=scale)
-        torch.cuda.synchronize(dev)
-
+    spin_up(wb, torch)
     for _ in range(W):
-        one_step()
+        wb.step()
     # ---- region A: K steps, whole-step timing -----------------------------------------------
     cache.reset_stats()
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    w0 = time.time()
-    e0.record(stream)
-    for _ in range(K):
-        one_step()
-    e1.record(stream)
-    barrier()
-    w1 = time.time()
-    ms_a = e0.elapsed_time(e1)
+    n_ret_a0 = wb.n_retained()
+    us_a, win = timed_steps(wb, K, barrier, stream, torch)
     launches = cache.stats()["kernel_launches"]
     if sampler:
-        sampler.window(w0, w1)
+        sampler.window(win[0], win[1])
     st = cache.stats()
-    if args.timeline and rank == 0:  # per-CTA trace of the last attention launch of region A (profiling aid)
-        tl = cache.attn_timeline().astype(np.int64)
-        t_first = int(tl[:, 0].min())
-        tr = cache.step_trace().astype(np.int64)
-        with open(args.timeline, "w") as f:
-            f.write("# step prologue stamps (ns relative to the first attention CTA start): append_start %d ticket %d "
-                    "commit %d evict_start %d evict_end %d | last CTA: wait_done %d state_loaded %d prefix %d loads_issued %d "
-                    "tasks %d pages_consumed %d block %d\n" % (tuple(int(x) - t_first for x in tr[:11]) + (int(tr[11]),)))
-            f.write("# cta start_ns end_ns smid tiles   (ns relative to the first CTA start)\n")
-            for b in range(tl.shape[0]):
-                f.write("%d %d %d %d %d\n" % (b, tl[b, 0] - t_first, tl[b, 1] - t_first if tl[b, 1] else -1,
-                                            tl[b, 2] - t_first if tl[b, 2] > (1 << 20) else tl[b, 2], tl[b, 3]))
+    n_ret_a1 = wb.n_retained()
+    steps_a = wb.step_no  # steps applied to the cache when region A's last output was produced
+    out_a = wb.out.clone()
+    shadow, parity_int = None, None
+    if check:
+        shadow = Shadow(wb)
+        shadow.advance(steps_a)
+        shadow.check(cache)  # integer state of every sequence after the timed region, bit-exact
+        ret_a = shadow.retained()
+        parity_int = f"bit-exact after region A (all {B} sequences: lengths, retained sets, page tables, runs, free stack)"
 
     # ---- region B: K steps with one event pair around every launch --------------------------------
-    # B1: the step as the library runs it by default (murmur_decode_step = ONE launch of the fused
-    #     step kernel) -> duration of the dominant kernel for `roofline`
+    # B1: the step as the library runs it (ONE launch) -> isolated launch duration, no PDL overlap
     # B2: the same step as three separate calls (append, evict, attention) -> per-stage breakdown
-    n_ret_b0 = sum(cache.seq_state(i)["n_retained"] for i in range(B))
     ones = [1] * B
-    Kb2 = min(K, 100)
     evs1 = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(K)]
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(Kb2)]
     barrier()
@@ -404,29 +599,25 @@ def run_murmur(args):
     torch.cuda._sleep(int(1e8))  # ~50 ms of GPU spin so the host runs ahead: event pairs then see kernels, not launch gaps
     cache.reset_stats()
     for j in range(K):
-        s = step_no[0] % n_gen
         evs1[j][0].record(stream)
-        cache.decode_step(ids, k_all[s], v_all[s], q_all[s], out, None, scale)
+        wb.step()
         evs1[j][1].record(stream)
-        step_no[0] += 1
     launches_per_step_b1 = cache.stats()["kernel_launches"] / K
     barrier()
-    n_ret_b1 = sum(cache.seq_state(i)["n_retained"] for i in range(B))
     torch.cuda._sleep(int(1e8))
     for j in range(Kb2):
-        s = step_no[0] % n_gen
+        k, v, q = wb.inputs(wb.step_no)
         evs[j][0].record(stream)
-        cache.kv_append(ids, ones, k_all[s], v_all[s])
+        cache.kv_append(ids, ones, k, v)
         evs[j][1].record(stream)
         cache.kv_evict(ids)
         evs[j][2].record(stream)
-        cache.decode_attn(ids, q_all[s], out=out, sm_scale=scale)
+        cache.decode_attn(ids, q, out=wb.out, sm_scale=scale)
         evs[j][3].record(stream)
-        step_no[0] += 1
+        wb.step_no += 1
     barrier()
-    w1 = time.time()
     if sampler:
-        sampler.window(w0, w1)
+        sampler.window(w0, time.time())
     step_list = sorted(e[0].elapsed_time(e[1]) * 1e3 for e in evs1)
     t_stepk = sum(step_list) / K
     t_stepk_med = step_list[K // 2]
@@ -437,52 +628,45 @@ def run_murmur(args):
     t_att = sum(attn_list) / Kb2
     t_att_med = attn_list[Kb2 // 2]
 
-    # ---- optional region P: the step as a per-layer engine would issue it -------------------------
-    # (layer l's K/V exist only when layer l runs: append(layer l) + attention(layer l), 28 times,
-    # with the eviction right after the first layer's append has reserved the slots)
-    us_per_layer_mode = None
-    if args.per_layer:
-        Kp = min(K, 50)
-        L = g.n_layers
-
-        def layer_step(s_idx):
-            for l in range(L):
-                cache.kv_append(ids, ones, k_all[s_idx][l:l + 1], v_all[s_idx][l:l + 1], layer_begin=l, layer_end=l + 1)
-                if l == 0:
-                    cache.kv_evict(ids)
-                cache.decode_attn(ids, q_all[s_idx][l:l + 1], out=out[l:l + 1], sm_scale=scale, layer_begin=l, layer_end=l + 1)
-
-        for _ in range(3):
-            layer_step(step_no[0] % n_gen)
-            step_no[0] += 1
-        barrier()
-        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        p0.record(stream)
-        for _ in range(Kp):
-            layer_step(step_no[0] % n_gen)
-            step_no[0] += 1
-        p1.record(stream)
-        barrier()
-        us_per_layer_mode = p0.elapsed_time(p1) / Kp * 1e3
+    # ---- region P: the step as a layer-by-layer engine issues it, from C ---------------------------
+    # (layer l's K/V exist only when layer l runs: murmur_decode_step_layers once per layer = 28 launches
+    # per step, issued by murmur_decode_step_chunked(layers_per_launch = 1) without leaving the library)
+    for _ in range(3):
+        k, v, q = wb.inputs(wb.step_no)
+        cache.decode_step_chunked(ids, k, v, q, wb.out, 1, None, scale)
+        wb.step_no += 1
+    barrier()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    cache.reset_stats()
+    p0.record(stream)
+    for _ in range(Kp):
+        k, v, q = wb.inputs(wb.step_no)
+        cache.decode_step_chunked(ids, k, v, q, wb.out, 1, None, scale)
+        wb.step_no += 1
+    p1.record(stream)
+    barrier()
+    us_per_layer_mode = p0.elapsed_time(p1) / Kp * 1e3
+    per_layer_launches = cache.stats()["kernel_launches"] / Kp
 
     # ---- region C: end to end from pinned host buffers -------------------------------------------
-    s0 = step_no[0]
-    sel = torch.arange(s0, s0 + We + Ke, device=dev) % n_gen
-    # per step: k_new | v_new | q packed back to back in one pinned block (moved with ONE host-to-device copy)
-    kv_n, q_n = k_all[0].numel(), q_all[0].numel()
+    s0 = wb.step_no
+    sel = torch.arange(s0, s0 + We + Ke, device=dev) % wb.n_gen
+    # per step: k_new | v_new | q packed back to back in one pinned block
+    kv_n, q_n = wb.k_all[0].numel(), wb.q_all[0].numel()
     hb = torch.empty((We + Ke, 2 * kv_n + q_n), dtype=torch.bfloat16).pin_memory()
-    hb[:, :kv_n] = k_all[sel].reshape(We + Ke, -1).cpu()
-    hb[:, kv_n:2 * kv_n] = v_all[sel].reshape(We + Ke, -1).cpu()
-    hb[:, 2 * kv_n:] = q_all[sel].reshape(We + Ke, -1).cpu()
-    kh = [hb[j, :kv_n].view(k_all[0].shape) for j in range(We + Ke)]
-    vh = [hb[j, kv_n:2 * kv_n].view(v_all[0].shape) for j in range(We + Ke)]
-    qh = [hb[j, 2 * kv_n:].view(q_all[0].shape) for j in range(We + Ke)]
-    oh = torch.empty(out.shape, dtype=torch.bfloat16).pin_memory()
+    hb[:, :kv_n] = wb.k_all[sel].reshape(We + Ke, -1).cpu()
+    hb[:, kv_n:2 * kv_n] = wb.v_all[sel].reshape(We + Ke, -1).cpu()
+    hb[:, 2 * kv_n:] = wb.q_all[sel].reshape(We + Ke, -1).cpu()
+    kh = [hb[j, :kv_n].view(wb.k_all[0].shape) for j in range(We + Ke)]
+    vh = [hb[j, kv_n:2 * kv_n].view(wb.v_all[0].shape) for j in range(We + Ke)]
+    qh = [hb[j, 2 * kv_n:].view(wb.q_all[0].shape) for j in range(We + Ke)]
+    oh = torch.empty(wb.out.shape, dtype=torch.bfloat16).pin_memory()
     for j in range(We):
         cache.decode_step_host(ids, kh[j], vh[j], qh[j], oh, scale)
         torch.cuda.synchronize(dev)
     barrier()
     c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    cache.reset_stats()
     w0 = time.time()
     c0.record(stream)
     for j in range(We, We + Ke):
@@ -493,61 +677,117 @@ def run_murmur(args):
     w1 = time.time()
     if sampler:
         sampler.window(w0, w1)
+    e2e_launches = cache.stats()["kernel_launches"] / Ke
     us_e2e_dev = c0.elapsed_time(c1) / Ke * 1e3
     us_e2e_wall = (w1 - w0) / Ke * 1e6
     us_e2e = max(us_e2e_dev, us_e2e_wall)
-    step_no[0] = s0 + We + Ke
+    wb.step_no = s0 + We + Ke
+    steps_c = wb.step_no
     h2d = (kh[0].numel() + vh[0].numel() + qh[0].numel()) * 2
     d2h = oh.numel() * 2
-    clocks = sampler.finish() if sampler else None
 
     # ---- reduce over ranks ---------------------------------------------------------------------
-    us_step = ms_a / K * 1e3
-    us_step, us_e2e, t_att, t_app, t_evi, t_att_med, t_stepk, t_stepk_med = max_over_ranks(
-        [us_step, us_e2e, t_att, t_app, t_evi, t_att_med, t_stepk, t_stepk_med], dist, dev)
+    us_step, us_e2e, t_att, t_app, t_evi, t_att_med, t_stepk, t_stepk_med, us_per_layer_mode = max_over_ranks(
+        [us_a, us_e2e, t_att, t_app, t_evi, t_att_med, t_stepk, t_stepk_med, us_per_layer_mode], dist, dev)
 
-    # ---- algorithmic bytes of one attention launch ------------------------------
-    # retained tokens per launch: the device's own |A(t)|, mean of the first and last step of region B
-    n_ret = (n_ret_b0 + n_ret_b1) // 2
+    # ---- algorithmic bytes of one step launch -----------------------------------
+    n_ret = (n_ret_a0 + n_ret_a1) // 2  # the device's own |A(t)|, mean over region A
+    alg_bytes = alg_bytes_of(cfg, n_ret)
     kv_bytes = n_ret * BYTES_PER_TOKEN_LAYER * g.n_layers
-    qo_bytes = 2 * g.n_layers * B * g.n_q_heads * g.head_dim * 2
-    alg_bytes = kv_bytes + qo_bytes
-    peak, peak_src = load_peak()
-    # dominant kernel of the timed step: the fused step kernel when the step is one launch, else the
-    # attention kernel of the multi-launch step
     one_launch = launches_per_step_b1 < 1.5
     if one_launch:
-        # region A is K back-to-back launches of this one kernel: its average launch duration over the
-        # timed region is region A's time / K (consecutive launches overlap their set-up through PDL);
-        # the event-pair-per-launch figure of region B1 (no overlap, includes the launch gap) is kept beside it
+        # region A is K back-to-back launches of this one kernel: its average launch duration over the timed
+        # region is region A's time / K (consecutive launches overlap their set-up through programmatic
+        # dependent launch = the steady state of a decode loop); the event-pair-per-launch figure of region
+        # B1 (no overlap, includes the launch gap) is kept beside it as isolated_launch_us
         dom_kernel, dom_us, dom_med = "attn_mma_kernel<step> (append + evict + attention, one launch)", us_step, t_stepk_med
     else:
         dom_kernel = "attn_mma_kernel" if st["attn_variant"] == 2 else "attn_generic_kernel"
         dom_us, dom_med = t_att, t_att_med
     achieved = alg_bytes / (dom_us * 1e-6) / 1e9
     attn_only = alg_bytes / (t_att * 1e-6) / 1e9
-    traffic = NCU_TRAFFIC_BYTES.get(cfg.name)
     roofline = {"bound": "hbm", "kernel": dom_kernel,
-                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": ncu_traffic_bytes(cfg.name), "kernel_source_hash": kernel_source_hash(),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                 "avg_launch_us": dom_us, "median_launch_us": dom_med, "isolated_launch_us": t_stepk if one_launch else t_att,
-                "how": ("region A time / K launches (one launch per step, CUDA events around the K steps)" if one_launch
+                "how": ("steady state: region A time / K launches (one launch per step, CUDA events around the K "
+                        "steps; consecutive launches overlap their set-up)" if one_launch
                         else "mean of per-launch CUDA event pairs (region B2)"),
                 "frac_of_nominal_8000": achieved / 8000.0}
 
-    # ---- CPU oracle on a bounded sample of the last step + parity of that step -----------------
-    cpu_baseline, parity = None, None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        # K/V of sequence 0 exactly as appended: prefill + first t0 outputs, then the step inputs in order
-        kp, vp = data[0].prefill_kv()
-        ko, vo = data[0].out_kv(0, t0)
-        order = torch.arange(step_no[0], device=dev) % n_gen
-        k_seq0 = torch.cat([kp, ko, k_all[order][:, :, 0].permute(1, 0, 2, 3)], dim=1)  # [L, n_pos, kv, d]
-        v_seq0 = torch.cat([vp, vo, v_all[order][:, :, 0].permute(1, 0, 2, 3)], dim=1)
-        cpu_baseline, parity = oracle_sample(cfg, cache, k_seq0, v_seq0, ids, q_all[(step_no[0] - 1) % n_gen], scale,
-                                             t0 + step_no[0], dev, float(args.cpu_budget_s))
-    err = cache.last_error()
-    cache.close()
+    # ---- oracle: parity of the timed outputs, CPU baseline, replay, protocol, other workloads -----
+    cpu_baseline = parity = replay = protocol = others = None
+    if check:
+        import workloads
+        from oracle import c as oracle_c
+        from oracle import policy as o_policy
+
+        shadow.advance(steps_c - steps_a)
+        ret_c = shadow.retained()
+        hk = {i: wb.host_kv(i, steps_c) for i in range(B)}
+        # region A's last output (the timed murmur_decode_step launches) and region C's (murmur_decode_step_host)
+        q_a = wb.inputs(steps_a - 1)[2]
+        best = None
+        for _ in range(2):
+            par_a, secs, used = oracle_compare(wb, hk, q_a, out_a, ret_a)
+            best = secs if best is None else min(best, secs)
+        par_c, _, _ = oracle_compare(wb, hk, wb.inputs(steps_c - 1)[2], oh, ret_c)
+        parity = {"compared": "murmur_decode_step: output of the LAST TIMED launch of region A; murmur_decode_step_host: "
+                              "host output of the last timed step of region C; every (sequence, layer, head), fp64 oracle",
+                  "decode_step": par_a, "decode_step_host": par_c, "integer_state": parity_int,
+                  "ok": bool(par_a["ok"] and par_c["ok"])}
+        # CPU baseline: the oracle's work for the same step = retained sets (oracle.policy) + plain-C attention
+        s0_ = cfg.seqs[0]
+        tp = time.perf_counter()
+        for s in cfg.seqs:
+            o_policy.retained_positions(s.P, s.S, s.M, t0 + steps_a, o_policy.Policy(*s.policy_tuple))
+        t_policy = time.perf_counter() - tp
+        co = oracle_c.load()
+        import workloads as _w
+        qb0 = _w.to_bits(q_a[:, 0])
+        n_l1 = max(1, min(g.n_layers, 4))
+        t1 = time.perf_counter()
+        co.attend(qb0[:n_l1], hk[0][0][:n_l1], hk[0][1][:n_l1], ret_a[0], scale, n_threads=1)
+        us_1t = ((time.perf_counter() - t1) / n_l1 * g.n_layers * B + t_policy) * 1e6
+        cpu_baseline = {"value": (best + t_policy) * 1e6, "unit": UNIT, "cores": int(used), "kind": "oracle",
+                        "single_thread_value": us_1t,
+                        "sample": f"the WHOLE last step of region A (t={t0 + steps_a}): oracle.policy retained sets + plain-C "
+                                  f"fp64 attention (oracle/c) of all {B} sequences x {g.n_layers} layers x {g.n_q_heads} heads, "
+                                  f"best of 2, not scaled; single_thread_value = sequence 0, layers 0..{n_l1 - 1} on one thread, "
+                                  f"scaled; host cores = {os.cpu_count()}"}
+        del hk
+        wb_err = cache.last_error()
+        wb.close()
+        torch.cuda.empty_cache()
+
+        # replay of region A on a second cache: integer state at EVERY step, final output bit-identical
+        wb2 = Workbench(cfg, t0, steps_a + 1, dev)
+        sh2 = Shadow(wb2)
+        for _ in range(steps_a):
+            wb2.step()
+            sh2.advance(1)
+            sh2.check(wb2.cache)
+        torch.cuda.synchronize(dev)
+        replay = {"steps": steps_a, "integer_state": "bit-exact vs oracle.paged_cache at every step (warm-up + region A)",
+                  "last_output_bit_identical_to_region_A": bool(torch.equal(wb2.out, out_a))}
+        wb2.close()
+        del wb2
+        torch.cuda.empty_cache()
+
+        if not args.no_protocol:
+            protocol = run_protocol(cfg, dev, torch)
+        if cfg.name == "chunked_12x300s" and not args.no_others:
+            others = {}
+            for name in OTHER_WORKLOADS:
+                others[name] = run_other_workload(name, dev, sampler, peak, True, torch)
+    else:
+        wb_err = cache.last_error()
+        wb.close()
+    clocks_all = sampler.finish() if sampler else {}
+    if others:
+        for name in others:
+            others[name]["clocks"] = clocks_all.get(name)
     if dist is not None:
         dist.destroy_process_group()
     if rank != 0:
@@ -556,19 +796,8 @@ def run_murmur(args):
         "metric": METRIC, "value": us_step, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": dict({"workload": cfg.name, "batch": B, "n_layers": g.n_layers, "n_q_heads": g.n_q_heads,
-                        "n_kv_heads": g.n_kv_heads, "head_dim": g.head_dim, "page_size": cfg.page_size,
-                        "retained_tokens_per_seq": n_ret // B, "t_first_timed": t0 + W + 1,
-                        "l2": "inputs larger than L2 (each step re-reads %.0f MB of K/V)" % (kv_bytes / 1e6),
-                        "parallelism": "replicas only" if world > 1 else "single GPU"},
-                       **({"speech_tokens": cfg.seqs[0].S, "prefix_tokens": cfg.seqs[0].P,
-                           "w_speech": cfg.seqs[0].w_speech, "w_out": cfg.seqs[0].w_out, "delay": cfg.seqs[0].delay,
-                           "n_sink_out": cfg.seqs[0].n_sink_out}
-                          if len({(x.S, x.w_speech, x.w_out) for x in cfg.seqs}) == 1 else
-                          {"ragged": True, "speech_tokens": [min(x.S for x in cfg.seqs), max(x.S for x in cfg.seqs)],
-                           "prefix_tokens": cfg.seqs[0].P, "w_speech": sorted({x.w_speech for x in cfg.seqs}),
-                           "w_out": sorted({x.w_out for x in cfg.seqs}), "n_sink_out": cfg.seqs[0].n_sink_out,
-                           "note": "all sequences kept active at a common t (the full-batch point of config 5)"})),
+        "config": dict(config_keys(cfg, world), retained_tokens_per_seq=n_ret // B, t_first_timed=t0 + W + 1,
+                       l2="inputs larger than L2 (each step re-reads %.0f MB of K/V)" % (kv_bytes / 1e6)),
         "tokens_per_s": whole_job_tokens_per_s(world, B, us_step),
         "step_kernel_us": t_stepk, "step_kernel_us_p10_p50_p90": [stepk_p10, t_stepk_med, stepk_p90],
         "launches_per_step": launches_per_step_b1,
@@ -576,16 +805,18 @@ def run_murmur(args):
                            "attn_hbm_gbs": attn_only, "attn_pct_of_measured_peak": 100.0 * attn_only / peak,
                            "note": "the same step as three API calls, one event pair per call (includes launch gaps)"},
         "per_layer_mode_us": us_per_layer_mode,
-        "attn_us": t_att, "append_us": t_app, "evict_us": t_evi,
-        "attn_hbm_gbs": attn_only, "attn_pct_of_measured_peak": 100.0 * attn_only / peak,
+        "per_layer_mode": {"us_per_step": us_per_layer_mode, "launches_per_step": per_layer_launches, "steps": Kp,
+                           "api": "murmur_decode_step_chunked(layers_per_launch=1): murmur_decode_step_layers once per layer, "
+                                  "issued from C (append-write + attention of layer l in ONE launch; the layer-0 launch "
+                                  "also reserves, commits and evicts)"},
         "step_hbm_gbs": alg_bytes / (us_step * 1e-6) / 1e9,
-        "roofline": roofline, "cpu_baseline": cpu_baseline, "parity_last_step": parity,
+        "roofline": roofline, "cpu_baseline": cpu_baseline, "parity": parity, "parity_last_step": parity,
+        "replay": replay, "protocol": protocol, "other_workloads": others,
         "e2e": {"value": us_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "device_us": us_e2e_dev, "wall_us": us_e2e_wall, "steps": Ke,
-                "api": "murmur_decode_step_host (pinned host k_new | v_new | q packed in one block -> one H2D copy, one launch, "
-                       "one D2H copy of out), stream-synchronised per step"},
+                "device_us": us_e2e_dev, "wall_us": us_e2e_wall, "steps": Ke, "launches_per_step": e2e_launches,
+                "api": "murmur_decode_step_host (pinned host k_new | v_new | q -> out), stream-synchronised per step"},
         "gpu_launches": int(launches), "attn_grid": st["attn_grid"], "attn_smem_bytes": st["attn_smem_bytes"],
-        "device_error_word": err, "clocks": clocks,
+        "device_error_word": wb_err, "clocks": clocks_all.get("main"),
         "paper_context": "paper reports end-to-end only: 88.43 s (chunked + speech eviction) vs 370.73 s single pass, "
                          "1x H100 80GB, batch 16, AMI-IHM (PAPER.md:201-206)",
     }
@@ -593,58 +824,52 @@ def run_murmur(args):
     return 0
 
 
-def oracle_sample(cfg, cache, k_seq0, v_seq0, ids, q_last, scale, t_now, dev, budget_s):
-    """Times oracle (policy + plain-C fp64 attention) on sequence 0 of the last step, as many layers
-    as fit the budget, and compares the GPU output of the same step with it."""
+def run_protocol(cfg, dev, torch) -> dict:
+    """SURVEY.md 8(d) "Protocol": the whole decode t = 1 .. T through one-launch steps; at the steps
+    {1, 2, k_o+w_o, k_o+w_o+1, d, d+1, d+2, T/2, T-1, T} the retained sets are compared with oracle.policy
+    and the output of EVERY (sequence, layer, head) with the fp64 oracle."""
     import numpy as np
-    import torch
 
-    import workloads
-    from oracle import attention as o_attn
-    from oracle import c as oracle_c
     from oracle import policy as o_policy
 
-    g = cfg.geom
-    co = oracle_c.load()
-    spec = cfg.seqs[0]
-    out = cache.decode_attn(ids, q_last, sm_scale=scale)  # recompute the last step's output (state unchanged)
+    s0 = cfg.seqs[0]
+    T = min(s.T for s in cfg.seqs)
+    marks = sorted({x for x in (1, 2, s0.n_sink_out + s0.w_out, s0.n_sink_out + s0.w_out + 1, s0.delay, s0.delay + 1,
+                                s0.delay + 2, T // 2, T - 1, T) if 1 <= x <= T})
+    wb = Workbench(cfg, 0, T, dev, n_gen_cap=T)
+    saved = {}
+    t_run = time.perf_counter()
+    for t in range(1, T + 1):
+        if t in marks:
+            out = torch.empty_like(wb.out)
+            wb.step(out=out)
+            ret = {}
+            for i, s in enumerate(cfg.seqs):
+                want = [x for x in o_policy.retained_positions(s.P, s.S, s.M, t, o_policy.Policy(*s.policy_tuple))
+                        if x < s.P + s.S + s.M + t]
+                assert np.array_equal(wb.cache.retained(i), np.asarray(want, dtype=np.int32)), f"retained set, seq {i}, t={t}"
+                assert wb.cache.seq_state(i)["t"] == t
+                ret[i] = want
+            saved[t] = (out, ret)
+        else:
+            wb.step()
     torch.cuda.synchronize(dev)
-    got = o_attn.bf16_bits_to_f64(workloads.to_bits(out[:, 0]))  # [L, n_q, d]
-    k_bits = workloads.to_bits(k_seq0)
-    v_bits = workloads.to_bits(v_seq0)
-    assert k_bits.shape[1] == spec.P + spec.S + spec.M + t_now
-    q_bits = workloads.to_bits(q_last[:, 0])
-    t_or = time.perf_counter()
-    ret = o_policy.retained_positions(spec.P, spec.S, spec.M, t_now, o_policy.Policy(*spec.policy_tuple))
-    t_policy = time.perf_counter() - t_or
-    assert list(cache.retained(0)) == list(ret), "retained set differs from the oracle"
-    # calibrate on one layer, then as many layers as fit the budget
-    tc = time.perf_counter()
-    o1, _, used = co.attend(q_bits[:1], k_bits[:1], v_bits[:1], ret, scale)
-    per_layer = max(time.perf_counter() - tc, 1e-5)
-    n_l = int(max(1, min(g.n_layers, budget_s / per_layer)))
-    best = None
-    for _ in range(2 if per_layer * n_l < budget_s / 2 else 1):
-        tc = time.perf_counter()
-        o_ref, _, used = co.attend(q_bits[:n_l], k_bits[:n_l], v_bits[:n_l], ret, scale)
-        el = time.perf_counter() - tc
-        best = el if best is None else min(best, el)
-    n_items = cfg.batch * g.n_layers
-    us_step = (best / n_l * n_items + t_policy * cfg.batch) * 1e6
-    # the same oracle on ONE thread (SURVEY.md 8(d)), on a slice small enough for ~2 s
-    n_l1 = int(max(1, min(n_l, 2.0 / max(per_layer * used, 1e-5))))
-    tc = time.perf_counter()
-    co.attend(q_bits[:n_l1], k_bits[:n_l1], v_bits[:n_l1], ret, scale, n_threads=1)
-    us_step_1t = ((time.perf_counter() - tc) / n_l1 * n_items + t_policy * cfg.batch) * 1e6
-    e = np.abs(got[:n_l] - o_ref)
-    parity = {"max_abs": float(e.max()), "mean_abs": float(e.mean()), "tol_max_abs": 2e-2, "tol_mean_abs": 2e-3,
-              "compared": f"sequence 0, layers 0..{n_l - 1}, all {g.n_q_heads} heads of the last step (t={t_now}); "
-                          "retained set bit-exact"}
-    cpu = {"value": us_step, "unit": UNIT, "cores": int(used), "kind": "oracle", "single_thread_value": us_step_1t,
-           "sample": f"oracle.policy retained set + plain-C fp64 attention (oracle/c) of sequence 0, layers 0..{n_l - 1} of "
-                     f"the last step ({len(ret)} retained tokens), best of runs, scaled x{n_items / n_l:.1f} to the "
-                     f"{n_items} (sequence, layer) items of a step; host cores = {os.cpu_count()}"}
-    return cpu, parity
+    gpu_s = time.perf_counter() - t_run
+    assert wb.cache.last_error() == 0
+    hk = {i: wb.host_kv(i, T) for i in range(cfg.batch)}
+    worst_max, worst_mean, ok = 0.0, 0.0, True
+    for t in marks:
+        out, ret = saved[t]
+        par, _, _ = oracle_compare(wb, hk, wb.inputs(t - 1)[2], out, ret)
+        worst_max, worst_mean, ok = max(worst_max, par["max_abs"]), max(worst_mean, par["mean_abs"]), ok and par["ok"]
+    wb.close()
+    del hk
+    torch.cuda.empty_cache()
+    return {"decode_steps": T, "checked_steps_t": marks, "full_tensor_steps": len(marks),
+            "retained_sets": "bit-exact vs oracle.policy at every checked step",
+            "attention": {"max_abs": worst_max, "mean_abs": worst_mean, "tol_max_abs": 2e-2, "tol_mean_abs": 2e-3, "ok": ok,
+                          "items": f"{cfg.batch} sequences x {cfg.geom.n_layers} layers x {cfg.geom.n_q_heads} heads per step"},
+            "wall_s_gpu_loop": gpu_s}
 
 
 def main():
@@ -655,16 +880,10 @@ def main():
     ap.add_argument("--impl", default="murmur", choices=["murmur", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--e2e-steps", type=int, default=100)
-    ap.add_argument("--variant", default="", choices=["", "generic", "mma"])
-    ap.add_argument("--grid", type=int, default=0)
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--per-layer", action="store_true",
-                    help="also time the step issued layer by layer (append(l) + attention(l) x 28, 57 launches)")
-    ap.add_argument("--no-pdl", action="store_true", help="A/B: launch the step's kernels without programmatic dependent launch")
-    ap.add_argument("--fuse", type=int, default=-1, help="A/B: MURMUR_OPT_FUSE_STEP value (2 = one launch per step, default)")
-    ap.add_argument("--no-fuse", action="store_true", help="A/B: murmur_decode_step as three launches (append, evict, attention)")
-    ap.add_argument("--timeline", default="", help="write the per-CTA trace of one attention launch to this file")
-    ap.add_argument("--cpu-budget-s", default="12")
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip every oracle leg (parity, cpu_baseline, replay, protocol, others)")
+    ap.add_argument("--no-protocol", action="store_true", help="skip the whole-decode protocol pass")
+    ap.add_argument("--no-others", action="store_true", help="skip the other_workloads block")
+    ap.add_argument("--cpu-budget-s", default="12", help="(kept for old command lines; the baseline now times one whole step)")
     ap.add_argument("--ref-budget-s", default="120")
     args = ap.parse_args()
     if args.impl == "reference":

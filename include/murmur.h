@@ -119,6 +119,10 @@ typedef struct {
                                      else falls back to 1);
                                      1 = two launches (append with the eviction fused in, then attention);
                                      0 = three launches (append, evict, attention) */
+#define MURMUR_OPT_PREFILL_VARIANT 5 /* value: MURMUR_PREFILL_AUTO / _MMA_SYNC / _UMMA */
+#define MURMUR_PREFILL_AUTO 0     /* = MURMUR_PREFILL_UMMA */
+#define MURMUR_PREFILL_MMA_SYNC 1 /* warp-level mma.sync kernel (the round-1 path, kept as a cross-check) */
+#define MURMUR_PREFILL_UMMA 2     /* tcgen05.mma, accumulators in tensor memory, TMA-fed operands */
 #define MURMUR_ATTN_AUTO 0    /* tensor-core split-K kernel when page_size >= 16, else generic */
 #define MURMUR_ATTN_GENERIC 1 /* one CTA per (layer, sequence, KV head), FFMA, no smem staging */
 #define MURMUR_ATTN_MMA 2     /* persistent split-K kernel: bulk-copy staging + mma.sync bf16 */
@@ -197,6 +201,29 @@ MURMUR_API murmur_status_t murmur_decode_step(murmur_cache_t* cache, const int32
                                               const void* k_new, const void* v_new, const void* q, void* out,
                                               float* lse, float sm_scale, void* stream);
 
+/* The decode step of an engine that produces layer l's K/V only when layer l runs (cache
+ * management must not eat the gain): the same step restricted to the layers [layer_begin, layer_end), ONE launch
+ * per call.  The call with layer_begin == 0 OPENS the step - it reserves the new token's slot in every listed
+ * sequence, advances the lengths and runs the eviction - and must come first; calls with layer_begin > 0 only
+ * write their layers' rows and attend (MURMUR_ERR_STATE unless the step is open for every listed sequence;
+ * rows of a token the open step's eviction already freed are dropped).  Layer ranges may be issued in any
+ * order and size after the opening one; murmur_decode_step == one call with [0, n_layers).
+ *   k_new, v_new : DEVICE bf16 [layer_end-layer_begin][n_seqs][n_kv_heads][head_dim]
+ *   q, out       : DEVICE bf16 [layer_end-layer_begin][n_seqs][n_q_heads][head_dim];  lse likewise or NULL */
+MURMUR_API murmur_status_t murmur_decode_step_layers(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                                     const void* k_new, const void* v_new, const void* q, void* out,
+                                                     float* lse, int32_t layer_begin, int32_t layer_end,
+                                                     float sm_scale, void* stream);
+
+/* The whole step issued from C as ceil(n_layers / layers_per_launch) launches of murmur_decode_step_layers, in
+ * layer order (buffers as for murmur_decode_step).  layers_per_launch = 1 is the launch pattern of a
+ * layer-by-layer engine (what bench.py reports as per_layer_mode_us); the host-buffer entry uses larger chunks
+ * to overlap its copies with the kernels.  layers_per_launch >= n_layers == murmur_decode_step. */
+MURMUR_API murmur_status_t murmur_decode_step_chunked(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                                      const void* k_new, const void* v_new, const void* q, void* out,
+                                                      float* lse, int32_t layers_per_launch, float sm_scale,
+                                                      void* stream);
+
 /* One whole decode step from HOST buffers (the end-to-end entry): copies k_new, v_new, q
  * (HOST, pinned or pageable, layouts as above with 1 token per sequence and all layers) to
  * device staging, runs append -> evict -> decode_attn, copies out (HOST bf16
@@ -226,7 +253,9 @@ MURMUR_API murmur_status_t murmur_chunk_plan(const float* seg_start, const float
  * murmur_kv_append of the chunk and before the first murmur_kv_evict.
  *   q, out : DEVICE bf16 [layer_end-layer_begin][pos_end-pos_begin][n_q_heads][head_dim]
  *   lse    : DEVICE fp32 [layer_end-layer_begin][pos_end-pos_begin][n_q_heads] or NULL
- * page_size >= 16.  First correct path: mma.sync tensor cores (not yet tcgen05). */
+ * page_size >= 16; q and out 16-byte aligned.  Runs on the 5th-generation tensor cores (tcgen05.mma, accumulators in
+ * tensor memory, operands staged by TMA straight from the paged pools); MURMUR_OPT_PREFILL_VARIANT selects the
+ * warp-level mma.sync kernel instead. */
 MURMUR_API murmur_status_t murmur_prefill_attn(murmur_cache_t* cache, int32_t seq, int32_t pos_begin, int32_t pos_end,
                                                const void* q, void* out, float* lse, int32_t layer_begin,
                                                int32_t layer_end, float sm_scale, void* stream);

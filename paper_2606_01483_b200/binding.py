@@ -21,6 +21,8 @@ MURMUR_OPT_ATTN_VARIANT = 1
 MURMUR_OPT_ATTN_GRID = 2
 MURMUR_OPT_PDL = 3
 MURMUR_OPT_FUSE_STEP = 4
+MURMUR_OPT_PREFILL_VARIANT = 5
+MURMUR_PREFILL_AUTO, MURMUR_PREFILL_MMA_SYNC, MURMUR_PREFILL_UMMA = 0, 1, 2
 MURMUR_ATTN_AUTO, MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA = 0, 1, 2
 
 STATUS_NAMES = {0: "MURMUR_OK", 1: "MURMUR_ERR_INVALID_ARG", 2: "MURMUR_ERR_STATE", 3: "MURMUR_ERR_OOM_PAGES",
@@ -30,7 +32,7 @@ STATUS_NAMES = {0: "MURMUR_OK", 1: "MURMUR_ERR_INVALID_ARG", 2: "MURMUR_ERR_STAT
 EXPORTED_SYMBOLS = [
     "murmur_pool_bytes", "murmur_workspace_bytes", "murmur_cache_create", "murmur_cache_destroy",
     "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
-    "murmur_decode_step", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
+    "murmur_decode_step", "murmur_decode_step_layers", "murmur_decode_step_chunked", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
     "murmur_profile_scratch_bytes", "murmur_attn_profile",
     "murmur_decode_attn_windowed", "murmur_prefill_attn", "murmur_chunk_plan",
@@ -88,6 +90,8 @@ def lib() -> C.CDLL:
     L.murmur_kv_evict.argtypes = [vp, vp, i32, vp]
     L.murmur_decode_attn.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, C.c_float, vp]
     L.murmur_decode_step.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, C.c_float, vp]
+    L.murmur_decode_step_layers.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, i32, i32, C.c_float, vp]
+    L.murmur_decode_step_chunked.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, i32, C.c_float, vp]
     L.murmur_decode_step_host.argtypes = [vp, vp, i32, vp, vp, vp, vp, C.c_float, vp]
     L.murmur_seq_get_state.argtypes = [vp, i32, vp, vp]
     L.murmur_kv_get_retained.argtypes = [vp, i32, vp, i32, vp, vp]
@@ -274,6 +278,27 @@ class MurmurCache:
                                               q.data_ptr(), out.data_ptr(),
                                               lse.data_ptr() if lse is not None else None, C.c_float(sm_scale),
                                               _stream()))
+
+    def decode_step_layers(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor, out: torch.Tensor,
+                           layer_begin: int, layer_end: int, lse: Optional[torch.Tensor] = None,
+                           sm_scale: Optional[float] = None):
+        """The decode step restricted to layers [layer_begin, layer_end), one launch; layer_begin == 0 opens the step."""
+        ids = seq_ids if isinstance(seq_ids, np.ndarray) and seq_ids.dtype == np.int32 else _ids(seq_ids)
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        self._check(self.L.murmur_decode_step_layers(self.h, ids.ctypes.data, len(ids), k_new.data_ptr(), v_new.data_ptr(),
+                                                     q.data_ptr(), out.data_ptr(),
+                                                     lse.data_ptr() if lse is not None else None, layer_begin, layer_end,
+                                                     C.c_float(sm_scale), _stream()))
+
+    def decode_step_chunked(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor, out: torch.Tensor,
+                            layers_per_launch: int, lse: Optional[torch.Tensor] = None, sm_scale: Optional[float] = None):
+        """The whole step issued from C as ceil(L / layers_per_launch) launches (1 = layer-by-layer engine pattern)."""
+        ids = seq_ids if isinstance(seq_ids, np.ndarray) and seq_ids.dtype == np.int32 else _ids(seq_ids)
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        self._check(self.L.murmur_decode_step_chunked(self.h, ids.ctypes.data, len(ids), k_new.data_ptr(), v_new.data_ptr(),
+                                                      q.data_ptr(), out.data_ptr(),
+                                                      lse.data_ptr() if lse is not None else None, layers_per_launch,
+                                                      C.c_float(sm_scale), _stream()))
 
     def decode_step_host(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor,
                          out: torch.Tensor, sm_scale: Optional[float] = None):

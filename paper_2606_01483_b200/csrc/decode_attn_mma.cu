@@ -124,6 +124,8 @@ struct AttnParams {
   float* lse;
   const uint16_t* k_new;  // step mode: [n_layers][n_seqs][n_kv][128] rows of this step's token
   const uint16_t* v_new;
+  int write_only;         // step mode, layers after the first of a step issued in layer ranges: the integer state is
+                          // already committed (slot reserved, eviction done) - only write this range's rows + attend
   int has_window;         // murmur_decode_attn_windowed: attend over the A(t) of THIS policy instead of the sequence's
   int w_s, d, k_s, w_o, k_o;
   int seq_base, n_seqs_total, layer_begin, n_layers_call;
@@ -207,9 +209,11 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     const SeqDev& sd = c.seqs[list.ids[i]];
     SeqParams sp = load_params(sd);
     const int old_nblk = (sp.len + p - 1) >> plog;
-    if (kStep) {
+    if (kStep && !prm.write_only) {
       sp.len += 1;
       if (!sd.active || ((sp.len + p - 1) >> plog) > c.max_blocks) s.abort = 2;
+    } else if (kStep && (!sd.active || sp.len < 1)) {
+      s.abort = 2;
     }
     s.sp[i] = sp;
     s.old_nblk[i] = old_nblk;
@@ -268,11 +272,13 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   if (kStep && warp == kConsumerWarps + kGroups) {
     // ===================================== keeper warp =====================================
     // All the old state this CTA needs is in shared memory now: take the ticket first.
+    // (write-only layer ranges change no integer state: no ticket, no table products, no commit)
+    const bool wo = prm.write_only != 0;
     int last = 0;
-    if (lane == 0) last = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
+    if (lane == 0 && !wo) last = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
     last = __shfl_sync(0xffffffffu, last, 0);
     // (1) the eviction's table products for the post-append state, spread over the CTAs
-    for (int task = (int)blockIdx.x; task < 2 * n_seqs; task += (int)gridDim.x) {
+    for (int task = (int)blockIdx.x; task < (wo ? 0 : 2 * n_seqs); task += (int)gridDim.x) {
       const int role = 1 + task / n_seqs, i = task % n_seqs;
       const AttnLookup lk{c.block_table + (size_t)list.ids[i] * c.max_blocks, s.old_nblk[i], s.newpage[i]};
       evict_task(c, list.ids[i], s.sp[i], role, lk);
@@ -288,7 +294,9 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         const int slot = (s.sp[i].len - 1) & (p - 1);
         const int page = s.tokpage[i];
         if (page < 0) {
-          atomicCAS(&c.ctrl[kCtrlError], 0, 2);
+          // write-only range: the eviction of this step (run with the first range) may already have
+          // freed the block of a token that is dead on arrival (w_out = 0) - its rows are dropped
+          if (!(wo && !s.newatt[i])) atomicCAS(&c.ctrl[kCtrlError], 0, 2);
           continue;
         }
         const uint4 val = reinterpret_cast<const uint4*>(is_v ? prm.v_new : prm.k_new)[(size_t)r * 16 + sub];
@@ -753,10 +761,12 @@ cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_bas
   return launch_mma<false>(c, list, prm, grid, pdl, st, info);
 }
 
-// The whole decode step (append one token per sequence, evict, attend) as ONE launch, all layers.
+// The whole decode step (append one token per sequence, evict, attend) as ONE launch over the layers
+// [layer_begin, layer_end); write_only: a later layer range of a step whose first range has already
+// reserved the slots and run the eviction.
 cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void* k_new, const void* v_new,
-                            const void* q, void* out, float* lse, float sm_scale, int grid, bool pdl, cudaStream_t st,
-                            LaunchInfo* info) {
+                            const void* q, void* out, float* lse, float sm_scale, int layer_begin, int layer_end,
+                            bool write_only, int grid, bool pdl, cudaStream_t st, LaunchInfo* info) {
   AttnParams prm{};
   prm.q = reinterpret_cast<const uint16_t*>(q);
   prm.out = reinterpret_cast<uint16_t*>(out);
@@ -765,8 +775,9 @@ cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void*
   prm.v_new = reinterpret_cast<const uint16_t*>(v_new);
   prm.seq_base = 0;
   prm.n_seqs_total = list.n;
-  prm.layer_begin = 0;
-  prm.n_layers_call = c.n_layers;
+  prm.layer_begin = layer_begin;
+  prm.n_layers_call = layer_end - layer_begin;
+  prm.write_only = write_only ? 1 : 0;
   prm.sm_scale = sm_scale;
   return launch_mma<true>(c, list, prm, grid, pdl, st, info);
 }

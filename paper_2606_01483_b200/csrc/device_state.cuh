@@ -198,11 +198,14 @@ cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_bas
                             void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
                             bool pdl, const SeqParams* window, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void* k_new, const void* v_new,
-                            const void* q, void* out, float* lse, float sm_scale, int grid, bool pdl, cudaStream_t st,
-                            LaunchInfo* info);
+                            const void* q, void* out, float* lse, float sm_scale, int layer_begin, int layer_end,
+                            bool write_only, int grid, bool pdl, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_prefill_attn(const CacheView& c, int seq, int pos_begin, int n_tok, const void* q, void* out,
                                 float* lse, int layer_begin, int layer_end, float sm_scale, cudaStream_t st,
                                 LaunchInfo* info);
+cudaError_t launch_prefill_attn_umma(const CacheView& c, int seq, int pos_begin, int n_tok, const void* q, void* out,
+                                     float* lse, int layer_begin, int layer_end, float sm_scale, cudaStream_t st,
+                                     LaunchInfo* info);
 cudaError_t launch_attn_profile(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                                 const SeqParams* candidate, float frac, void* out, float* scratch, long long stride,
                                 int layer_begin, int layer_end, float sm_scale, cudaStream_t st, LaunchInfo* info);

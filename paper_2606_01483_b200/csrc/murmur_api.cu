@@ -110,6 +110,7 @@ struct murmur_cache {
   int attn_grid_opt;
   int pdl_opt;         // programmatic dependent launch between the kernels of a step
   int fuse_step_opt;   // murmur_decode_step: append + evict in one launch
+  int prefill_variant_opt;  // MURMUR_PREFILL_*
   murmur_stats_t stats;
   cudaError_t last_cuda;
   uint8_t* ws;
@@ -179,6 +180,7 @@ murmur_status_t murmur_cache_create(const murmur_cache_desc_t* d, murmur_cache_t
   c->attn_grid_opt = 0;
   c->pdl_opt = 1;
   c->fuse_step_opt = 2;
+  c->prefill_variant_opt = MURMUR_PREFILL_AUTO;
   std::memset(&c->stats, 0, sizeof c->stats);
   c->last_cuda = cudaSuccess;
   int dev = 0;
@@ -457,13 +459,28 @@ static murmur_status_t check_step(murmur_cache_t* c, const int32_t* seq_ids, int
   return MURMUR_OK;
 }
 
-murmur_status_t murmur_decode_step(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* k_new,
-                                   const void* v_new, const void* q, void* out, float* lse, float sm_scale,
-                                   void* stream) {
+// One decode step restricted to the layers [layer_begin, layer_end).  layer_begin == 0 opens the step:
+// slots reserved, lengths advanced, eviction run; later ranges only write their rows and attend.
+static murmur_status_t step_layers_impl(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* k_new,
+                                        const void* v_new, const void* q, void* out, float* lse, int32_t layer_begin,
+                                        int32_t layer_end, float sm_scale, void* stream) {
   if (!c || !k_new || !v_new || !q || !out) return MURMUR_ERR_INVALID_ARG;
   if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
-  murmur_status_t st = check_step(c, seq_ids, n_seqs);
-  if (st != MURMUR_OK) return st;
+  if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
+  const bool opens = (layer_begin == 0);
+  murmur_status_t st;
+  if (opens) {
+    st = check_step(c, seq_ids, n_seqs);
+    if (st != MURMUR_OK) return st;
+  } else {
+    if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch) return MURMUR_ERR_INVALID_ARG;
+    st = check_ids(c, seq_ids, n_seqs);
+    if (st != MURMUR_OK) return st;
+    for (int i = 0; i < n_seqs; ++i) {  // the step must have been opened: token reserved, eviction run
+      const HostSeq& hs = c->seqs[seq_ids[i]];
+      if (hs.sp.len < 1 || hs.evict_len != hs.sp.len) return MURMUR_ERR_STATE;
+    }
+  }
   int32_t ones[kMaxSeqsPerLaunch];
   for (int i = 0; i < n_seqs; ++i) ones[i] = 1;
   int variant = c->attn_variant_opt;
@@ -475,31 +492,67 @@ murmur_status_t murmur_decode_step(murmur_cache_t* c, const int32_t* seq_ids, in
     for (int i = 0; i < n_seqs; ++i) list.ids[i] = seq_ids[i];
     const int grid = c->attn_grid_opt > 0 ? c->attn_grid_opt : c->sm_count;
     LaunchInfo li{};
-    MM_CUDA(c, launch_step_mma(c->view, list, k_new, v_new, q, out, lse, sm_scale, grid, c->pdl_opt != 0,
-                               (cudaStream_t)stream, &li));
+    MM_CUDA(c, launch_step_mma(c->view, list, k_new, v_new, q, out, lse, sm_scale, layer_begin, layer_end, !opens, grid,
+                               c->pdl_opt != 0, (cudaStream_t)stream, &li));
     note(c, li);
-    const int32_t p = c->desc.page_size;
-    for (int i = 0; i < n_seqs; ++i) {  // host mirror of the append (validated by check_step) ...
-      HostSeq& hs = c->seqs[seq_ids[i]];
-      c->free_pages -= blocks_for(hs.sp.len + 1, p) - blocks_for(hs.sp.len, p);
-      hs.sp.len += 1;
+    if (opens) {
+      const int32_t p = c->desc.page_size;
+      for (int i = 0; i < n_seqs; ++i) {  // host mirror of the append (validated by check_step) ...
+        HostSeq& hs = c->seqs[seq_ids[i]];
+        c->free_pages -= blocks_for(hs.sp.len + 1, p) - blocks_for(hs.sp.len, p);
+        hs.sp.len += 1;
+      }
+      mirror_evict(c, seq_ids, n_seqs);  // ... and of the eviction
+      c->stats.append_calls += 1;
     }
-    mirror_evict(c, seq_ids, n_seqs);  // ... and of the eviction
-    c->stats.append_calls += 1;
     c->stats.attn_calls += 1;
     c->stats.attn_grid = li.grid;
     c->stats.attn_smem_bytes = li.smem;
     c->stats.attn_variant = variant;
     return MURMUR_OK;
   }
-  const bool fuse = c->fuse_step_opt != 0;  // n_seqs <= 128 (check_step): one append launch
-  st = append_impl(c, seq_ids, ones, n_seqs, k_new, v_new, 0, c->desc.n_layers, fuse, stream);
+  const bool fuse = opens && c->fuse_step_opt != 0;  // n_seqs <= 128 (check_step): one append launch
+  st = append_impl(c, seq_ids, ones, n_seqs, k_new, v_new, layer_begin, layer_end, fuse, stream);
   if (st != MURMUR_OK) return st;
-  if (!fuse) {
+  if (opens && !fuse) {
     st = murmur_kv_evict(c, seq_ids, n_seqs, stream);
     if (st != MURMUR_OK) return st;
   }
-  return murmur_decode_attn(c, seq_ids, n_seqs, q, out, lse, 0, c->desc.n_layers, sm_scale, stream);
+  return murmur_decode_attn(c, seq_ids, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, stream);
+}
+
+murmur_status_t murmur_decode_step(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* k_new,
+                                   const void* v_new, const void* q, void* out, float* lse, float sm_scale,
+                                   void* stream) {
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  return step_layers_impl(c, seq_ids, n_seqs, k_new, v_new, q, out, lse, 0, c->desc.n_layers, sm_scale, stream);
+}
+
+murmur_status_t murmur_decode_step_layers(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* k_new,
+                                          const void* v_new, const void* q, void* out, float* lse, int32_t layer_begin,
+                                          int32_t layer_end, float sm_scale, void* stream) {
+  return step_layers_impl(c, seq_ids, n_seqs, k_new, v_new, q, out, lse, layer_begin, layer_end, sm_scale, stream);
+}
+
+murmur_status_t murmur_decode_step_chunked(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* k_new,
+                                           const void* v_new, const void* q, void* out, float* lse,
+                                           int32_t layers_per_launch, float sm_scale, void* stream) {
+  if (!c || layers_per_launch < 1) return MURMUR_ERR_INVALID_ARG;
+  if (n_seqs < 1 || !k_new || !v_new || !q || !out) return MURMUR_ERR_INVALID_ARG;
+  const int L = c->desc.n_layers;
+  const size_t kv_l = (size_t)n_seqs * c->desc.n_kv_heads * kRowBytes;  // bytes of one layer of k_new / v_new
+  const size_t q_l = (size_t)n_seqs * c->desc.n_q_heads * kRowBytes;    // ... of q / out
+  const size_t lse_l = (size_t)n_seqs * c->desc.n_q_heads;              // floats
+  for (int lb = 0; lb < L; lb += layers_per_launch) {
+    const int le = lb + layers_per_launch < L ? lb + layers_per_launch : L;
+    // the opening range validates the whole step (all-or-nothing) before anything is enqueued
+    murmur_status_t st = step_layers_impl(c, seq_ids, n_seqs, (const uint8_t*)k_new + lb * kv_l,
+                                          (const uint8_t*)v_new + lb * kv_l, (const uint8_t*)q + lb * q_l,
+                                          (uint8_t*)out + lb * q_l, lse ? lse + lb * lse_l : nullptr, lb, le, sm_scale,
+                                          stream);
+    if (st != MURMUR_OK) return st;
+  }
+  return MURMUR_OK;
 }
 
 murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs,
@@ -549,8 +602,14 @@ murmur_status_t murmur_prefill_attn(murmur_cache_t* c, int32_t seq, int32_t pos_
   if (pos_begin < 0 || pos_begin >= pos_end || pos_end > hs.sp.len) return MURMUR_ERR_INVALID_ARG;
   if (hs.freed_blocks != 0) return MURMUR_ERR_STATE;  // something below pos_end may be gone
   LaunchInfo li{};
-  MM_CUDA(c, launch_prefill_attn(c->view, seq, pos_begin, pos_end - pos_begin, q, out, lse, layer_begin, layer_end,
-                                 sm_scale, (cudaStream_t)stream, &li));
+  if (c->prefill_variant_opt == MURMUR_PREFILL_MMA_SYNC) {
+    MM_CUDA(c, launch_prefill_attn(c->view, seq, pos_begin, pos_end - pos_begin, q, out, lse, layer_begin, layer_end,
+                                   sm_scale, (cudaStream_t)stream, &li));
+  } else {  // tcgen05 + tensor memory (the tensor maps need 16-byte aligned bases)
+    if (((uintptr_t)q | (uintptr_t)out) & 15) return MURMUR_ERR_INVALID_ARG;
+    MM_CUDA(c, launch_prefill_attn_umma(c->view, seq, pos_begin, pos_end - pos_begin, q, out, lse, layer_begin,
+                                        layer_end, sm_scale, (cudaStream_t)stream, &li));
+  }
   note(c, li);
   return MURMUR_OK;
 }
@@ -764,6 +823,10 @@ murmur_status_t murmur_set_option(murmur_cache_t* c, int32_t option, int32_t val
     case MURMUR_OPT_FUSE_STEP:
       if (value < 0 || value > 2) return MURMUR_ERR_INVALID_ARG;
       c->fuse_step_opt = value;
+      return MURMUR_OK;
+    case MURMUR_OPT_PREFILL_VARIANT:
+      if (value < MURMUR_PREFILL_AUTO || value > MURMUR_PREFILL_UMMA) return MURMUR_ERR_INVALID_ARG;
+      c->prefill_variant_opt = value;
       return MURMUR_OK;
     default:
       return MURMUR_ERR_INVALID_ARG;

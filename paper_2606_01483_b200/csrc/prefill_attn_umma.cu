@@ -1,0 +1,357 @@
+// murmur_prefill_attn on the 5th-generation tensor cores: tcgen05.mma with accumulators in tensor memory.
+//
+// PAPER.md:95 (chunks are submitted to the engine, which first runs prompt + speech tokens through the
+// model) and PAPER.md:77 (prefill = what is left of model time after the 95.3 % of decoding).  Position
+// x attends, by Eq. 1, to the cache positions y <= x.  This is the one dense
+// contraction of the path, so it runs where dense contractions belong on sm_100a.
+//
+// Work item (one CTA) = a PAIR of row blocks of the same (layer, KV head); a row block is 128
+// consecutive query positions of one query head.  Row blocks are enumerated with the head of the GQA
+// group fastest, so the two blocks of a pair nearly always cover the SAME query positions for two heads
+// that share K/V: every 128-key K/V tile is staged once and used by both (M = 256 rows per staged tile).
+// Heaviest pairs (latest queries) are launched first.
+//
+// Per CTA, 10 warps:
+//   warp 0      TMA producer: Q blocks (tensor map over q, 128-byte swizzle written by the copy engine) and
+//               the K/V tiles, one box per (page, d-half) straight from the paged pools.  The pools' rows are
+//               stored pre-swizzled (16-byte chunk c of slot s at c ^ (s & 7), device_state.cuh); a
+//               [p slots][64 bf16] box of one d-half therefore lands as exactly the 128-byte-swizzled tile
+//               image tcgen05.mma expects - the decode kernels' layout needs no re-tiling.
+//   warp 1      MMA issuer (one lane): S_w = Q_w K^T (SS, both operands K-major) and O_w += P_w V (A = P from
+//               tensor memory, B = V MN-major), completion signalled with tcgen05.commit.
+//   warps 2-5 / 6-9   softmax warpgroup of row block 0 / 1: thread = row = TMEM lane.  Scores are read with
+//               tcgen05.ld, masked on the diagonal, exponentiated in the exp2 domain; P is written back as
+//               bf16 over the first half of the S columns (tcgen05.st).  The running maximum is only raised
+//               when it grows by more than 2^8 (the accumulator is then rescaled in tensor memory), so the
+//               rescale is rare and exact in the end: l and O always share one reference maximum.
+// Tensor memory (512 columns): S_0, S_1 (128 fp32 columns each; P_w aliases the first 64 of S_w), O_0, O_1.
+#include <cuda_bf16.h>
+
+#include "device_state.cuh"
+#include "ptx_utils.cuh"
+#include "umma_utils.cuh"
+
+namespace murmur {
+namespace {
+
+constexpr int kBM = 128;                      // query rows per row block (TMEM lanes)
+constexpr int kBN = 128;                      // keys per K/V tile
+constexpr int kHalfBytes = kBN * 128;         // one d-half of a 128-row tile: [128][64 bf16] = 16 KB
+constexpr int kUStages = 2;
+constexpr int kUThreads = 320;
+constexpr uint32_t kTmemCols = 512;
+constexpr float kRescaleLog2 = 8.f;           // raise the reference maximum only past 2^8
+
+struct __align__(1024) USmem {
+  uint8_t q[2][2][kHalfBytes];                // [row block][d-half]
+  uint8_t k[kUStages][2][kHalfBytes];         // [stage][d-half]
+  uint8_t v[kUStages][2][kHalfBytes];
+  unsigned long long q_full, k_full[kUStages], v_full[kUStages], kv_empty[kUStages];
+  unsigned long long s_ready[2], p_ready[2], o_done[2];
+  uint32_t tmem_base;
+};
+
+struct UParams {
+  uint16_t* out;   // [layers][n_tok][n_q][128]
+  float* lse;      // [layers][n_tok][n_q] or null
+  int seq, pos_begin, n_tok, layer_begin;
+  float sm_scale;
+};
+
+__global__ void __launch_bounds__(kUThreads, 1)
+prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                    const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CacheView c,
+                    const __grid_constant__ UParams prm) {
+  extern __shared__ uint8_t smem_raw[];
+  USmem& s = *reinterpret_cast<USmem*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u));
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int G = c.group, p = c.p, plog = c.p_log2;
+  const int kvh = blockIdx.y, lc = blockIdx.z, layer = prm.layer_begin + lc;
+  const int n_qb = (prm.n_tok + kBM - 1) / kBM;
+  const int n_rb = n_qb * G;                       // row blocks of this (layer, KV head): e = b * G + g
+  const int n_pairs = (n_rb + 1) >> 1;
+  const int pair = n_pairs - 1 - (int)blockIdx.x;  // heaviest first
+  const int pos_end = prm.pos_begin + prm.n_tok;
+  const int len = c.seqs[prm.seq].len;
+
+  int act[2], hq[2], x0[2], xl[2], nkt[2];
+#pragma unroll
+  for (int w = 0; w < 2; ++w) {
+    const int e = 2 * pair + w;
+    act[w] = e < n_rb;
+    const int b = act[w] ? e / G : 0;
+    hq[w] = kvh * G + (act[w] ? e % G : 0);
+    x0[w] = prm.pos_begin + b * kBM;
+    xl[w] = min(pos_end, x0[w] + kBM) - 1;
+    nkt[w] = act[w] ? (xl[w] >> 7) + 1 : 0;
+  }
+  const int n_kt = max(nkt[0], nkt[1]);
+  const int x_last = max(xl[0], act[1] ? xl[1] : 0);
+
+  // ---- set-up: barriers, tensor memory, finite K/V stages ------------------------------------------
+  if (tid == 0) {
+    mbar_init(&s.q_full, 1);
+    for (int i = 0; i < kUStages; ++i) {
+      mbar_init(&s.k_full[i], 1);
+      mbar_init(&s.v_full[i], 1);
+      mbar_init(&s.kv_empty[i], 1);
+    }
+    for (int w = 0; w < 2; ++w) {
+      mbar_init(&s.s_ready[w], 1);
+      mbar_init(&s.p_ready[w], kBM);
+      mbar_init(&s.o_done[w], 1);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    tma_prefetch_desc(&tm_q);
+    tma_prefetch_desc(&tm_k);
+    tma_prefetch_desc(&tm_v);
+  }
+  if (warp == 1) {
+    tmem_alloc(&s.tmem_base, kTmemCols);
+    tmem_relinquish();
+  }
+  // rows of a partial last tile that no copy writes must still be finite (P = 0 times NaN is NaN)
+  for (int i = tid; i < (int)(sizeof(s.v) / 16); i += kUThreads) reinterpret_cast<uint4*>(&s.v[0][0][0])[i] = make_uint4(0u, 0u, 0u, 0u);
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = s.tmem_base;
+
+  if (warp == 0) {
+    // ============================== TMA producer ==============================
+    if (lane == 0) {
+      mbar_expect_tx(&s.q_full, (uint32_t)((act[0] + act[1]) * 2 * kHalfBytes));
+#pragma unroll
+      for (int w = 0; w < 2; ++w)
+        if (act[w])
+          for (int h = 0; h < 2; ++h) tma_load_4d(&s.q[w][h][0], &tm_q, 64 * h, hq[w], x0[w] - prm.pos_begin, lc, &s.q_full);
+      const int32_t* tab = c.block_table + (size_t)prm.seq * c.max_blocks;
+      const int ppt = kBN >> plog;  // pages per tile
+      for (int j = 0; j < n_kt; ++j) {
+        const int st = j % kUStages;
+        const uint32_t ph = (uint32_t)(j / kUStages) & 1u;
+        mbar_wait(&s.kv_empty[st], ph ^ 1u);
+        const int rows = min(kBN, x_last + 1 - j * kBN);   // keys beyond x_last are never needed
+        const int pages = (rows + p - 1) >> plog;           // whole pages (all mapped: x_last < len)
+        const uint32_t bytes = (uint32_t)pages * (uint32_t)p * kRowBytes;
+        mbar_expect_tx(&s.k_full[st], bytes);
+        for (int pg = 0; pg < pages; ++pg) {
+          const int page = tab[j * ppt + pg];
+          for (int h = 0; h < 2; ++h) tma_load_5d(&s.k[st][h][pg * p * 128], &tm_k, 64 * h, 0, kvh, page, layer, &s.k_full[st]);
+        }
+        mbar_expect_tx(&s.v_full[st], bytes);
+        for (int pg = 0; pg < pages; ++pg) {
+          const int page = tab[j * ppt + pg];
+          for (int h = 0; h < 2; ++h) tma_load_5d(&s.v[st][h][pg * p * 128], &tm_v, 64 * h, 0, kvh, page, layer, &s.v_full[st]);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ============================== MMA issuer ==============================
+    const uint32_t idesc_s = umma_idesc_bf16(kBM, kBN, 0, 0);   // S = Q K^T: A, B K-major
+    const uint32_t idesc_o = umma_idesc_bf16(kBM, 128, 0, 1);   // O += P V: A from TMEM, B (V) MN-major, N = d = 128
+    mbar_wait(&s.q_full, 0u);
+    for (int j = 0; j < n_kt; ++j) {
+      const int st = j % kUStages;
+      const uint32_t ph = (uint32_t)(j / kUStages) & 1u;
+      mbar_wait(&s.k_full[st], ph);
+      tc_fence_after();
+      if (lane == 0) {
+#pragma unroll
+        for (int w = 0; w < 2; ++w) {
+          if (j < nkt[w]) {
+            // S_w is free: PV_{j-1} of this row block (which read P over the same columns) was issued before
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+              for (int kk = 0; kk < 4; ++kk)
+                umma_ss(tb + 128u * w, smem_desc_kmajor(smem_u32(&s.q[w][h][0]) + kk * 32),
+                        smem_desc_kmajor(smem_u32(&s.k[st][h][0]) + kk * 32), idesc_s, (h | kk) ? 1u : 0u);
+            umma_commit(&s.s_ready[w]);
+          }
+        }
+      }
+      __syncwarp();
+      mbar_wait(&s.v_full[st], ph);
+      // rows at or beyond the sequence length (inside the last mapped page) hold whatever the pool holds:
+      // their P is 0, but 0 * NaN would poison O - zero them
+      const int first_bad = len - j * kBN;
+      if (first_bad < kBN) {
+        for (int i = lane; i < (kBN - max(first_bad, 0)) * 16; i += 32) {
+          const int r = max(first_bad, 0) + (i >> 4), ch = i & 15;
+          *reinterpret_cast<uint4*>(&s.v[st][ch >> 3][r * 128 + (ch & 7) * 16]) = make_uint4(0u, 0u, 0u, 0u);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+      }
+#pragma unroll
+      for (int w = 0; w < 2; ++w) {
+        if (j < nkt[w]) {
+          mbar_wait(&s.p_ready[w], (uint32_t)j & 1u);
+          tc_fence_after();
+          if (lane == 0) {
+#pragma unroll
+            for (int kk = 0; kk < 8; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk..
+              umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk,
+                      smem_desc_mnmajor(smem_u32(&s.v[st][0][0]) + kk * 16 * 128, kHalfBytes), idesc_o, (j | kk) ? 1u : 0u);
+            umma_commit(&s.o_done[w]);
+          }
+          __syncwarp();
+        }
+      }
+      if (lane == 0) umma_commit(&s.kv_empty[st]);
+      __syncwarp();
+    }
+  } else {
+    // ============================== softmax warpgroups ==============================
+    const int w = (warp - 2) >> 2;         // row block of this warpgroup
+    const int q4 = warp & 3;               // TMEM lane quarter this warp may access
+    const int row = q4 * 32 + lane;
+    const int x = x0[w] + row;             // this thread's query position
+    const uint32_t lane_base = tb + ((uint32_t)(q4 * 32) << 16);
+    const uint32_t s_addr = lane_base + 128u * w, o_addr = lane_base + 256u + 128u * w;
+    const float c2 = prm.sm_scale * 1.4426950408889634f;
+    float m = -INFINITY, l = 0.f;
+    const int n = nkt[w];
+    for (int j = 0; j < n; ++j) {
+      mbar_wait(&s.s_ready[w], (uint32_t)j & 1u);
+      tc_fence_after();
+      uint32_t sc[128];
+      {
+        uint32_t(&a0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[0]);
+        uint32_t(&a1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[32]);
+        uint32_t(&a2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[64]);
+        uint32_t(&a3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[96]);
+        tmem_ld32(s_addr, a0);
+        tmem_ld32(s_addr + 32, a1);
+        tmem_ld32(s_addr + 64, a2);
+        tmem_ld32(s_addr + 96, a3);
+        tmem_wait_ld();
+      }
+      const int y0 = j * kBN;
+      if (y0 + kBN - 1 > x0[w]) {  // the tile reaches past the first row's position: causal mask
+#pragma unroll
+        for (int i = 0; i < 128; ++i)
+          if (y0 + i > x) sc[i] = 0xff800000u;  // -inf
+      }
+      float mx = -INFINITY;
+#pragma unroll
+      for (int i = 0; i < 128; ++i) mx = fmaxf(mx, __uint_as_float(sc[i]));
+      float m_new = fmaxf(m, mx);
+      if (j == 0) {
+        m = m_new;  // key 0 <= every query position: finite
+      } else {
+        const bool need = (m_new - m) * c2 > kRescaleLog2;
+        if (__any_sync(0xffffffffu, need)) {
+          // rescale O (and l) of the rows whose reference maximum moves; PV of the previous tile must have landed
+          mbar_wait(&s.o_done[w], (uint32_t)(j - 1) & 1u);
+          tc_fence_after();
+          const float f = need ? ex2((m - m_new) * c2) : 1.f;
+#pragma unroll
+          for (int cc = 0; cc < 4; ++cc) {
+            uint32_t o[32];
+            tmem_ld32(o_addr + 32 * cc, o);
+            tmem_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+            tmem_st32(o_addr + 32 * cc, o);
+          }
+          l *= f;
+          if (need) m = m_new;
+        }
+      }
+      const float ms = m * c2;
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) {
+        uint32_t pk[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const float p0 = ex2(fmaf(__uint_as_float(sc[32 * cc + 2 * i]), c2, -ms));
+          const float p1 = ex2(fmaf(__uint_as_float(sc[32 * cc + 2 * i + 1]), c2, -ms));
+          l += p0 + p1;
+          pk[i] = pack_bf16(p0, p1);
+        }
+        tmem_st16(s_addr + 16 * cc, pk);
+      }
+      tmem_wait_st();
+      tc_fence_before();
+      mbar_arrive(&s.p_ready[w]);
+    }
+    if (n > 0) {
+      // ---- epilogue: O / l -> bf16 -> out ----
+      mbar_wait(&s.o_done[w], (uint32_t)(n - 1) & 1u);
+      tc_fence_after();
+      const float inv = 1.f / l;
+      const bool valid = x <= xl[w];
+      const size_t orow = ((size_t)lc * prm.n_tok + (size_t)(x - prm.pos_begin)) * c.n_q + hq[w];
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) {
+        uint32_t o[32];
+        tmem_ld32(o_addr + 32 * cc, o);
+        tmem_wait_ld();
+        if (valid) {
+          uint4* dst = reinterpret_cast<uint4*>(prm.out + orow * kHeadDim + 32 * cc);
+#pragma unroll
+          for (int v4 = 0; v4 < 4; ++v4) {
+            uint4 val;
+            val.x = pack_bf16(__uint_as_float(o[8 * v4 + 0]) * inv, __uint_as_float(o[8 * v4 + 1]) * inv);
+            val.y = pack_bf16(__uint_as_float(o[8 * v4 + 2]) * inv, __uint_as_float(o[8 * v4 + 3]) * inv);
+            val.z = pack_bf16(__uint_as_float(o[8 * v4 + 4]) * inv, __uint_as_float(o[8 * v4 + 5]) * inv);
+            val.w = pack_bf16(__uint_as_float(o[8 * v4 + 6]) * inv, __uint_as_float(o[8 * v4 + 7]) * inv);
+            dst[v4] = val;
+          }
+        }
+      }
+      if (valid && prm.lse != nullptr) prm.lse[orow] = m * prm.sm_scale + __logf(l);
+    }
+  }
+  // ---- teardown: the single-lane roles diverged - reconverge before the aligned CTA barrier ----------
+  __syncwarp();
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tb, kTmemCols);
+}
+
+}  // namespace
+
+cudaError_t launch_prefill_attn_umma(const CacheView& c, int seq, int pos_begin, int n_tok, const void* q, void* out,
+                                     float* lse, int layer_begin, int layer_end, float sm_scale, cudaStream_t st,
+                                     LaunchInfo* info) {
+  const int n_layers_call = layer_end - layer_begin;
+  CUtensorMap tm_q, tm_k, tm_v;
+  {
+    const uint64_t dims[4] = {128, (uint64_t)c.n_q, (uint64_t)n_tok, (uint64_t)n_layers_call};
+    const uint64_t str[3] = {256, (uint64_t)c.n_q * 256, (uint64_t)n_tok * c.n_q * 256};
+    const uint32_t box[4] = {64, 1, (uint32_t)kBM, 1};
+    if (!encode_tmap_bf16(&tm_q, q, 4, dims, str, box, true)) return cudaErrorInvalidValue;
+  }
+  {
+    const uint64_t dims[5] = {128, (uint64_t)c.p, (uint64_t)c.n_kv, (uint64_t)c.n_pages, (uint64_t)c.n_layers};
+    const uint64_t str[4] = {256, (uint64_t)c.p * 256, (uint64_t)c.n_kv * c.p * 256, (uint64_t)c.n_pages * c.n_kv * c.p * 256};
+    const uint32_t box[5] = {64, (uint32_t)c.p, 1, 1, 1};
+    if (!encode_tmap_bf16(&tm_k, c.k_pool, 5, dims, str, box, false)) return cudaErrorInvalidValue;
+    if (!encode_tmap_bf16(&tm_v, c.v_pool, 5, dims, str, box, false)) return cudaErrorInvalidValue;
+  }
+  const int smem = (int)sizeof(USmem) + 1024;  // + slack for the 1024-byte alignment of the tiles
+  cudaError_t ea = opt_in_smem_once(kSmemPrefillUmma, reinterpret_cast<const void*>(prefill_umma_kernel), smem);
+  if (ea != cudaSuccess) return ea;
+  UParams prm{};
+  prm.out = reinterpret_cast<uint16_t*>(out);
+  prm.lse = lse;
+  prm.seq = seq;
+  prm.pos_begin = pos_begin;
+  prm.n_tok = n_tok;
+  prm.layer_begin = layer_begin;
+  prm.sm_scale = sm_scale;
+  const int n_qb = (n_tok + kBM - 1) / kBM;
+  const int n_pairs = (n_qb * c.group + 1) / 2;
+  dim3 grid((unsigned)n_pairs, (unsigned)c.n_kv, (unsigned)n_layers_call);
+  prefill_umma_kernel<<<grid, kUThreads, smem, st>>>(tm_q, tm_k, tm_v, c, prm);
+  info->launches += 1;
+  info->grid = (int)(grid.x * grid.y * grid.z);
+  info->smem = smem;
+  return cudaGetLastError();
+}
+
+}  // namespace murmur

@@ -198,6 +198,28 @@ class SideBySide:
                                  sm_scale=self.scale, layer_begin=l, layer_end=l + 1)
         return q, out, lse
 
+    def layer_range_step(self, seq_ids: Sequence[int], ranges: Sequence, want_lse: bool = False):
+        """One decode step through murmur_decode_step_layers, one call (= one launch) per layer range;
+        ranges[0] must start at layer 0 (it opens the step)."""
+        ks, vs = [], []
+        for i in seq_ids:
+            u = self.t_of(i)
+            k, v = self.data[i].out_kv(u, u + 1)
+            ks.append(k)
+            vs.append(v)
+            self._store(i, k, v)
+        k_new = torch.cat(ks, dim=1).contiguous()
+        v_new = torch.cat(vs, dim=1).contiguous()
+        self.oracle.append(seq_ids, [1] * len(seq_ids))
+        self.oracle.evict(seq_ids)
+        q = self.queries(seq_ids)
+        out = torch.empty_like(q)
+        lse = torch.empty(q.shape[:3], dtype=torch.float32, device=self.device) if want_lse else None
+        for a, b in ranges:
+            self.gpu.decode_step_layers(seq_ids, k_new[a:b].contiguous(), v_new[a:b].contiguous(), q[a:b].contiguous(),
+                                        out[a:b], a, b, lse=lse[a:b] if want_lse else None, sm_scale=self.scale)
+        return q, out, lse
+
     def queries(self, seq_ids: Sequence[int]) -> torch.Tensor:
         """[L, n_seqs, n_q, d]: query of each sequence's newest output token."""
         qs = [self.data[i].q_step(max(1, self.t_of(i))) for i in seq_ids]

@@ -549,7 +549,61 @@ def test_per_layer_mode_append_write_only_layers(dev):
     a.close()
 
 
-@pytest.mark.parametrize("mode", ["one_launch", "two_launches", "three_calls", "per_layer"])
+def test_decode_step_layers_one_launch_per_layer_range(dev):
+    """murmur_decode_step_layers: the step issued in layer ranges, ONE launch per call - the opening call
+    (layers [0, 1)) reserves, commits and evicts, the others (issued out of order here) only write their
+    rows and attend.  Ragged page-16 batch with a w_out = 0 sequence, run past two pages of tokens; integer
+    state bit-exact, rows of all layers gathered back bit-exact, attention of every layer in tolerance."""
+    specs = _ragged16_specs_with_w_out_0()
+    cfg = workloads.config5().with_seqs(specs).with_layers(4)
+    a = _mk(cfg, dev)
+    active = list(range(cfg.batch))
+    a.bulk_prefill(active, 1)
+    step = 0
+    while active:
+        order = active[::-1] if step % 2 else list(active)
+        n0 = a.gpu.stats()["kernel_launches"]
+        ranges = [(0, 1), (2, 4), (1, 2)] if step % 2 else [(0, 2), (2, 3), (3, 4)]
+        q, out, lse = a.layer_range_step(order, ranges, want_lse=True)
+        assert a.gpu.stats()["kernel_launches"] == n0 + 3, "one launch per layer range"
+        a.check_integer_state(active)
+        a.check_attention(order, q, out, lse)
+        if step % 5 == 0 or any((a.oracle.seqs[i].length % 16) in (0, 1) for i in active):
+            for i in active:
+                a.check_gather(i, layers=None)
+        done = [i for i in active if a.t_of(i) >= cfg.seqs[i].T]
+        for i in done:
+            a.gpu.seq_end(i)
+            a.oracle.seq_end(i)
+        active = [i for i in active if i not in done]
+        step += 1
+    assert step > 2 * 16
+    assert list(a.gpu.free_stack()) == a.oracle.free_stack
+    assert a.gpu.last_error() == 0
+    a.close()
+
+
+def test_decode_step_layers_rejects_a_range_of_an_unopened_step(dev):
+    from paper_2606_01483_b200 import MurmurCache, MurmurError
+
+    c = MurmurCache(3, 28, 4, 128, 16, max_seqs=2, max_blocks_per_seq=8, n_pages=8, device=dev)
+    c.seq_begin(0, 4, 20, 0, (8, 4, 0, 8, 1))
+    kv = torch.zeros(3, 30, 4, 128, dtype=torch.bfloat16, device=dev)
+    c.kv_append([0], [30], kv, kv.clone())  # appended, not evicted: no step is open
+    k1 = torch.zeros(1, 1, 4, 128, dtype=torch.bfloat16, device=dev)
+    q1 = torch.zeros(1, 1, 28, 128, dtype=torch.bfloat16, device=dev)
+    with pytest.raises(MurmurError) as e:
+        c.decode_step_layers([0], k1, k1.clone(), q1, torch.empty_like(q1), 1, 2)
+    assert e.value.status == 2
+    assert c.seq_state(0)["length"] == 30
+    c.decode_step_layers([0], k1, k1.clone(), q1, torch.empty_like(q1), 0, 1)  # opens the step
+    assert c.seq_state(0)["length"] == 31
+    c.decode_step_layers([0], k1, k1.clone(), q1, torch.empty_like(q1), 2, 3)
+    assert c.seq_state(0)["length"] == 31 and c.last_error() == 0
+    c.close()
+
+
+@pytest.mark.parametrize("mode", ["one_launch", "two_launches", "three_calls", "per_layer", "layer_calls"])
 def test_evict_unmaps_the_block_of_the_newest_token(dev, mode):
     """w_out = 0 with page 16: at every step whose token completes a block of dead outputs, the same
     step's eviction frees the block that token was just written to.  Every form of the step must leave
@@ -571,6 +625,8 @@ def test_evict_unmaps_the_block_of_the_newest_token(dev, mode):
             q, out, lse = a.fused_step(ids, want_lse=True)
         elif mode == "per_layer":
             q, out, lse = a.per_layer_step(ids, want_lse=True)
+        elif mode == "layer_calls":
+            q, out, lse = a.layer_range_step(ids, [(0, 1), (1, 2)], want_lse=True)
         else:
             a.append_step(ids)
             a.evict(ids)
