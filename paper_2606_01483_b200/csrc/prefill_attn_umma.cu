@@ -18,7 +18,9 @@
 //               [p slots][64 bf16] box of one d-half therefore lands as exactly the 128-byte-swizzled tile
 //               image tcgen05.mma expects - the decode kernels' layout needs no re-tiling.
 //   warp 1      MMA issuer (one lane): S_w = Q_w K^T (SS, both operands K-major) and O_w += P_w V (A = P from
-//               tensor memory, B = V MN-major), completion signalled with tcgen05.commit.
+//               tensor memory, B = V MN-major), completion signalled with tcgen05.commit.  Issue order per
+//               tile j:  S(1,j)  PV(0,j)  S(0,j+1)  PV(1,j) - the two row blocks run half a period apart, so
+//               one warpgroup's softmax has the other's MMAs to hide under.
 //   warps 2-5 / 6-9   softmax warpgroup of row block 0 / 1: thread = row = TMEM lane.  Scores are read with
 //               tcgen05.ld, masked on the diagonal, exponentiated in the exp2 domain; P is written back as
 //               bf16 over the first half of the S columns (tcgen05.st).  The running maximum is only raised
@@ -46,7 +48,7 @@ struct __align__(1024) USmem {
   uint8_t q[2][2][kHalfBytes];                // [row block][d-half]
   uint8_t k[kUStages][2][kHalfBytes];         // [stage][d-half]
   uint8_t v[kUStages][2][kHalfBytes];
-  unsigned long long q_full, k_full[kUStages], v_full[kUStages], kv_empty[kUStages];
+  unsigned long long q_full, k_full[kUStages], v_full[kUStages], k_empty[kUStages], v_empty[kUStages];
   unsigned long long s_ready[2], p_ready[2], o_done[2];
   uint32_t tmem_base;
 };
@@ -94,11 +96,12 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     for (int i = 0; i < kUStages; ++i) {
       mbar_init(&s.k_full[i], 1);
       mbar_init(&s.v_full[i], 1);
-      mbar_init(&s.kv_empty[i], 1);
+      mbar_init(&s.k_empty[i], 1);
+      mbar_init(&s.v_empty[i], 1);
     }
     for (int w = 0; w < 2; ++w) {
       mbar_init(&s.s_ready[w], 1);
-      mbar_init(&s.p_ready[w], kBM);
+      mbar_init(&s.p_ready[w], 4);  // one arrival per softmax warp
       mbar_init(&s.o_done[w], 1);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -116,7 +119,13 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tb = s.tmem_base;
+  // All 512 columns are ours, so the allocation starts at lane 0 / column 0; using the literal (checked here)
+  // keeps the tcgen05 operands provably warp-uniform for the compiler.
+  if (s.tmem_base != 0u) {
+    if (tid == 0) atomicCAS(&c.ctrl[kCtrlError], 0, 4);
+    __trap();
+  }
+  constexpr uint32_t tb = 0u;
 
   if (warp == 0) {
     // ============================== TMA producer ==============================
@@ -131,7 +140,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       for (int j = 0; j < n_kt; ++j) {
         const int st = j % kUStages;
         const uint32_t ph = (uint32_t)(j / kUStages) & 1u;
-        mbar_wait(&s.kv_empty[st], ph ^ 1u);
+        mbar_wait(&s.k_empty[st], ph ^ 1u);
         const int rows = min(kBN, x_last + 1 - j * kBN);   // keys beyond x_last are never needed
         const int pages = (rows + p - 1) >> plog;           // whole pages (all mapped: x_last < len)
         const uint32_t bytes = (uint32_t)pages * (uint32_t)p * kRowBytes;
@@ -140,6 +149,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
           const int page = tab[j * ppt + pg];
           for (int h = 0; h < 2; ++h) tma_load_5d(&s.k[st][h][pg * p * 128], &tm_k, 64 * h, 0, kvh, page, layer, &s.k_full[st]);
         }
+        mbar_wait(&s.v_empty[st], ph ^ 1u);
         mbar_expect_tx(&s.v_full[st], bytes);
         for (int pg = 0; pg < pages; ++pg) {
           const int page = tab[j * ppt + pg];
@@ -152,28 +162,46 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const uint32_t idesc_s = umma_idesc_bf16(kBM, kBN, 0, 0);   // S = Q K^T: A, B K-major
     const uint32_t idesc_o = umma_idesc_bf16(kBM, 128, 0, 1);   // O += P V: A from TMEM, B (V) MN-major, N = d = 128
     mbar_wait(&s.q_full, 0u);
-    for (int j = 0; j < n_kt; ++j) {
+    // Issue order (the two row blocks half a period apart, so that one warpgroup's softmax always runs
+    // under the other's MMAs):  S(0,0);  then per tile j:  S(1,j)  PV(0,j)  S(0,j+1)  PV(1,j).
+    // S_w aliases P_w: S(w,j+1) is issued after PV(w,j), and tcgen05.mma executes in issue order.
+    // Descriptors: one base per operand tile, the k-steps only add to the start-address field.
+    const uint64_t qd[2][2] = {{smem_desc_kmajor(smem_u32(&s.q[0][0][0])), smem_desc_kmajor(smem_u32(&s.q[0][1][0]))},
+                               {smem_desc_kmajor(smem_u32(&s.q[1][0][0])), smem_desc_kmajor(smem_u32(&s.q[1][1][0]))}};
+    auto issue_s = [&](int w, int j) {  // S_w = Q_w K_j^T
       const int st = j % kUStages;
-      const uint32_t ph = (uint32_t)(j / kUStages) & 1u;
-      mbar_wait(&s.k_full[st], ph);
+      mbar_wait(&s.k_full[st], (uint32_t)(j / kUStages) & 1u);
       tc_fence_after();
+      const uint64_t kd0 = smem_desc_kmajor(smem_u32(&s.k[st][0][0])), kd1 = smem_desc_kmajor(smem_u32(&s.k[st][1][0]));
       if (lane == 0) {
 #pragma unroll
-        for (int w = 0; w < 2; ++w) {
-          if (j < nkt[w]) {
-            // S_w is free: PV_{j-1} of this row block (which read P over the same columns) was issued before
+        for (int kk = 0; kk < 4; ++kk) umma_ss(tb + 128u * w, qd[w][0] + 2u * kk, kd0 + 2u * kk, idesc_s, kk ? 1u : 0u);  // +32 bytes per k-step
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-              for (int kk = 0; kk < 4; ++kk)
-                umma_ss(tb + 128u * w, smem_desc_kmajor(smem_u32(&s.q[w][h][0]) + kk * 32),
-                        smem_desc_kmajor(smem_u32(&s.k[st][h][0]) + kk * 32), idesc_s, (h | kk) ? 1u : 0u);
-            umma_commit(&s.s_ready[w]);
-          }
-        }
+        for (int kk = 0; kk < 4; ++kk) umma_ss(tb + 128u * w, qd[w][1] + 2u * kk, kd1 + 2u * kk, idesc_s, 1u);
+        umma_commit(&s.s_ready[w]);
       }
       __syncwarp();
-      mbar_wait(&s.v_full[st], ph);
+    };
+    auto issue_pv = [&](int w, int j) {  // O_w += P_w V_j
+      const int st = j % kUStages;
+      mbar_wait(&s.p_ready[w], (uint32_t)j & 1u);
+      tc_fence_after();
+      const uint64_t vd = smem_desc_mnmajor(smem_u32(&s.v[st][0][0]), kHalfBytes);
+      if (lane == 0) {
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk.. (+2048 bytes = +128)
+          umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, vd + 128u * kk, idesc_o, (j | kk) ? 1u : 0u);
+        umma_commit(&s.o_done[w]);
+      }
+      __syncwarp();
+    };
+    if (nkt[0] > 0) issue_s(0, 0);
+    for (int j = 0; j < n_kt; ++j) {
+      const int st = j % kUStages;
+      if (j < nkt[1]) issue_s(1, j);
+      if (lane == 0) umma_commit(&s.k_empty[st]);  // K_j: both S(0,j) and S(1,j) are behind this point
+      __syncwarp();
+      mbar_wait(&s.v_full[st], (uint32_t)(j / kUStages) & 1u);
       // rows at or beyond the sequence length (inside the last mapped page) hold whatever the pool holds:
       // their P is 0, but 0 * NaN would poison O - zero them
       const int first_bad = len - j * kBN;
@@ -185,22 +213,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
       }
-#pragma unroll
-      for (int w = 0; w < 2; ++w) {
-        if (j < nkt[w]) {
-          mbar_wait(&s.p_ready[w], (uint32_t)j & 1u);
-          tc_fence_after();
-          if (lane == 0) {
-#pragma unroll
-            for (int kk = 0; kk < 8; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk..
-              umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk,
-                      smem_desc_mnmajor(smem_u32(&s.v[st][0][0]) + kk * 16 * 128, kHalfBytes), idesc_o, (j | kk) ? 1u : 0u);
-            umma_commit(&s.o_done[w]);
-          }
-          __syncwarp();
-        }
-      }
-      if (lane == 0) umma_commit(&s.kv_empty[st]);
+      if (j < nkt[0]) issue_pv(0, j);
+      if (j + 1 < nkt[0]) issue_s(0, j + 1);
+      if (j < nkt[1]) issue_pv(1, j);
+      if (lane == 0) umma_commit(&s.v_empty[st]);
       __syncwarp();
     }
   } else {
@@ -276,7 +292,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       }
       tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(&s.p_ready[w]);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&s.p_ready[w]);
     }
     if (n > 0) {
       // ---- epilogue: O / l -> bf16 -> out ----
@@ -310,7 +327,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
   __syncwarp();
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tb, kTmemCols);
+  if (warp == 1) tmem_dealloc(0u, kTmemCols);
 }
 
 }  // namespace
