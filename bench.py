@@ -678,6 +678,7 @@ def run_murmur(args):
     if sampler:
         sampler.window(w0, w1)
     e2e_launches = cache.stats()["kernel_launches"] / Ke
+    e2e_zero_copy = cache.stats()["host_zero_copy_steps"] == Ke
     us_e2e_dev = c0.elapsed_time(c1) / Ke * 1e3
     us_e2e_wall = (w1 - w0) / Ke * 1e6
     us_e2e = max(us_e2e_dev, us_e2e_wall)
@@ -814,6 +815,10 @@ def run_murmur(args):
         "replay": replay, "protocol": protocol, "other_workloads": others,
         "e2e": {"value": us_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "device_us": us_e2e_dev, "wall_us": us_e2e_wall, "steps": Ke, "launches_per_step": e2e_launches,
+                "path": ("zero-copy: the step kernel reads k_new / v_new / q from the pinned host buffers and stores out to the "
+                         "pinned host buffer through their device-mapped addresses (the declared bytes cross PCIe inside the "
+                         "timed kernel; no staging copies)" if e2e_zero_copy else
+                         "staged: cudaMemcpyAsync host->device, step, cudaMemcpyAsync device->host"),
                 "api": "murmur_decode_step_host (pinned host k_new | v_new | q -> out), stream-synchronised per step"},
         "gpu_launches": int(launches), "attn_grid": st["attn_grid"], "attn_smem_bytes": st["attn_smem_bytes"],
         "device_error_word": wb_err, "clocks": clocks_all.get("main"),

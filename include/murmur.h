@@ -106,6 +106,7 @@ typedef struct {
   int32_t attn_smem_bytes; /* dynamic shared memory of the last attention launch */
   int32_t attn_variant;    /* variant used by the last attention launch (MURMUR_ATTN_*) */
   int32_t sm_count;
+  int64_t host_zero_copy_steps; /* murmur_decode_step_host calls that ran on page-locked host buffers in place */
 } murmur_stats_t;
 
 /* Options for murmur_set_option. */
@@ -119,6 +120,8 @@ typedef struct {
                                      else falls back to 1);
                                      1 = two launches (append with the eviction fused in, then attention);
                                      0 = three launches (append, evict, attention) */
+#define MURMUR_OPT_HOST_ZERO_COPY 6 /* value: 1 (default) = murmur_decode_step_host works on page-locked host buffers
+                                      in place (zero-copy); 0 = always stage through device buffers */
 #define MURMUR_OPT_PREFILL_VARIANT 5 /* value: MURMUR_PREFILL_AUTO / _MMA_SYNC / _UMMA */
 #define MURMUR_PREFILL_AUTO 0     /* = MURMUR_PREFILL_UMMA */
 #define MURMUR_PREFILL_MMA_SYNC 1 /* warp-level mma.sync kernel (the round-1 path, kept as a cross-check) */
@@ -224,12 +227,15 @@ MURMUR_API murmur_status_t murmur_decode_step_chunked(murmur_cache_t* cache, con
                                                       float* lse, int32_t layers_per_launch, float sm_scale,
                                                       void* stream);
 
-/* One whole decode step from HOST buffers (the end-to-end entry): copies k_new, v_new, q
- * (HOST, pinned or pageable, layouts as above with 1 token per sequence and all layers) to
- * device staging, runs append -> evict -> decode_attn, copies out (HOST bf16
- * [n_layers][n_seqs][n_q_heads][head_dim]) back, all on `stream`; returns after enqueueing
- * (synchronise the stream before reading out_host).  n_seqs <= MURMUR_MAX_SEQS_PER_LAUNCH.  If the three
- * input buffers are packed back to back (k_new, then v_new, then q) they are moved with one copy. */
+/* One whole decode step from HOST buffers (the end-to-end entry): k_new, v_new, q in, out back (HOST bf16, layouts
+ * as for murmur_decode_step with all layers), all on `stream`; returns after enqueueing (synchronise the stream
+ * before reading out_host).  n_seqs <= MURMUR_MAX_SEQS_PER_LAUNCH.
+ *   Page-locked buffers (cudaHostAlloc, cudaHostRegister, torch pin_memory; all four, 16-byte aligned): ZERO-COPY -
+ *   the one-launch step kernel reads q / k_new / v_new from the host buffers and stores out to the host buffer
+ *   itself, through their device-mapped addresses; the data crosses PCIe inside the kernel, overlapped with the
+ *   K/V stream from HBM, and there is no staging copy.  MURMUR_OPT_HOST_ZERO_COPY = 0 turns this off.
+ *   Pageable buffers: staged - cudaMemcpyAsync to device staging (one copy if k_new, v_new, q are packed back to
+ *   back), the step, cudaMemcpyAsync of out back. */
 MURMUR_API murmur_status_t murmur_decode_step_host(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
                                                    const void* k_new_host, const void* v_new_host,
                                                    const void* q_host, void* out_host, float sm_scale, void* stream);

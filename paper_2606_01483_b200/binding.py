@@ -22,6 +22,7 @@ MURMUR_OPT_ATTN_GRID = 2
 MURMUR_OPT_PDL = 3
 MURMUR_OPT_FUSE_STEP = 4
 MURMUR_OPT_PREFILL_VARIANT = 5
+MURMUR_OPT_HOST_ZERO_COPY = 6
 MURMUR_PREFILL_AUTO, MURMUR_PREFILL_MMA_SYNC, MURMUR_PREFILL_UMMA = 0, 1, 2
 MURMUR_ATTN_AUTO, MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA = 0, 1, 2
 
@@ -56,7 +57,8 @@ class Policy(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("kernel_launches", C.c_int64), ("append_calls", C.c_int64), ("evict_calls", C.c_int64),
                 ("attn_calls", C.c_int64), ("free_pages", C.c_int64), ("attn_grid", C.c_int32),
-                ("attn_smem_bytes", C.c_int32), ("attn_variant", C.c_int32), ("sm_count", C.c_int32)]
+                ("attn_smem_bytes", C.c_int32), ("attn_variant", C.c_int32), ("sm_count", C.c_int32),
+                ("host_zero_copy_steps", C.c_int64)]
 
 
 class MurmurError(RuntimeError):

@@ -111,6 +111,7 @@ struct murmur_cache {
   int pdl_opt;         // programmatic dependent launch between the kernels of a step
   int fuse_step_opt;   // murmur_decode_step: append + evict in one launch
   int prefill_variant_opt;  // MURMUR_PREFILL_*
+  int host_zero_copy_opt;   // murmur_decode_step_host: work on page-locked host buffers in place
   murmur_stats_t stats;
   cudaError_t last_cuda;
   uint8_t* ws;
@@ -181,6 +182,7 @@ murmur_status_t murmur_cache_create(const murmur_cache_desc_t* d, murmur_cache_t
   c->pdl_opt = 1;
   c->fuse_step_opt = 2;
   c->prefill_variant_opt = MURMUR_PREFILL_AUTO;
+  c->host_zero_copy_opt = 1;
   std::memset(&c->stats, 0, sizeof c->stats);
   c->last_cuda = cudaSuccess;
   int dev = 0;
@@ -567,6 +569,30 @@ murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_id
   cudaStream_t s = (cudaStream_t)stream;
   const size_t kv_b = (size_t)c->desc.n_layers * n_seqs * c->desc.n_kv_heads * kRowBytes;
   const size_t q_b = (size_t)c->desc.n_layers * n_seqs * c->desc.n_q_heads * kRowBytes;
+  // Zero-copy path: when all four buffers are page-locked (cudaHostAlloc / cudaHostRegister / torch pin_memory)
+  // the step kernel works on their device-mapped addresses directly - Q and the new K/V rows arrive by the same
+  // bulk copies straight from host memory while the pool streams from HBM, and `out` is stored to the host
+  // buffer by the kernel.  The bytes still cross PCIe inside the call; no staging copy on either side.
+  if (c->host_zero_copy_opt) {
+    const void* hp[4] = {k_new_host, v_new_host, q_host, out_host};
+    void* dp[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool mapped = true;
+    for (int i = 0; i < 4 && mapped; ++i) {
+      cudaPointerAttributes at{};
+      if (cudaPointerGetAttributes(&at, hp[i]) != cudaSuccess) {
+        (void)cudaGetLastError();  // unregistered host memory on older drivers: not an error here
+        mapped = false;
+      } else if (at.type != cudaMemoryTypeHost || at.devicePointer == nullptr || ((uintptr_t)at.devicePointer & 15)) {
+        mapped = false;
+      } else {
+        dp[i] = at.devicePointer;
+      }
+    }
+    if (mapped) {
+      c->stats.host_zero_copy_steps += 1;
+      return murmur_decode_step(c, seq_ids, n_seqs, dp[0], dp[1], dp[2], dp[3], nullptr, sm_scale, stream);
+    }
+  }
   uint8_t* dk = c->ws + c->cv.stage_k;
   uint8_t* dv = c->ws + c->cv.stage_v;
   uint8_t* dq = c->ws + c->cv.stage_q;
@@ -824,6 +850,9 @@ murmur_status_t murmur_set_option(murmur_cache_t* c, int32_t option, int32_t val
       if (value < 0 || value > 2) return MURMUR_ERR_INVALID_ARG;
       c->fuse_step_opt = value;
       return MURMUR_OK;
+    case MURMUR_OPT_HOST_ZERO_COPY:
+      c->host_zero_copy_opt = value != 0;
+      return MURMUR_OK;
     case MURMUR_OPT_PREFILL_VARIANT:
       if (value < MURMUR_PREFILL_AUTO || value > MURMUR_PREFILL_UMMA) return MURMUR_ERR_INVALID_ARG;
       c->prefill_variant_opt = value;
@@ -843,6 +872,7 @@ murmur_status_t murmur_reset_stats(murmur_cache_t* c) {
   if (!c) return MURMUR_ERR_INVALID_ARG;
   c->stats.kernel_launches = 0;
   c->stats.append_calls = c->stats.evict_calls = c->stats.attn_calls = 0;
+  c->stats.host_zero_copy_steps = 0;
   return MURMUR_OK;
 }
 

@@ -345,30 +345,45 @@ def test_config5_full_size_28_layers_full_tensor(dev):
 
 
 # -------------------------------------------------------------------------------- host-buffer entry
-def test_decode_step_host_matches_device_calls(dev):
+@pytest.mark.parametrize("mode", ["pinned_zero_copy", "pinned_packed_staged", "pinned_staged", "pageable"])
+def test_decode_step_host_matches_device_calls(dev, mode):
+    """murmur_decode_step_host from page-locked buffers in place (zero-copy: the kernel reads q / k_new / v_new and
+    writes out through the buffers' device-mapped addresses), from page-locked buffers with zero-copy switched
+    off (staged; packed back to back = one copy), and from pageable buffers (always staged)."""
+    from paper_2606_01483_b200 import binding
+
     cfg = workloads.config1().with_layers(3)
     a = _mk(cfg, dev)
+    if mode in ("pinned_packed_staged", "pinned_staged"):
+        a.gpu.set_option(binding.MURMUR_OPT_HOST_ZERO_COPY, 0)
     a.bulk_prefill([0], 100)
-    for _ in range(3):
+    for _ in range(4):
         u = a.t_of(0)
         k, v = a.data[0].out_kv(u, u + 1)
         q = a.data[0].q_step(u + 1).unsqueeze(1).contiguous()
-        if u % 2:  # packed back to back in one pinned block: moved with a single host-to-device copy
+        if mode == "pinned_packed_staged":  # packed back to back in one pinned block: a single host-to-device copy
             hb = torch.empty(2 * k.numel() + q.numel(), dtype=torch.bfloat16).pin_memory()
             hb[: k.numel()] = k.reshape(-1).cpu()
             hb[k.numel(): 2 * k.numel()] = v.reshape(-1).cpu()
             hb[2 * k.numel():] = q.reshape(-1).cpu()
             kh, vh, qh = hb[: k.numel()].view(k.shape), hb[k.numel(): 2 * k.numel()].view(v.shape), hb[2 * k.numel():].view(q.shape)
+            oh = torch.empty(q.shape, dtype=torch.bfloat16).pin_memory()
+        elif mode == "pageable":
+            kh, vh, qh = k.cpu(), v.cpu(), q.cpu()
+            oh = torch.empty(q.shape, dtype=torch.bfloat16)
         else:
             kh, vh, qh = k.cpu().pin_memory(), v.cpu().pin_memory(), q.cpu().pin_memory()
-        oh = torch.empty(q.shape, dtype=torch.bfloat16).pin_memory()
+            oh = torch.empty(q.shape, dtype=torch.bfloat16).pin_memory()
+        n0 = a.gpu.stats()["host_zero_copy_steps"]
         a.gpu.decode_step_host([0], kh, vh, qh, oh)
         torch.cuda.synchronize()
+        assert a.gpu.stats()["host_zero_copy_steps"] - n0 == (1 if mode == "pinned_zero_copy" else 0)
         a._store(0, k, v)
         a.oracle.append([0], [1])
         a.oracle.evict([0])
         a.check_integer_state([0])
         a.check_attention([0], q, oh.to(dev))
+        a.check_gather(0, layers=None)  # the rows the kernel scattered from the host buffer
     a.close()
 
 
