@@ -25,6 +25,10 @@ What it computes (PAPER.md = /root/reference/PAPER.md):
                      the mass a candidate window policy preserves.
 * ``prefill``      - causal self-attention of the prefill tokens: Eq. 1 of each
                      prefill position over the positions up to and including itself.
+* ``indexset``     - general index-set eviction (the future work of PAPER.md:224): per-(layer, KV head) retained
+                     index sets, dense stable compaction, head-ragged append, Eq. 1 over the slabs, and the
+                     mass-set producer of query-aware sets.  A convention of this build: parity unpinned
+                     against the paper, pinned against its defining properties.
 * ``cost_model``   - Eq. 3 theoretical attention-cost ratio.
 * ``c/``           - a plain C twin of ``attention`` (fp64, optional OpenMP) used for the
                      timed CPU baseline; checked against ``attention`` in tests.
