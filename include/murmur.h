@@ -295,6 +295,62 @@ MURMUR_API murmur_status_t murmur_attn_profile(murmur_cache_t* cache, const int3
                                                void* out, void* scratch, size_t scratch_bytes, int32_t layer_begin,
                                                int32_t layer_end, float sm_scale, void* stream);
 
+/* ---- general index-set eviction: "indexed mode" --------------------------------------------
+ * "The evictable tokens are not contiguous and cannot be captured by a simple positional policy. This motivates
+ * future work on ... query-aware ... eviction policies"; the sparsity is per layer and head
+ * (PAPER.md:29, 77, 99).  These calls are the cache side of such policies (definitions: DESIGN.md "f3" - a
+ * convention of this build, the paper defines none):
+ *   index set     per (layer l, KV head h), an ascending list of ORIGINAL absolute positions to keep;
+ *   indexed mode  the sequence's rows are stored densely per slab (l, h): slot s holds the row of the s-th smallest
+ *                 retained position (dense, stable: order preserved); slabs have different lengths;
+ *   pages         a page id still addresses one logical block in every layer and head, so the sequence keeps blocks
+ *                 0 .. ceil(longest slab / page_size) - 1; surplus pages go back on the free stack, ascending.
+ * A sequence enters indexed mode with its first murmur_kv_evict_indexed and stays there; the positional calls
+ * (murmur_kv_append / _evict / _decode_attn / _decode_step / _prefill_attn / _kv_gather) then return MURMUR_ERR_STATE
+ * for it and the *_indexed calls take over.  murmur_seq_end works in both modes. */
+/* Bytes of the DEVICE buffer murmur_indexed_enable needs (slab lengths + position tables); 0 if unsupported. */
+MURMUR_API size_t murmur_indexed_bytes(const murmur_cache_desc_t* desc);
+/* Hands the handle a caller-owned DEVICE buffer (256-byte aligned, >= murmur_indexed_bytes()) for the indexed-mode
+ * tables; it must outlive the handle.  MURMUR_ERR_STATE while any sequence is in indexed mode. */
+MURMUR_API murmur_status_t murmur_indexed_enable(murmur_cache_t* cache, void* buffer, size_t bytes, void* stream);
+/* Query-aware index sets from the quantity the paper measures (Fig. 5 at PAPER.md:85): for every
+ * (layer, KV head), the union over the query heads of the group of each head's fewest-token set holding >= mass_frac
+ * of its Eq. 1 mass over the resident positions (as murmur_attn_profile finds it), plus both system prompts
+ * (never evicted) and the n_recent newest positions.  `seq` must be positional (not yet indexed).
+ *   q        : DEVICE bf16 [n_layers][n_q_heads][head_dim] (the step's queries of this sequence)
+ *   sel_pos  : DEVICE int32 [n_layers][n_kv_heads][cap] out, ascending;  sel_cnt: DEVICE int32 [n_layers][n_kv_heads] out
+ *   scratch  : DEVICE, >= murmur_select_scratch_bytes()
+ * A set larger than cap raises the device error word (its count is still written). */
+MURMUR_API size_t murmur_select_scratch_bytes(murmur_cache_t* cache, int32_t seq);
+MURMUR_API murmur_status_t murmur_select_mass_sets(murmur_cache_t* cache, int32_t seq, const void* q, float mass_frac,
+                                                   int32_t n_recent, int32_t* sel_pos, int32_t* sel_cnt, int32_t cap,
+                                                   void* scratch, size_t scratch_bytes, float sm_scale, void* stream);
+/* Applies index sets (layouts as above, DEVICE, each set strictly ascending, a subset of what its slab holds, >= 1
+ * element): afterwards slot s of slab (l, h) holds the row of position sel_pos[l][h][s] and everything else is gone.
+ * The compaction is in place (rows only move towards lower addresses); *bytes_moved_out (HOST, may be NULL) = bytes of
+ * K/V rows that changed address - the cost of cache management made countable.  A positional
+ * sequence must have been evicted since its last append (its live page list is the source).  SYNCHRONISES the stream
+ * (the set sizes are read back for the page accounting).  A position that is not held raises the device error word. */
+MURMUR_API murmur_status_t murmur_kv_evict_indexed(murmur_cache_t* cache, int32_t seq, const int32_t* sel_pos,
+                                                   const int32_t* sel_cnt, int32_t cap, int64_t* bytes_moved_out,
+                                                   void* stream);
+/* Appends ONE token to every slab of every listed (indexed-mode) sequence; its original position is the sequence's
+ * running token count.  A page is popped when a sequence's longest slab starts a new block (call order; all-or-nothing).
+ *   k_new, v_new : DEVICE bf16 [n_layers][n_seqs][n_kv_heads][head_dim] */
+MURMUR_API murmur_status_t murmur_kv_append_indexed(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                                    const void* k_new, const void* v_new, void* stream);
+/* Eq. 1 of every query head hq over the rows of slab (l, hq / group), all layers.
+ *   q, out : DEVICE bf16 [n_layers][n_seqs][n_q_heads][head_dim];  lse: DEVICE fp32 [n_layers][n_seqs][n_q_heads] or NULL
+ * First path (FFMA straight from the pool); the tensor-core streaming kernel serves the positional mode. */
+MURMUR_API murmur_status_t murmur_decode_attn_indexed(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                                      const void* q, void* out, float* lse, float sm_scale, void* stream);
+/* Introspection (synchronise): the original positions held by slab (layer, kv_head), by slot; and the rows of every
+ * slab by slot, k_out / v_out DEVICE bf16 [n_layers][n_kv_heads][cap_rows][head_dim] (zero beyond a slab's length). */
+MURMUR_API murmur_status_t murmur_kv_get_indexed(murmur_cache_t* cache, int32_t seq, int32_t layer, int32_t kv_head,
+                                                 int32_t* pos_out, int32_t cap, int32_t* n_out, void* stream);
+MURMUR_API murmur_status_t murmur_kv_gather_indexed(murmur_cache_t* cache, int32_t seq, void* k_out, void* v_out,
+                                                    int32_t cap_rows, void* stream);
+
 /* ---- introspection (tests; each call synchronises the stream it is given) ------------------ */
 /* state_out[0..5] = length, t, n_live_blocks, n_runs, n_attn_tiles, n_retained (device values). */
 MURMUR_API murmur_status_t murmur_seq_get_state(murmur_cache_t* cache, int32_t seq, int32_t* state_out, void* stream);

@@ -37,6 +37,9 @@ EXPORTED_SYMBOLS = [
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
     "murmur_profile_scratch_bytes", "murmur_attn_profile",
     "murmur_decode_attn_windowed", "murmur_prefill_attn", "murmur_chunk_plan",
+    "murmur_indexed_bytes", "murmur_indexed_enable", "murmur_select_scratch_bytes", "murmur_select_mass_sets",
+    "murmur_kv_evict_indexed", "murmur_kv_append_indexed", "murmur_decode_attn_indexed", "murmur_kv_get_indexed",
+    "murmur_kv_gather_indexed",
     "murmur_set_option", "murmur_get_stats", "murmur_reset_stats", "murmur_status_str",
     "murmur_last_cuda_error", "murmur_version",
 ]
@@ -111,6 +114,17 @@ def lib() -> C.CDLL:
     L.murmur_profile_scratch_bytes.argtypes = [vp, vp, i32, i32, i32]
     L.murmur_profile_scratch_bytes.restype = C.c_size_t
     L.murmur_attn_profile.argtypes = [vp, vp, i32, vp, vp, C.c_float, vp, vp, C.c_size_t, i32, i32, C.c_float, vp]
+    L.murmur_indexed_bytes.restype = C.c_size_t
+    L.murmur_indexed_bytes.argtypes = [C.POINTER(CacheDesc)]
+    L.murmur_indexed_enable.argtypes = [vp, vp, C.c_size_t, vp]
+    L.murmur_select_scratch_bytes.restype = C.c_size_t
+    L.murmur_select_scratch_bytes.argtypes = [vp, i32]
+    L.murmur_select_mass_sets.argtypes = [vp, i32, vp, C.c_float, i32, vp, vp, i32, vp, C.c_size_t, C.c_float, vp]
+    L.murmur_kv_evict_indexed.argtypes = [vp, i32, vp, vp, i32, vp, vp]
+    L.murmur_kv_append_indexed.argtypes = [vp, vp, i32, vp, vp, vp]
+    L.murmur_decode_attn_indexed.argtypes = [vp, vp, i32, vp, vp, vp, C.c_float, vp]
+    L.murmur_kv_get_indexed.argtypes = [vp, i32, i32, i32, vp, i32, vp, vp]
+    L.murmur_kv_gather_indexed.argtypes = [vp, i32, vp, vp, i32, vp]
     L.murmur_set_option.argtypes = [vp, i32, i32]
     L.murmur_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.murmur_reset_stats.argtypes = [vp]
@@ -312,6 +326,71 @@ class MurmurCache:
         self._check(self.L.murmur_decode_step_host(self.h, ids.ctypes.data, len(ids), k_new.data_ptr(),
                                                    v_new.data_ptr(), q.data_ptr(), out.data_ptr(),
                                                    C.c_float(sm_scale), _stream()))
+
+    # ---- general index-set eviction (indexed mode) ------------------------------------------
+    def indexed_enable(self):
+        """Allocates the indexed-mode tables (a torch tensor owned by this object) and hands them to the handle."""
+        n = self.L.murmur_indexed_bytes(C.byref(self.desc))
+        self.indexed_buf = torch.empty(n, dtype=torch.uint8, device=self.device)
+        self._check(self.L.murmur_indexed_enable(self.h, self.indexed_buf.data_ptr(), n, _stream()))
+
+    def select_mass_sets(self, seq: int, q: torch.Tensor, mass_frac: float, n_recent: int, cap: int,
+                         sm_scale: Optional[float] = None) -> Tuple[torch.Tensor, torch.Tensor]:
+        """Query-aware index sets of one positional sequence: (sel_pos int32 [L, n_kv, cap], sel_cnt int32 [L, n_kv]) on the device."""
+        assert q.dtype == torch.bfloat16 and q.is_cuda and q.is_contiguous() and tuple(q.shape) == (self.n_layers, self.n_q, self.d)
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        nb = self.L.murmur_select_scratch_bytes(self.h, seq)
+        if nb == 0:
+            raise MurmurError(2, "murmur_select_scratch_bytes: sequence not active or already indexed")
+        scratch = torch.empty(nb, dtype=torch.uint8, device=self.device)
+        sel_pos = torch.zeros(self.n_layers, self.n_kv, cap, dtype=torch.int32, device=self.device)
+        sel_cnt = torch.zeros(self.n_layers, self.n_kv, dtype=torch.int32, device=self.device)
+        self._check(self.L.murmur_select_mass_sets(self.h, seq, q.data_ptr(), C.c_float(mass_frac), n_recent, sel_pos.data_ptr(),
+                                                   sel_cnt.data_ptr(), cap, scratch.data_ptr(), nb, C.c_float(sm_scale), _stream()))
+        torch.cuda.synchronize(self.device)
+        return sel_pos, sel_cnt
+
+    def kv_evict_indexed(self, seq: int, sel_pos: torch.Tensor, sel_cnt: torch.Tensor) -> int:
+        """Applies per-(layer, KV head) index sets (device int32 tensors); returns the bytes of K/V rows moved."""
+        assert sel_pos.dtype == torch.int32 and sel_pos.is_cuda and sel_pos.is_contiguous() and sel_pos.dim() == 3
+        assert sel_cnt.dtype == torch.int32 and sel_cnt.is_cuda and sel_cnt.is_contiguous()
+        assert tuple(sel_pos.shape[:2]) == (self.n_layers, self.n_kv) == tuple(sel_cnt.shape)
+        moved = C.c_int64(0)
+        self._check(self.L.murmur_kv_evict_indexed(self.h, seq, sel_pos.data_ptr(), sel_cnt.data_ptr(), sel_pos.shape[2],
+                                                   C.byref(moved), _stream()))
+        return moved.value
+
+    def kv_append_indexed(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor):
+        ids = _ids(seq_ids)
+        for t in (k_new, v_new):
+            assert t.dtype == torch.bfloat16 and t.is_cuda and t.is_contiguous()
+            assert tuple(t.shape) == (self.n_layers, len(ids), self.n_kv, self.d)
+        self._check(self.L.murmur_kv_append_indexed(self.h, ids.ctypes.data, len(ids), k_new.data_ptr(), v_new.data_ptr(), _stream()))
+
+    def decode_attn_indexed(self, seq_ids, q: torch.Tensor, lse: Optional[torch.Tensor] = None,
+                            sm_scale: Optional[float] = None) -> torch.Tensor:
+        ids = _ids(seq_ids)
+        shape = (self.n_layers, len(ids), self.n_q, self.d)
+        assert q.dtype == torch.bfloat16 and q.is_cuda and q.is_contiguous() and tuple(q.shape) == shape
+        out = torch.empty(shape, dtype=torch.bfloat16, device=self.device)
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        self._check(self.L.murmur_decode_attn_indexed(self.h, ids.ctypes.data, len(ids), q.data_ptr(), out.data_ptr(),
+                                                      lse.data_ptr() if lse is not None else None, C.c_float(sm_scale), _stream()))
+        return out
+
+    def indexed_positions(self, seq: int, layer: int, kv_head: int) -> np.ndarray:
+        cap = self.max_blocks * self.page_size
+        a = np.zeros(cap, dtype=np.int32)
+        n = C.c_int32(0)
+        self._check(self.L.murmur_kv_get_indexed(self.h, seq, layer, kv_head, a.ctypes.data, cap, C.byref(n), _stream()))
+        return a[: n.value].copy()
+
+    def gather_indexed(self, seq: int, cap_rows: int) -> Tuple[torch.Tensor, torch.Tensor]:
+        shape = (self.n_layers, self.n_kv, cap_rows, self.d)
+        k = torch.empty(shape, dtype=torch.bfloat16, device=self.device)
+        v = torch.empty(shape, dtype=torch.bfloat16, device=self.device)
+        self._check(self.L.murmur_kv_gather_indexed(self.h, seq, k.data_ptr(), v.data_ptr(), cap_rows, _stream()))
+        return k, v
 
     # ---- introspection ------------------------------------------------------------------
     def seq_state(self, seq: int) -> dict:

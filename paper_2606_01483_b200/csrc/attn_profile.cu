@@ -39,6 +39,7 @@ struct ProfParams {
   int seq_base, n_seqs_total, layer_begin;
   float sm_scale, frac;
   int use_candidate;
+  uint8_t* member;  // optional [CTA][stride]: 1 where the position is in the mass set of any head of the group
   SeqParams cand;  // policy fields only (P, S, M, len are taken from the sequence)
 };
 
@@ -138,6 +139,10 @@ attn_profile_kernel(const __grid_constant__ CacheView c, const __grid_constant__
   const int per = (len + kProfThreads - 1) / kProfThreads;
   const int x0 = min(len, tid * per), x1 = min(len, x0 + per);
 
+  uint8_t* member = prm.member != nullptr ? prm.member + cta * (size_t)prm.stride : nullptr;
+  if (member != nullptr)
+    for (int x = x0; x < x1; ++x) member[x] = 0;  // each thread owns the positions [x0, x1) throughout
+
   for (int h = 0; h < G; ++h) {
     float* e = sc + (size_t)h * prm.stride;
     // ---- pass 2: softmax numerators, total, region masses, candidate coverage ----
@@ -192,6 +197,7 @@ attn_profile_kernel(const __grid_constant__ CacheView c, const __grid_constant__
       if (key > tau) {
         gt[region_of(x, sp.P, sp.S, sp.M)] += 1.0;
         gt[3] += (double)w;
+        if (member != nullptr) member[x] = 1;
       } else if (key == tau) {
         ++ties;
       }
@@ -223,12 +229,13 @@ attn_profile_kernel(const __grid_constant__ CacheView c, const __grid_constant__
         const float w = e[x];
         if (w >= 0.f && __float_as_uint(w) == tau) {
           tk[region_of(x, sp.P, sp.S, sp.M)] += 1.0;
+          if (member != nullptr) member[x] = 1;
           ++rank;
         }
       }
     }
     block_sum4(tk, s_red);
-    if (tid == 0) {
+    if (tid == 0 && prm.out != nullptr) {
       murmur_profile_t r;
       r.n_prompt = (int32_t)cd[0];
       r.n_speech = (int32_t)cd[1];
@@ -252,8 +259,10 @@ attn_profile_kernel(const __grid_constant__ CacheView c, const __grid_constant__
 
 cudaError_t launch_attn_profile(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                                 const SeqParams* candidate, float frac, void* out, float* scratch, long long stride,
-                                int layer_begin, int layer_end, float sm_scale, cudaStream_t st, LaunchInfo* info) {
+                                int layer_begin, int layer_end, float sm_scale, uint8_t* member_mask, cudaStream_t st,
+                                LaunchInfo* info) {
   ProfParams prm{};
+  prm.member = member_mask;
   prm.q = reinterpret_cast<const uint16_t*>(q);
   prm.out = reinterpret_cast<murmur_profile_t*>(out);
   prm.scratch = scratch;

@@ -62,7 +62,11 @@ struct SeqDev {  // 320 bytes
   // the next decode step (which attends at L + 1) finds its table ready and only copies it.
   TileGen tg[2];
   int32_t tg_len[2];
-  int32_t pad[4];
+  // indexed mode (kv_indexed.cu): rows stored densely per (layer, KV head) slab; blocks 0 .. idx_blocks-1 mapped
+  int32_t idx_mode;      // 1: the sequence is in indexed mode (the positional fields above no longer apply)
+  int32_t idx_blocks;    // logical blocks mapped
+  int32_t idx_next_pos;  // original position the next appended token gets
+  int32_t idx_max_len;   // rows of the longest slab
 };
 static_assert(sizeof(SeqDev) == 320, "SeqDev must be 320 bytes");
 
@@ -112,6 +116,15 @@ __device__ __forceinline__ void step_stamp(const CacheView& c, int k) {
 #endif
 }
 #endif
+
+// Indexed-mode tables, in a caller-provided device buffer (murmur_indexed_enable):
+//   len [max_seqs][n_layers * n_kv]        rows of each slab
+//   pos [max_seqs][n_layers * n_kv][cap]   original position of the row in each slot (ascending), cap = max_blocks * p
+struct IdxView {
+  int32_t* len;
+  int32_t* pos;
+  int32_t cap;
+};
 
 struct SeqList {  // per-launch sequence list, passed by value (no H2D copy, graph-capturable)
   int32_t n;
@@ -206,9 +219,24 @@ cudaError_t launch_prefill_attn(const CacheView& c, int seq, int pos_begin, int 
 cudaError_t launch_prefill_attn_umma(const CacheView& c, int seq, int pos_begin, int n_tok, const void* q, void* out,
                                      float* lse, int layer_begin, int layer_end, float sm_scale, cudaStream_t st,
                                      LaunchInfo* info);
+// member_mask (optional): uint8 [layers][n_seqs][n_kv][stride], set to 1 at the positions that belong to the mass
+// set of ANY query head of the group; out may then be null.
 cudaError_t launch_attn_profile(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                                 const SeqParams* candidate, float frac, void* out, float* scratch, long long stride,
-                                int layer_begin, int layer_end, float sm_scale, cudaStream_t st, LaunchInfo* info);
+                                int layer_begin, int layer_end, float sm_scale, uint8_t* member_mask, cudaStream_t st,
+                                LaunchInfo* info);
+cudaError_t launch_indexed_defrag(const CacheView& c, const IdxView& ix, int seq, const int32_t* sel_pos, const int32_t* sel_cnt,
+                                  int cap_sel, bool from_positional, unsigned long long* moved_dev, cudaStream_t st,
+                                  LaunchInfo* info);
+cudaError_t launch_indexed_append(const CacheView& c, const IdxView& ix, const SeqList& list, const void* k_new,
+                                  const void* v_new, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_indexed_attn(const CacheView& c, const IdxView& ix, const SeqList& list, const void* q, void* out,
+                                float* lse, float sm_scale, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_indexed_gather(const CacheView& c, const IdxView& ix, int seq, void* k_out, void* v_out, int cap_out,
+                                  cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_indexed_seq_end(const CacheView& c, int seq, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_select_compact(const CacheView& c, int seq, const uint8_t* mask, long long mask_stride, int n_recent,
+                                  int32_t* sel_pos, int32_t* sel_cnt, int cap_sel, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_expand_retained(const CacheView& c, int seq, int32_t* pos_out_dev, int cap, cudaStream_t st,
                                    LaunchInfo* info);
 cudaError_t launch_gather(const CacheView& c, int seq, const int32_t* positions_dev, int n, int layer_begin,

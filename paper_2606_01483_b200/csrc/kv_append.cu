@@ -43,6 +43,7 @@ __global__ void seq_begin_kernel(CacheView c, int seq, SeqParams sp) {
     s.active = 1;
     s.n_live = 0; s.n_runs = 0; s.n_tiles = 0; s.n_retained = 0;
     s.tg_len[0] = s.tg_len[1] = -1;
+    s.idx_mode = 0; s.idx_blocks = 0; s.idx_next_pos = 0; s.idx_max_len = 0;
   }
 }
 

@@ -39,6 +39,9 @@ struct HostSeq {
   SeqParams sp{};
   int32_t evict_len = -1;   // length when murmur_kv_evict last ran (-1: never)
   int32_t freed_blocks = 0;  // blocks of this sequence returned to the pool so far
+  bool indexed = false;      // indexed mode (kv_indexed.cu): the positional fields above are frozen
+  int32_t idx_blocks = 0;    // blocks mapped in indexed mode
+  int32_t idx_max_len = 0;   // rows of the longest slab
 };
 
 constexpr size_t kAlign = 256;
@@ -115,6 +118,8 @@ struct murmur_cache {
   murmur_stats_t stats;
   cudaError_t last_cuda;
   uint8_t* ws;
+  IdxView idx{nullptr, nullptr, 0};        // indexed-mode tables (murmur_indexed_enable)
+  unsigned long long* idx_moved = nullptr;  // device counter of rows moved by the last index-set eviction
 };
 
 namespace {
@@ -134,8 +139,8 @@ void note(murmur_cache* c, const LaunchInfo& li) { c->stats.kernel_launches += l
 
 inline int32_t blocks_for(int32_t len, int32_t p) { return (len + p - 1) / p; }
 
-// ids in range, active, distinct
-murmur_status_t check_ids(murmur_cache* c, const int32_t* ids, int32_t n) {
+// ids in range, active, distinct; want_indexed: 0 = positional sequences only, 1 = indexed-mode sequences only
+murmur_status_t check_ids(murmur_cache* c, const int32_t* ids, int32_t n, int want_indexed = 0) {
   if (!ids || n < 0) return MURMUR_ERR_INVALID_ARG;
   for (int i = 0; i < n; ++i) {
     if (ids[i] < 0 || ids[i] >= c->desc.max_seqs) return MURMUR_ERR_INVALID_ARG;
@@ -143,7 +148,7 @@ murmur_status_t check_ids(murmur_cache* c, const int32_t* ids, int32_t n) {
       if (ids[j] == ids[i]) return MURMUR_ERR_INVALID_ARG;
   }
   for (int i = 0; i < n; ++i)
-    if (!c->seqs[ids[i]].active) return MURMUR_ERR_STATE;
+    if (!c->seqs[ids[i]].active || (int)c->seqs[ids[i]].indexed != want_indexed) return MURMUR_ERR_STATE;
   return MURMUR_OK;
 }
 
@@ -260,6 +265,14 @@ murmur_status_t murmur_seq_end(murmur_cache_t* c, int32_t seq, void* stream) {
   HostSeq& hs = c->seqs[seq];
   if (!hs.active) return MURMUR_ERR_STATE;
   LaunchInfo li{};
+  if (hs.indexed) {
+    MM_CUDA(c, launch_indexed_seq_end(c->view, seq, (cudaStream_t)stream, &li));
+    note(c, li);
+    c->free_pages += hs.idx_blocks;
+    c->stats.free_pages = c->free_pages;
+    hs = HostSeq();
+    return MURMUR_OK;
+  }
   MM_CUDA(c, launch_seq_end(c->view, seq, (cudaStream_t)stream, &li));
   note(c, li);
   c->free_pages += blocks_for(hs.sp.len, c->desc.page_size) - hs.freed_blocks;
@@ -625,6 +638,7 @@ murmur_status_t murmur_prefill_attn(murmur_cache_t* c, int32_t seq, int32_t pos_
   if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
   if (c->desc.page_size < 16) return MURMUR_ERR_UNSUPPORTED;
   const HostSeq& hs = c->seqs[seq];
+  if (hs.indexed) return MURMUR_ERR_STATE;
   if (pos_begin < 0 || pos_begin >= pos_end || pos_end > hs.sp.len) return MURMUR_ERR_INVALID_ARG;
   if (hs.freed_blocks != 0) return MURMUR_ERR_STATE;  // something below pos_end may be gone
   LaunchInfo li{};
@@ -680,8 +694,180 @@ murmur_status_t murmur_attn_profile(murmur_cache_t* c, const int32_t* seq_ids, i
   LaunchInfo li{};
   MM_CUDA(c, launch_attn_profile(c->view, list, 0, n_seqs, q, cand ? &cs : nullptr, mass_frac, out,
                                  reinterpret_cast<float*>(scratch), profile_stride(c, seq_ids, n_seqs), layer_begin,
-                                 layer_end, sm_scale, (cudaStream_t)stream, &li));
+                                 layer_end, sm_scale, nullptr, (cudaStream_t)stream, &li));
   note(c, li);
+  return MURMUR_OK;
+}
+
+
+// ---- general index-set eviction (indexed mode) ------------------------------------------------------
+static size_t idx_len_bytes(const murmur_cache_desc_t* d) {
+  return align_up((size_t)d->max_seqs * d->n_layers * d->n_kv_heads * 4);
+}
+
+size_t murmur_indexed_bytes(const murmur_cache_desc_t* d) {
+  if (!geometry_ok(d)) return 0;
+  const size_t cap = (size_t)d->max_blocks_per_seq * d->page_size;
+  return kAlign + idx_len_bytes(d) + align_up((size_t)d->max_seqs * d->n_layers * d->n_kv_heads * cap * 4);
+}
+
+murmur_status_t murmur_indexed_enable(murmur_cache_t* c, void* buffer, size_t bytes, void* stream) {
+  if (!c || !buffer) return MURMUR_ERR_INVALID_ARG;
+  if (((uintptr_t)buffer & (kAlign - 1)) || bytes < murmur_indexed_bytes(&c->desc)) return MURMUR_ERR_INVALID_ARG;
+  for (const HostSeq& hs : c->seqs)
+    if (hs.indexed) return MURMUR_ERR_STATE;  // tables in use
+  uint8_t* b = reinterpret_cast<uint8_t*>(buffer);
+  MM_CUDA(c, cudaMemsetAsync(b, 0, kAlign + idx_len_bytes(&c->desc), (cudaStream_t)stream));
+  c->idx_moved = reinterpret_cast<unsigned long long*>(b);
+  c->idx.len = reinterpret_cast<int32_t*>(b + kAlign);
+  c->idx.pos = reinterpret_cast<int32_t*>(b + kAlign + idx_len_bytes(&c->desc));
+  c->idx.cap = c->desc.max_blocks_per_seq * c->desc.page_size;
+  return MURMUR_OK;
+}
+
+size_t murmur_select_scratch_bytes(murmur_cache_t* c, int32_t seq) {
+  if (check_seq(c, seq) != MURMUR_OK || c->seqs[seq].indexed) return 0;
+  const size_t stride = (size_t)profile_stride(c, &seq, 1);
+  return (size_t)c->desc.n_layers * c->desc.n_q_heads * stride * 4 + align_up((size_t)c->desc.n_layers * c->desc.n_kv_heads * stride);
+}
+
+murmur_status_t murmur_select_mass_sets(murmur_cache_t* c, int32_t seq, const void* q, float mass_frac, int32_t n_recent,
+                                        int32_t* sel_pos, int32_t* sel_cnt, int32_t cap, void* scratch, size_t scratch_bytes,
+                                        float sm_scale, void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!q || !sel_pos || !sel_cnt || !scratch || cap < 1 || n_recent < 0) return MURMUR_ERR_INVALID_ARG;
+  if (!(sm_scale > 0.f) || !(mass_frac > 0.f) || mass_frac > 1.f) return MURMUR_ERR_INVALID_ARG;
+  const HostSeq& hs = c->seqs[seq];
+  if (hs.indexed || hs.sp.len < 1) return MURMUR_ERR_STATE;  // sets are selected over a positional cache
+  if (scratch_bytes < murmur_select_scratch_bytes(c, seq)) return MURMUR_ERR_INVALID_ARG;
+  const long long stride = profile_stride(c, &seq, 1);
+  float* sc = reinterpret_cast<float*>(scratch);
+  uint8_t* mask = reinterpret_cast<uint8_t*>(scratch) + (size_t)c->desc.n_layers * c->desc.n_q_heads * (size_t)stride * 4;
+  SeqList list;
+  list.n = 1;
+  list.ids[0] = seq;
+  LaunchInfo li{};
+  MM_CUDA(c, launch_attn_profile(c->view, list, 0, 1, q, nullptr, mass_frac, nullptr, sc, stride, 0, c->desc.n_layers,
+                                 sm_scale, mask, (cudaStream_t)stream, &li));
+  MM_CUDA(c, launch_select_compact(c->view, seq, mask, stride, n_recent, sel_pos, sel_cnt, cap, (cudaStream_t)stream, &li));
+  note(c, li);
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_evict_indexed(murmur_cache_t* c, int32_t seq, const int32_t* sel_pos, const int32_t* sel_cnt,
+                                        int32_t cap, int64_t* bytes_moved_out, void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!sel_pos || !sel_cnt || cap < 1) return MURMUR_ERR_INVALID_ARG;
+  if (!c->idx.pos) return MURMUR_ERR_STATE;  // murmur_indexed_enable first
+  HostSeq& hs = c->seqs[seq];
+  if (!hs.indexed && (hs.sp.len < 1 || hs.evict_len != hs.sp.len)) return MURMUR_ERR_STATE;  // live page list must be current
+  cudaStream_t s = (cudaStream_t)stream;
+  const int n_slabs = c->desc.n_layers * c->desc.n_kv_heads;
+  std::vector<int32_t> cnt(n_slabs);
+  MM_CUDA(c, cudaMemcpyAsync(cnt.data(), sel_cnt, (size_t)n_slabs * 4, cudaMemcpyDeviceToHost, s));
+  MM_CUDA(c, cudaStreamSynchronize(s));
+  const int32_t held = hs.indexed ? hs.idx_max_len : hs.sp.len;  // a slab cannot grow by eviction
+  int32_t mx = 0;
+  for (int i = 0; i < n_slabs; ++i) {
+    if (cnt[i] < 1 || cnt[i] > cap || cnt[i] > held) return MURMUR_ERR_INVALID_ARG;
+    mx = cnt[i] > mx ? cnt[i] : mx;
+  }
+  const int32_t p = c->desc.page_size;
+  const int32_t blocks_held = hs.indexed ? hs.idx_blocks : blocks_for(hs.sp.len, p) - hs.freed_blocks;
+  const int32_t nb_new = blocks_for(mx, p);
+  if (nb_new > blocks_held) return MURMUR_ERR_INVALID_ARG;
+  MM_CUDA(c, cudaMemsetAsync(c->idx_moved, 0, 8, s));
+  LaunchInfo li{};
+  MM_CUDA(c, launch_indexed_defrag(c->view, c->idx, seq, sel_pos, sel_cnt, cap, !hs.indexed, c->idx_moved, s, &li));
+  note(c, li);
+  unsigned long long moved = 0;
+  MM_CUDA(c, cudaMemcpyAsync(&moved, c->idx_moved, 8, cudaMemcpyDeviceToHost, s));
+  MM_CUDA(c, cudaStreamSynchronize(s));
+  if (bytes_moved_out) *bytes_moved_out = (int64_t)moved * 2 * kRowBytes;
+  c->free_pages += blocks_held - nb_new;
+  c->stats.free_pages = c->free_pages;
+  hs.indexed = true;
+  hs.idx_blocks = nb_new;
+  hs.idx_max_len = mx;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_append_indexed(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* k_new,
+                                         const void* v_new, void* stream) {
+  if (!c || !k_new || !v_new) return MURMUR_ERR_INVALID_ARG;
+  if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs, 1);
+  if (st != MURMUR_OK) return st;
+  const int32_t p = c->desc.page_size;
+  int64_t need = 0;
+  for (int i = 0; i < n_seqs; ++i) {
+    const HostSeq& hs = c->seqs[seq_ids[i]];
+    if (hs.idx_max_len + 1 > c->idx.cap) return MURMUR_ERR_STATE;
+    need += blocks_for(hs.idx_max_len + 1, p) - hs.idx_blocks;
+  }
+  if (need > c->free_pages) return MURMUR_ERR_OOM_PAGES;  // all-or-nothing
+  SeqList list;
+  list.n = n_seqs;
+  for (int i = 0; i < n_seqs; ++i) list.ids[i] = seq_ids[i];
+  LaunchInfo li{};
+  MM_CUDA(c, launch_indexed_append(c->view, c->idx, list, k_new, v_new, (cudaStream_t)stream, &li));
+  note(c, li);
+  for (int i = 0; i < n_seqs; ++i) {
+    HostSeq& hs = c->seqs[seq_ids[i]];
+    hs.idx_blocks = blocks_for(hs.idx_max_len + 1, p);
+    hs.idx_max_len += 1;
+  }
+  c->free_pages -= need;
+  c->stats.free_pages = c->free_pages;
+  c->stats.append_calls += 1;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_decode_attn_indexed(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q,
+                                           void* out, float* lse, float sm_scale, void* stream) {
+  if (!c || !q || !out) return MURMUR_ERR_INVALID_ARG;
+  if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch || !(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs, 1);
+  if (st != MURMUR_OK) return st;
+  SeqList list;
+  list.n = n_seqs;
+  for (int i = 0; i < n_seqs; ++i) list.ids[i] = seq_ids[i];
+  LaunchInfo li{};
+  MM_CUDA(c, launch_indexed_attn(c->view, c->idx, list, q, out, lse, sm_scale, (cudaStream_t)stream, &li));
+  note(c, li);
+  c->stats.attn_calls += 1;
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_get_indexed(murmur_cache_t* c, int32_t seq, int32_t layer, int32_t kv_head, int32_t* pos_out,
+                                      int32_t cap, int32_t* n_out, void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!c->seqs[seq].indexed) return MURMUR_ERR_STATE;
+  if (!n_out || cap < 0 || (cap > 0 && !pos_out)) return MURMUR_ERR_INVALID_ARG;
+  if (layer < 0 || layer >= c->desc.n_layers || kv_head < 0 || kv_head >= c->desc.n_kv_heads) return MURMUR_ERR_INVALID_ARG;
+  MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  const size_t slab = (size_t)seq * c->desc.n_layers * c->desc.n_kv_heads + (size_t)layer * c->desc.n_kv_heads + kv_head;
+  int32_t n = 0;
+  MM_CUDA(c, cudaMemcpy(&n, c->idx.len + slab, 4, cudaMemcpyDeviceToHost));
+  *n_out = n;
+  if (n > cap) return MURMUR_ERR_INVALID_ARG;
+  if (n > 0) MM_CUDA(c, cudaMemcpy(pos_out, c->idx.pos + slab * c->idx.cap, (size_t)n * 4, cudaMemcpyDeviceToHost));
+  return MURMUR_OK;
+}
+
+murmur_status_t murmur_kv_gather_indexed(murmur_cache_t* c, int32_t seq, void* k_out, void* v_out, int32_t cap_rows,
+                                         void* stream) {
+  murmur_status_t st = check_seq(c, seq);
+  if (st != MURMUR_OK) return st;
+  if (!c->seqs[seq].indexed) return MURMUR_ERR_STATE;
+  if (!k_out || !v_out || cap_rows < 1) return MURMUR_ERR_INVALID_ARG;
+  LaunchInfo li{};
+  MM_CUDA(c, launch_indexed_gather(c->view, c->idx, seq, k_out, v_out, cap_rows, (cudaStream_t)stream, &li));
+  note(c, li);
+  MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
   return MURMUR_OK;
 }
 
@@ -786,6 +972,7 @@ murmur_status_t murmur_kv_gather(murmur_cache_t* c, int32_t seq, const int32_t* 
                                  int32_t layer_begin, int32_t layer_end, void* k_out, void* v_out, void* stream) {
   murmur_status_t st = check_seq(c, seq);
   if (st != MURMUR_OK) return st;
+  if (c->seqs[seq].indexed) return MURMUR_ERR_STATE;  // rows are addressed by slot there: murmur_kv_gather_indexed
   if (!positions || n < 0 || !k_out || !v_out) return MURMUR_ERR_INVALID_ARG;
   if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
   if ((size_t)n > c->cv.scratch_ints) return MURMUR_ERR_INVALID_ARG;
