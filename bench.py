@@ -131,6 +131,17 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
+    def wait_ready(self, timeout_s: float = 3.0):
+        """Blocks until the sampler process has written its first sample (it takes ~0.1-0.5 s to start)."""
+        t_end = time.time() + timeout_s
+        while self.proc is not None and time.time() < t_end:
+            try:
+                if os.path.getsize(self.path) > 0:
+                    return
+            except OSError:
+                pass
+            time.sleep(0.01)
+
     def window(self, t0: float, t1: float, tag: str = "main"):
         self.windows.setdefault(tag, []).append((t0, t1))
 
@@ -566,6 +577,8 @@ def run_murmur(args):
         torch.cuda.synchronize(dev)
 
     sampler = ClockSampler(local_rank) if rank == 0 else None
+    if sampler:
+        sampler.wait_ready()
     spin_up(wb, torch)
     for _ in range(W):
         wb.step()
@@ -718,7 +731,7 @@ def run_murmur(args):
                 "frac_of_nominal_8000": achieved / 8000.0}
 
     # ---- oracle: parity of the timed outputs, CPU baseline, replay, protocol, other workloads -----
-    cpu_baseline = parity = replay = protocol = others = None
+    cpu_baseline = parity = replay = protocol = others = index_sets = None
     if check:
         import workloads
         from oracle import c as oracle_c
@@ -782,6 +795,7 @@ def run_murmur(args):
             others = {}
             for name in OTHER_WORKLOADS:
                 others[name] = run_other_workload(name, dev, sampler, peak, True, torch)
+            index_sets = run_index_set_eviction(dev, torch)
     else:
         wb_err = cache.last_error()
         wb.close()
@@ -812,7 +826,7 @@ def run_murmur(args):
                                   "also reserves, commits and evicts)"},
         "step_hbm_gbs": alg_bytes / (us_step * 1e-6) / 1e9,
         "roofline": roofline, "cpu_baseline": cpu_baseline, "parity": parity, "parity_last_step": parity,
-        "replay": replay, "protocol": protocol, "other_workloads": others,
+        "replay": replay, "protocol": protocol, "other_workloads": others, "index_set_eviction": index_sets,
         "e2e": {"value": us_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "device_us": us_e2e_dev, "wall_us": us_e2e_wall, "steps": Ke, "launches_per_step": e2e_launches,
                 "path": ("zero-copy: the step kernel reads k_new / v_new / q from the pinned host buffers and stores out to the "
@@ -877,6 +891,212 @@ def run_protocol(cfg, dev, torch) -> dict:
             "wall_s_gpu_loop": gpu_s}
 
 
+def run_index_set_eviction(dev, torch) -> dict:
+    """SURVEY 8f-3 on the config-2 shape: query-aware index sets (>= 99 % of every query head's Eq. 1 mass, both
+    prompts, the 16 newest positions) for every sequence of an un-evicted cache, applied by the in-place dense
+    compaction; reports the bytes the compaction moved next to the bytes it retains, and checks sequence 0's slabs
+    and attention against oracle/indexset.py."""
+    import numpy as np
+
+    import workloads
+    from oracle import indexset as o_ix
+    from oracle import paged_cache as o_cache
+    from oracle import policy as o_policy
+
+    W = workloads.WINDOW_OFF
+    cfg = workloads.config2(W, W)
+    t0 = 300
+    wb = Workbench(cfg, t0, 2, dev)
+    g = cfg.geom
+    L, H = g.n_layers, g.n_kv_heads
+    wb.cache.indexed_enable()
+    n = cfg.seqs[0].P + cfg.seqs[0].S + cfg.seqs[0].M + t0
+    frac, n_recent = 0.99, 16
+    e0, e1, e2, e3 = (torch.cuda.Event(enable_timing=True) for _ in range(4))
+    stream = torch.cuda.current_stream()
+    sets = []
+    torch.cuda.synchronize(dev)
+    e0.record(stream)
+    for i in range(cfg.batch):
+        sets.append(wb.cache.select_mass_sets(i, wb.data[i].q_step(t0).contiguous(), frac, n_recent, cap=n, sm_scale=wb.scale))
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    moved = 0
+    t_def = time.perf_counter()
+    for i in range(cfg.batch):
+        moved += wb.cache.kv_evict_indexed(i, sets[i][0], sets[i][1])
+    t_def = time.perf_counter() - t_def
+    rows = sum(int(sets[i][1].sum()) for i in range(cfg.batch))
+    q = wb.q_all[0]  # [L, B, n_q, d]: the queries of step t0 + 1 (any queries do for a timing + parity check)
+    for _ in range(3):
+        out = wb.cache.decode_attn_indexed(wb.ids, q, sm_scale=wb.scale)
+    torch.cuda.synchronize(dev)
+    e2.record(stream)
+    for _ in range(10):
+        out = wb.cache.decode_attn_indexed(wb.ids, q, sm_scale=wb.scale)
+    e3.record(stream)
+    torch.cuda.synchronize(dev)
+    # parity of sequence 0 against the oracle, with the sets the GPU selected
+    oc = o_cache.OraclePagedCache(wb.n_pages, cfg.page_size, cfg.batch, wb.max_blocks)
+    s0 = cfg.seqs[0]
+    oc.seq_begin(0, s0.P, s0.S, s0.M, o_policy.Policy(*s0.policy_tuple))
+    oc.append([0], [n])
+    oc.evict([0])
+    oix = o_ix.OracleIndexedCache(oc, L, H)
+    sel = [[sets[0][0][l, h, : int(sets[0][1][l, h])].cpu().tolist() for h in range(H)] for l in range(L)]
+    oix.evict_indexed(0, sel)
+    kb, vb = wb.host_kv(0, 0)
+    gk, gv = wb.cache.gather_indexed(0, oix.seqs[0].max_len())
+    gk, gv = workloads.to_bits(gk), workloads.to_bits(gv)
+    rows_ok = all(np.array_equal(gk[l, h, : len(sel[l][h])], kb[l][sel[l][h], h]) and
+                  np.array_equal(gv[l, h, : len(sel[l][h])], vb[l][sel[l][h], h]) and
+                  wb.cache.indexed_positions(0, l, h).tolist() == sel[l][h] for l in range(L) for h in range(H))
+    got = workloads.to_bits(out[:, 0])
+    from oracle import attention as o_attn
+
+    gotf = o_attn.bf16_bits_to_f64(got)
+    qb = workloads.to_bits(q[:, 0])
+    mx, sm = 0.0, 0.0
+    for l in range(L):
+        o_ref, _ = o_ix.attend_indexed(qb[l], kb[l], vb[l], sel[l], wb.scale)
+        e = np.abs(gotf[l] - o_ref)
+        mx, sm = max(mx, float(e.max())), sm + float(e.sum())
+    mean = sm / (L * g.n_q_heads * g.head_dim)
+    res = {"workload": "config-2 shape, un-evicted (%d tokens / sequence), sets selected at t = %d" % (n, t0),
+           "mass_frac": frac, "n_recent": n_recent,
+           "rows_before": cfg.batch * n * L * H, "rows_retained": rows, "kept_pct": 100.0 * rows / (cfg.batch * n * L * H),
+           "retained_bytes": rows * 512, "defrag_bytes_moved": moved, "moved_over_retained": moved / max(1, rows * 512),
+           "select_us_per_sequence": e0.elapsed_time(e1) * 1e3 / cfg.batch,
+           "evict_indexed_wall_us_per_sequence": t_def * 1e6 / cfg.batch,
+           "decode_attn_indexed_us": e2.elapsed_time(e3) * 1e3 / 10,
+           "pages_freed": int(wb.cache.stats()["free_pages"]) - 2,
+           "parity_sequence_0": {"slab_tables_and_rows_bit_exact": bool(rows_ok), "max_abs": mx, "mean_abs": mean,
+                                 "ok": bool(rows_ok and mx <= 2e-2 and mean <= 2e-3)},
+           "device_error_word": wb.cache.last_error(),
+           "note": "first path: FFMA attention over the slabs; the point of the line is the cache-management cost "
+                   "(PAPER.md:154, 214) next to what it buys"}
+    wb.close()
+    del wb
+    torch.cuda.empty_cache()
+    return res
+
+
+def run_prefill(args):
+    """--workload prefill_300s: causal prefill attention of one 300 s chunk (64 prompt + 2250 speech tokens, 28 layers)
+    over the paged cache, murmur_prefill_attn (tcgen05 + TMEM).  A step = one call over all layers.  Bound: tensor."""
+    import numpy as np
+    import torch
+
+    import workloads
+    from paper_2606_01483_b200 import MURMUR_WINDOW_OFF, MurmurCache, binding
+
+    dev = torch.device("cuda:%d" % int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    binding.lib()
+    cfg = workloads.config2()
+    g = cfg.geom
+    K, W = args.steps, max(3, args.warmup)
+    d = workloads.SeqData(cfg, 0, device=dev)
+    k, v = d.prefill_kv()
+    n, L = k.shape[1], g.n_layers
+    nb = (n + cfg.page_size - 1) // cfg.page_size + 2
+    c = MurmurCache(L, g.n_q_heads, g.n_kv_heads, g.head_dim, cfg.page_size, 1, nb, nb + 2, device=dev)
+    c.seq_begin(0, cfg.seqs[0].P, cfg.seqs[0].S, 0, (MURMUR_WINDOW_OFF, 0, 0, MURMUR_WINDOW_OFF, 0))
+    c.kv_append([0], [n], k.contiguous(), v.contiguous())
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(2606)
+    q = torch.randn(L, n, g.n_q_heads, g.head_dim, generator=gen, device=dev).to(torch.bfloat16)
+    out = torch.empty_like(q)
+    lse = torch.empty(L, n, g.n_q_heads, dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+    sampler = ClockSampler(dev.index or 0)
+    for _ in range(W):
+        c.prefill_attn(0, 0, n, q, out=out, lse=lse)
+    torch.cuda.synchronize(dev)
+    sampler.wait_ready()
+    for _ in range(20):  # clocks up and the sampler inside a loaded stretch before the timed region
+        c.prefill_attn(0, 0, n, q, out=out, lse=lse)
+    torch.cuda.synchronize(dev)
+    c.reset_stats()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0 = time.time()
+    e0.record(stream)
+    for _ in range(K):
+        c.prefill_attn(0, 0, n, q, out=out, lse=lse)
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    sampler.window(w0, time.time())
+    launches = c.stats()["kernel_launches"]
+    ms = e0.elapsed_time(e1) / K
+    # the round-1 mma.sync kernel, for context
+    c.set_option(binding.MURMUR_OPT_PREFILL_VARIANT, binding.MURMUR_PREFILL_MMA_SYNC)
+    out_old = torch.empty_like(q)
+    for _ in range(2):
+        c.prefill_attn(0, 0, n, q, out=out_old)
+    torch.cuda.synchronize(dev)
+    e0.record(stream)
+    for _ in range(5):
+        c.prefill_attn(0, 0, n, q, out=out_old)
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    ms_old = e0.elapsed_time(e1) / 5
+    flops = 4.0 * g.head_dim * (n * (n + 1) / 2) * g.n_q_heads * L  # causal: QK^T + PV over y <= x
+    tfs = flops / (ms * 1e-3) / 1e12
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            peak, peak_src = float(json.load(f)["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst: the kernel is timed alone)"
+    except Exception:
+        peak, peak_src = 1590.0, "fallback (B200_PROFILING.md 1.59 PFLOP/s)"
+    # oracle: sampled rows (first, tile / page boundaries, last) of 3 layers, all heads, fp64
+    from oracle import attention as o_attn
+
+    rows = [0, 1, 63, 64, 127, 128, 129, 1000, 2047, 2048, n - 2, n - 1]
+    layers = [0, L // 2, L - 1]
+    kb, vb, qb = workloads.to_bits(k), workloads.to_bits(v), workloads.to_bits(q[layers][:, rows])
+    got = o_attn.bf16_bits_to_f64(workloads.to_bits(out[layers][:, rows]))
+    lse_np = lse[layers][:, rows].cpu().numpy().astype(np.float64)
+    mx, sm, cnt, lse_mx = 0.0, 0.0, 0, 0.0
+    t_or = time.perf_counter()
+    for a, l in enumerate(layers):
+        for b, x in enumerate(rows):
+            o_ref, lse_ref, _ = o_attn.attend_retained(qb[a, b], kb[l], vb[l], range(x + 1), 1.0 / math.sqrt(g.head_dim))
+            e = np.abs(got[a, b] - o_ref)
+            mx, sm, cnt = max(mx, float(e.max())), sm + float(e.sum()), cnt + e.size
+            lse_mx = max(lse_mx, float(np.max(np.abs(lse_np[a, b] - lse_ref))))
+    t_or = time.perf_counter() - t_or
+    pairs = sum(x + 1 for x in rows) * len(layers) * g.n_q_heads
+    all_pairs = n * (n + 1) / 2 * L * g.n_q_heads
+    cpu_ms = t_or * all_pairs / pairs * 1e3
+    clocks = sampler.finish().get("main")
+    err = c.last_error()
+    c.close()
+    line = {
+        "metric": "prefill-attn ms per 300 s chunk (causal, 28 layers, 2314 tokens)", "value": ms, "unit": "ms/chunk",
+        "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "prefill_300s", "tokens": n, "n_layers": L, "n_q_heads": g.n_q_heads, "n_kv_heads": g.n_kv_heads,
+                   "head_dim": g.head_dim, "page_size": cfg.page_size, "l2": "q + out = 2 x 464 MB per call (> 126 MB L2); K/V 133 MB"},
+        "tflops": tfs, "tokens_per_s": n / (ms * 1e-3),
+        "roofline": {"bound": "tensor", "kernel": "prefill_umma_kernel (tcgen05.mma, accumulators in TMEM, TMA-fed)",
+                     "achieved": tfs, "peak": peak, "unit": "TFLOP/s", "frac": tfs / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_flops_per_launch": flops,
+                     "how": "causal flops 4 d sum_x (x + 1) per head and layer / mean launch duration (CUDA events, %d launches)" % K},
+        "mma_sync_kernel_ms": ms_old, "speedup_vs_mma_sync": ms_old / ms,
+        "max_abs_diff_vs_mma_sync": float((out.float() - out_old.float()).abs().max()),
+        "cpu_baseline": {"value": cpu_ms, "unit": "ms/chunk", "cores": 1, "kind": "oracle",
+                         "sample": f"oracle.attention (numpy fp64) on {len(rows)} query rows x {len(layers)} layers x {g.n_q_heads} heads, "
+                                   f"scaled by (query, key) pairs x{all_pairs / pairs:.0f}"},
+        "parity": {"max_abs": mx, "mean_abs": sm / cnt, "lse_max_abs": lse_mx, "tol_max_abs": 2e-2, "tol_mean_abs": 2e-3,
+                   "ok": bool(mx <= 2e-2 and sm / cnt <= 2e-3 and lse_mx < 2e-3),
+                   "compared": f"output of the last timed launch: rows {rows} of layers {layers}, all heads, vs Eq. 1 in fp64"},
+        "e2e": {"value": ms, "unit": "ms/chunk", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                "note": "prefill Q/K/V are produced on the device by the model's projections; no host entry exists for this call"},
+        "gpu_launches": int(launches), "device_error_word": err, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -893,6 +1113,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "prefill_300s":
+        return run_prefill(args)
     return run_murmur(args)
 
 
