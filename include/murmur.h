@@ -116,7 +116,7 @@ typedef struct {
                                      dependent launch (each waits on-device for its predecessor), 0 = plain */
 #define MURMUR_OPT_FUSE_STEP 4    /* murmur_decode_step as: 2 (default) = ONE launch (the attention CTAs derive the
                                      post-append state themselves, keeper warps scatter the rows, commit and evict;
-                                     needs the tensor-core attention variant and <= 32 sequences in the call,
+                                     needs the tensor-core attention variant and <= 64 sequences in the call,
                                      else falls back to 1);
                                      1 = two launches (append with the eviction fused in, then attention);
                                      0 = three launches (append, evict, attention) */

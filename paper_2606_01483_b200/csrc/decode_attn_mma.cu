@@ -39,6 +39,7 @@ namespace murmur {
 namespace {
 
 constexpr int kStages = 6;
+constexpr int kMinTilesPerRange = 6;
 constexpr int kSliceWarps = 4;   // the four 16-row slices of a 64-row tile, one warp each
 constexpr int kGroups = 2;       // warp groups; each works through its OWN tile range, fed through its own half of the ring
 constexpr int kConsumerWarps = kSliceWarps * kGroups;
@@ -62,14 +63,14 @@ struct __align__(128) SmemLayout {
   float scratch[kGroups][2][kFragFloats];  // per group: two hand-over buffers of the end-of-item tree merge
   unsigned long long full_k[kStages], full_v[kStages], empty[kStages], q_full[kGroups][2], q_empty[kGroups][2];
   int meta[kStages][2];  // row_begin, row_end of the tile in each stage
-  int nt[kMaxSeqsAttn];
-  int pre[kMaxSeqsAttn + 1];
-  // per-sequence state the tiles are generated from (the kernel does not read the evict's tile list)
-  SeqParams sp[kMaxSeqsAttn];    // lengths as attended; step mode: AFTER this step's append
-  TileGen tg[kMaxSeqsAttn];      // runs + tile offsets of each sequence (closed form of sp)
+  int pre[kMaxSeqsAttn + 1];     // tiles of the sequences before each one (exclusive prefix sum of tg[].n_tiles)
+  // per-sequence state the tiles are generated from (the kernel does not read the evict's tile list); kept
+  // small - 64 sequences have to fit next to the 6-stage ring
+  int len[kMaxSeqsAttn];         // length as attended; step mode: AFTER this step's append
+  TileGen tg[kMaxSeqsAttn];      // runs + tile offsets of each sequence (closed form of the policy at that length)
   int old_nblk[kMaxSeqsAttn];    // blocks mapped in the block table when the kernel starts
   int newpage[kMaxSeqsAttn];     // step mode: page this step's append maps for the new block, else -1
-  int newatt[kMaxSeqsAttn];      // step mode: 1 if this step's token is in the retained set
+  uint8_t newatt[kMaxSeqsAttn];  // step mode: 1 if this step's token is in the retained set
   int tokpage[kMaxSeqsAttn];     // step mode: page this step's token is written to (read BEFORE the ticket: the
                                  // eviction of the same step may unmap that very block)
   int blk_total;                      // step mode: pages this step's append pops
@@ -98,11 +99,11 @@ __device__ __forceinline__ Cursor locate(const SmemLayout& s, int n_seqs, int n_
   int i = 0;
   while (i + 1 < n_seqs && (unsigned)n_kv * (unsigned)s.pre[i + 1] <= rem) ++i;
   rem -= (unsigned)n_kv * (unsigned)s.pre[i];
-  const unsigned h = rem / (unsigned)s.nt[i];
+  const unsigned h = rem / (unsigned)s.tg[i].n_tiles;
   c.layer = (int)layer;
   c.i = i;
   c.h = (int)h;
-  c.k = (int)(rem - h * (unsigned)s.nt[i]);
+  c.k = (int)(rem - h * (unsigned)s.tg[i].n_tiles);
   return c;
 }
 
@@ -115,7 +116,7 @@ __device__ __forceinline__ void next_item(const SmemLayout& s, int n_seqs, int n
       c.i = 0;
       ++c.layer;
     }
-  } while (s.nt[c.i] == 0);
+  } while (s.tg[c.i].n_tiles == 0);
 }
 
 struct AttnParams {
@@ -152,7 +153,15 @@ __device__ __forceinline__ int warp_scan(int v, int& excl, int lane) {
   excl = inc - v;
   return __shfl_sync(0xffffffffu, inc, 31);
 }
-static_assert(kMaxSeqsAttn <= 32, "one sequence per lane in the set-up scans");
+static_assert(kMaxSeqsAttn <= 64, "two sequences per lane in the set-up scans");
+// Exclusive scan over <= 64 values held two per lane (v0 = element 2 lane, v1 = element 2 lane + 1).
+__device__ __forceinline__ int warp_scan2(int v0, int v1, int& ex0, int& ex1, int lane) {
+  int ex;
+  const int total = warp_scan(v0 + v1, ex, lane);
+  ex0 = ex;
+  ex1 = ex + v0;
+  return total;
+}
 
 // kStep = false: murmur_decode_attn (the cache is as murmur_kv_evict left it).
 // kStep = true : the whole decode step in this one launch (murmur_decode_step): every CTA derives
@@ -215,7 +224,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     } else if (kStep && (!sd.active || sp.len < 1)) {
       s.abort = 2;
     }
-    s.sp[i] = sp;
+    s.len[i] = sp.len;
     s.old_nblk[i] = old_nblk;
     s.newpage[i] = -1;
     if (kStep) {
@@ -226,14 +235,12 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     // generate it here only if it is missing (e.g. a bulk append that was not followed by an evict)
     if (!kStep && prm.has_window) {  // per-call window (e.g. per-layer windows): tables generated here
       sp.w_s = prm.w_s; sp.d = prm.d; sp.k_s = prm.k_s; sp.w_o = prm.w_o; sp.k_o = prm.k_o;
-      s.sp[i] = sp;
       s.tg[i] = make_tilegen(sp, p, plog);
     } else if (ld_acquire(&sd.tg_len[sp.len & 1]) == sp.len) {  // the length validates the table stored before it
       s.tg[i] = sd.tg[sp.len & 1];
     } else {
       s.tg[i] = make_tilegen(sp, p, plog);
     }
-    s.nt[i] = s.tg[i].n_tiles;
     int last_b = 0;
 #pragma unroll
     for (int k = 0; k < 6; ++k)
@@ -241,20 +248,30 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     s.newatt[i] = (kStep && last_b == sp.len) ? 1 : 0;
   }
   __syncthreads();
-  if (warp == 0) {  // prefix sums over <= 32 sequences: tiles, and (step mode) new-block demand
-    int ex;
-    const int tiles_all = warp_scan(lane < n_seqs ? s.nt[lane] : 0, ex, lane);
-    if (lane < n_seqs) s.pre[lane] = ex;
+  if (warp == 0) {  // prefix sums over <= 64 sequences (two per lane): tiles, and (step mode) new-block demand
+    const int i0 = 2 * lane, i1 = 2 * lane + 1;
+    int e0, e1;
+    const int tiles_all = warp_scan2(i0 < n_seqs ? s.tg[i0].n_tiles : 0, i1 < n_seqs ? s.tg[i1].n_tiles : 0, e0, e1, lane);
+    if (i0 < n_seqs) s.pre[i0] = e0;
+    if (i1 < n_seqs) s.pre[i1] = e1;
     if (lane == 0) s.pre[n_seqs] = tiles_all;
     if (kStep) {
-      const int need = (lane < n_seqs && ((s.sp[lane].len + p - 1) >> plog) > s.old_nblk[lane]) ? 1 : 0;
-      const int blk_all = warp_scan(need, ex, lane);
+      const int need0 = (i0 < n_seqs && ((s.len[i0] + p - 1) >> plog) > s.old_nblk[i0]) ? 1 : 0;
+      const int need1 = (i1 < n_seqs && ((s.len[i1] + p - 1) >> plog) > s.old_nblk[i1]) ? 1 : 0;
+      const int blk_all = warp_scan2(need0, need1, e0, e1, lane);
       if (blk_all > free_top) {  // cannot happen after the host-side check; all CTAs agree
         if (lane == 0) s.abort = 3;
-      } else if (need) {  // pops in call order (C3)
-        const int pg = c.free_stack[free_top - 1 - ex];
-        s.newpage[lane] = pg;
-        s.tokpage[lane] = pg;
+      } else {  // pops in call order (C3)
+        if (need0) {
+          const int pg = c.free_stack[free_top - 1 - e0];
+          s.newpage[i0] = pg;
+          s.tokpage[i0] = pg;
+        }
+        if (need1) {
+          const int pg = c.free_stack[free_top - 1 - e1];
+          s.newpage[i1] = pg;
+          s.tokpage[i1] = pg;
+        }
       }
       if (lane == 0) s.blk_total = blk_all;
     }
@@ -281,7 +298,9 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     for (int task = (int)blockIdx.x; task < (wo ? 0 : 2 * n_seqs); task += (int)gridDim.x) {
       const int role = 1 + task / n_seqs, i = task % n_seqs;
       const AttnLookup lk{c.block_table + (size_t)list.ids[i] * c.max_blocks, s.old_nblk[i], s.newpage[i]};
-      evict_task(c, list.ids[i], s.sp[i], role, lk);
+      SeqParams sp = load_params(c.seqs[list.ids[i]]);  // regions and policy never change during a step;
+      sp.len = s.len[i];                                 // the length (committed at some point of this launch) is ours
+      evict_task(c, list.ids[i], sp, role, lk);
     }
     // (2) this step's K/V rows into the pools: one half-warp per 256-byte row (pre-swizzled)
     {
@@ -291,7 +310,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         const unsigned is_v = u >= per_kv, r = is_v ? u - per_kv : u;
         const unsigned r2 = r / (unsigned)n_kv, h = r - r2 * (unsigned)n_kv;
         const unsigned lc = r2 / (unsigned)n_seqs, i = r2 - lc * (unsigned)n_seqs;
-        const int slot = (s.sp[i].len - 1) & (p - 1);
+        const int slot = (s.len[i] - 1) & (p - 1);
         const int page = s.tokpage[i];
         if (page < 0) {
           // write-only range: the eviction of this step (run with the first range) may already have
@@ -307,12 +326,12 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     // (3) last CTA through the ticket: commit the append, then free the dead pages
     if (last) {
       for (int i = lane; i < n_seqs; i += 32) {
-        c.seqs[list.ids[i]].len = s.sp[i].len;
+        c.seqs[list.ids[i]].len = s.len[i];
         if (s.newpage[i] >= 0) c.block_table[(size_t)list.ids[i] * c.max_blocks + s.old_nblk[i]] = s.newpage[i];
       }
       if (lane == 0) c.ctrl[kCtrlAppendTicket] = 0;
       __syncwarp();
-      evict_free_warp(c, list.ids, n_seqs, s.sp, free_top - s.blk_total);
+      evict_free_warp(c, list.ids, n_seqs, s.len, free_top - s.blk_total);
     }
     return;
   }
@@ -327,8 +346,12 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     if (tid == 0) atomicCAS(&c.ctrl[kCtrlError], 0, 5);
     return;
   }
-  const long long V = min(total, (long long)kGroups * gridDim.x);
-  if ((long long)kGroups * blockIdx.x >= V) return;
+  // Number of ranges: two per CTA, but never fewer than kMinTilesPerRange tiles each - a launch with little work
+  // (one layer of a layer-by-layer engine: a few hundred tiles) would otherwise cut every item into many
+  // one- or two-tile segments, each paying a Q load, a tree merge and a split-K partial.  Range v belongs to
+  // half v / gridDim.x of CTA v % gridDim.x, so a short range list is spread over all SMs first.
+  const long long V = max(1ll, min(min(total, (long long)kGroups * gridDim.x), total / kMinTilesPerRange));
+  if ((long long)blockIdx.x >= V) return;
   // range v = [v total / V, (v + 1) total / V), in 32-bit arithmetic (v r < V^2 <= 2^22)
   const unsigned rq = (unsigned)total / (unsigned)V, rr = (unsigned)total - rq * (unsigned)V;
   auto range_lo = [&](long long v) { return (long long)((unsigned)v * rq + ((unsigned)v * rr) / (unsigned)V); };
@@ -357,7 +380,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       ti.row_end = td.row_end;
       // step mode: this step's token (if attended) is the last row of the item's last tile; it is not
       // in the pool yet and is handled apart (newrow), so the tile ends one row earlier
-      const int row_end_pool = td.row_end - ((kStep && s.newatt[cc.i] && tix == s.nt[cc.i] - 1) ? 1 : 0);
+      const int row_end_pool = td.row_end - ((kStep && s.newatt[cc.i] && tix == s.tg[cc.i].n_tiles - 1) ? 1 : 0);
       ti.row_end = row_end_pool;
       ti.tx = (uint32_t)(row_end_pool - td.row_begin) * kRowBytes;
       const int layer = prm.layer_begin + cc.layer;
@@ -374,12 +397,12 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     };
     // This producer warp feeds consumer group gg: it walks the group's range in batches of <= 32
     // tiles of one item; lane j of the warp holds the prepared copies of tile j of the batch.
-    const long long v = (long long)kGroups * blockIdx.x + gg;
+    const long long v = (long long)gg * gridDim.x + blockIdx.x;
     if (v >= V) return;
     const long long lo = range_lo(v), hi = range_lo(v + 1);
     Cursor cur = locate(s, n_seqs, n_kv, lo);
     long long remaining = hi - lo;  // tiles left, counted from the start of the current item's segment
-    int seg = (int)min((long long)(s.nt[cur.i] - cur.k), remaining);
+    int seg = (int)min((long long)(s.tg[cur.i].n_tiles - cur.k), remaining);
     int base = 0, cnt = min(32, seg);
     int sub = 0;         // position of the next tile in the group's kSub stages
     uint32_t ph = 0;     // its phase parity
@@ -393,7 +416,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         // segment ends with the item's last tile (natural layout, straight from k_new / v_new)
         const int qb = item_no & 1;
         mbar_wait(&s.q_empty[gg][qb], ((item_no >> 1) & 1) ^ 1);
-        const bool mini = kStep && s.newatt[cur.i] && (cur.k + seg == s.nt[cur.i]);
+        const bool mini = kStep && s.newatt[cur.i] && (cur.k + seg == s.tg[cur.i].n_tiles);
         const size_t seq_row = (size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i;
         mbar_expect_tx(&s.q_full[gg][qb], (uint32_t)((G + (mini ? 2 : 0)) * kRowBytes));
         bulk_g2s(&s.q[gg][qb][0], prm.q + (seq_row * c.n_q + (size_t)cur.h * G) * kHeadDim, (uint32_t)(G * kRowBytes),
@@ -434,7 +457,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
         ++item_no;
         if (remaining > 0) {
           next_item(s, n_seqs, n_kv, cur);
-          seg = (int)min((long long)s.nt[cur.i], remaining);
+          seg = (int)min((long long)s.tg[cur.i].n_tiles, remaining);
         }
       }
       cnt = remaining > 0 ? min(32, seg - base) : 0;
@@ -464,7 +487,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   const uint32_t v_off = (uint32_t)(slice0 + lv_row) * kRowBytes;
 
   // this group's tile range
-  const long long vrange = (long long)kGroups * blockIdx.x + grp;
+  const long long vrange = (long long)grp * gridDim.x + blockIdx.x;
   if (vrange >= V) return;
   const long long lo = range_lo(vrange), hi = range_lo(vrange + 1);
   const int bar0 = 2 + 4 * grp;  // this group's named barriers
@@ -476,7 +499,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   bool first_segment = true;
 
   while (remaining > 0) {
-    const int nt_i = s.nt[cur.i];
+    const int nt_i = s.tg[cur.i].n_tiles;
     const int seg = (int)min((long long)(nt_i - cur.k), remaining);
     const bool complete = (cur.k == 0) && (seg == nt_i);
 

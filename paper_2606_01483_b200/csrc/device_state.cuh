@@ -22,7 +22,7 @@ constexpr int kTileRows = 64;            // rows of one attention tile (tokens)
 constexpr int kMaxGroup = 8;             // query heads per KV head, padded to the MMA N = 8
 constexpr int kMaxRuns = 6;
 constexpr int kMaxSeqsPerLaunch = 128;
-constexpr int kMaxSeqsAttn = 32;         // sequences per launch of the tensor-core attention kernel (smem tables)
+constexpr int kMaxSeqsAttn = 64;         // sequences per launch of the tensor-core attention kernel (smem tables)
 constexpr int kOStride = 132;            // floats per head row in split-K partials / merge scratch
 constexpr int kPartialFloats = 36 * 32;   // split-K partial in MMA fragment layout: o[32] + m[2] + l[2] per lane, [reg][lane]
 constexpr int kMaxAttnGrid = 1024;       // upper bound on CTAs of the persistent attention kernel

@@ -279,13 +279,16 @@ __device__ __forceinline__ void evict_free(const CacheView& c, const int32_t* id
 
 // Product 0 by ONE warp (the keeper warp of the single-kernel decode step): sequences in call
 // order, so the push offset is a running sum and no CTA-wide synchronisation is needed.
-__device__ __forceinline__ void evict_free_warp(const CacheView& c, const int32_t* ids, int n, const SeqParams* sp_sh,
+// len_sh[i] = the sequence's length as of this evict (regions and policy are read from SeqDev: they never change).
+__device__ __forceinline__ void evict_free_warp(const CacheView& c, const int32_t* ids, int n, const int* len_sh,
                                                 int free_top0) {
   const int lane = threadIdx.x & 31;
   const unsigned lt_mask = (1u << lane) - 1;
   int top = free_top0;
   for (int i = 0; i < n; ++i) {
-    const DeadRanges dr = dead_block_ranges(sp_sh[i], c.p_log2);
+    SeqParams sp = load_params(c.seqs[ids[i]]);
+    sp.len = len_sh[i];
+    const DeadRanges dr = dead_block_ranges(sp, c.p_log2);
     int32_t* tab = c.block_table + (size_t)ids[i] * c.max_blocks;
 #pragma unroll
     for (int k = 0; k < 2; ++k) {

@@ -459,19 +459,23 @@ def test_decode_step_one_launch_random_policies(dev, seed):
     sbs.close()
 
 
-def test_decode_step_more_than_32_sequences_falls_back(dev):
-    """n_seqs > 32 exceeds the step kernel's per-sequence tables (kMaxSeqsAttn): murmur_decode_step takes the two-launch form and
-    the attention call is split in chunks; results are the same."""
-    specs = [seq_spec(4, 20 + (i % 7), 6, 16, 8, n_sink_out=1) for i in range(70)]
-    cfg = Config("many", 90, Geometry(n_layers=1), 16, tuple(specs))
+@pytest.mark.parametrize("n_seqs,one_launch", [(33, True), (64, True), (70, False)])
+def test_decode_step_many_sequences(dev, n_seqs, one_launch):
+    """Up to 64 sequences the whole step is ONE launch (the step kernel's per-sequence tables hold 64); beyond that
+    murmur_decode_step takes the two-launch form and the attention call is split in chunks; results are the same.
+    Ragged windows, so that the new-block prefix sums and the free stack see work in both halves of the list."""
+    specs = [seq_spec(4, 20 + (i % 7), 8, 16, 8 + (i % 3), n_sink_out=1 + (i % 2)) for i in range(n_seqs)]
+    cfg = Config("many", 90, Geometry(n_layers=2), 16, tuple(specs))
     sbs = _mk(cfg, dev)
-    ids = list(range(70))
+    ids = list(range(n_seqs))
     sbs.bulk_prefill(ids, 1)
-    for _ in range(3):
-        q, out, lse = sbs.fused_step(ids, want_lse=True)
+    for k in range(6):
+        order = ids[::-1] if k % 2 else ids
+        n0 = sbs.gpu.stats()["kernel_launches"]
+        q, out, lse = sbs.fused_step(order, want_lse=True)
+        assert (sbs.gpu.stats()["kernel_launches"] - n0 == 1) == one_launch
         sbs.check_integer_state(ids)
-        sbs.check_attention(ids, q, out, lse, seq_subset=[0, 33, 63, 64, 69])
-    assert sbs.gpu.stats()["kernel_launches"] > 0
+        sbs.check_attention(order, q, out, lse)
     sbs.close()
 
 
