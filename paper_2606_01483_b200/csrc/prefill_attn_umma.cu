@@ -29,6 +29,8 @@
 // Tensor memory (512 columns): S_0, S_1 (128 fp32 columns each; P_w aliases the first 64 of S_w), O_0, O_1.
 #include <cuda_bf16.h>
 
+#include <type_traits>
+
 #include "device_state.cuh"
 #include "ptx_utils.cuh"
 #include "umma_utils.cuh"
@@ -165,40 +167,48 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     // Issue order (the two row blocks half a period apart, so that one warpgroup's softmax always runs
     // under the other's MMAs):  S(0,0);  then per tile j:  S(1,j)  PV(0,j)  S(0,j+1)  PV(1,j).
     // S_w aliases P_w: S(w,j+1) is issued after PV(w,j), and tcgen05.mma executes in issue order.
-    // Descriptors: one base per operand tile, the k-steps only add to the start-address field.
-    const uint64_t qd[2][2] = {{smem_desc_kmajor(smem_u32(&s.q[0][0][0])), smem_desc_kmajor(smem_u32(&s.q[0][1][0]))},
-                               {smem_desc_kmajor(smem_u32(&s.q[1][0][0])), smem_desc_kmajor(smem_u32(&s.q[1][1][0]))}};
-    auto issue_s = [&](int w, int j) {  // S_w = Q_w K_j^T
+    // Descriptors: one base per operand tile, the k-steps only add to the start-address field.  The row block is a
+    // compile-time constant of each call so that descriptors and TMEM addresses are formed on the uniform datapath:
+    // the issuing warp shares its scheduler with softmax warps, and every extra instruction (or register -> uniform
+    // register move) between two tcgen05.mma shows up as tensor-pipe idle time.
+    constexpr std::integral_constant<int, 0> W0{};
+    constexpr std::integral_constant<int, 1> W1{};
+    auto issue_s = [&](auto wc, int j) {  // S_w = Q_w K_j^T
+      constexpr int w = decltype(wc)::value;
       const int st = j % kUStages;
       mbar_wait(&s.k_full[st], (uint32_t)(j / kUStages) & 1u);
       tc_fence_after();
-      const uint64_t kd0 = smem_desc_kmajor(smem_u32(&s.k[st][0][0])), kd1 = smem_desc_kmajor(smem_u32(&s.k[st][1][0]));
       if (lane == 0) {
+        const uint64_t qd0 = smem_desc_kmajor(smem_u32(&s.q[w][0][0])), qd1 = smem_desc_kmajor(smem_u32(&s.q[w][1][0]));
+        const uint64_t kd0 = smem_desc_kmajor(smem_u32(&s.k[st][0][0])), kd1 = smem_desc_kmajor(smem_u32(&s.k[st][1][0]));
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk) umma_ss(tb + 128u * w, qd[w][0] + 2u * kk, kd0 + 2u * kk, idesc_s, kk ? 1u : 0u);  // +32 bytes per k-step
+        for (int kk = 0; kk < 4; ++kk) umma_ss(tb + 128u * w, qd0 + 2u * kk, kd0 + 2u * kk, idesc_s, kk ? 1u : 0u);  // +32 bytes per k-step
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk) umma_ss(tb + 128u * w, qd[w][1] + 2u * kk, kd1 + 2u * kk, idesc_s, 1u);
+        for (int kk = 0; kk < 4; ++kk) umma_ss(tb + 128u * w, qd1 + 2u * kk, kd1 + 2u * kk, idesc_s, 1u);
         umma_commit(&s.s_ready[w]);
       }
       __syncwarp();
     };
-    auto issue_pv = [&](int w, int j) {  // O_w += P_w V_j
+    auto issue_pv = [&](auto wc, int j) {  // O_w += P_w V_j
+      constexpr int w = decltype(wc)::value;
       const int st = j % kUStages;
       mbar_wait(&s.p_ready[w], (uint32_t)j & 1u);
       tc_fence_after();
-      const uint64_t vd = smem_desc_mnmajor(smem_u32(&s.v[st][0][0]), kHalfBytes);
       if (lane == 0) {
+        const uint64_t vd = smem_desc_mnmajor(smem_u32(&s.v[st][0][0]), kHalfBytes);
+        const uint32_t acc = j ? 1u : 0u;
+        umma_ts(tb + 256u + 128u * w, tb + 128u * w, vd, idesc_o, acc);
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk.. (+2048 bytes = +128)
-          umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, vd + 128u * kk, idesc_o, (j | kk) ? 1u : 0u);
+        for (int kk = 1; kk < 8; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk.. (+2048 bytes = +128)
+          umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, vd + 128u * kk, idesc_o, 1u);
         umma_commit(&s.o_done[w]);
       }
       __syncwarp();
     };
-    if (nkt[0] > 0) issue_s(0, 0);
+    if (nkt[0] > 0) issue_s(W0, 0);
     for (int j = 0; j < n_kt; ++j) {
       const int st = j % kUStages;
-      if (j < nkt[1]) issue_s(1, j);
+      if (j < nkt[1]) issue_s(W1, j);
       if (lane == 0) umma_commit(&s.k_empty[st]);  // K_j: both S(0,j) and S(1,j) are behind this point
       __syncwarp();
       mbar_wait(&s.v_full[st], (uint32_t)(j / kUStages) & 1u);
@@ -213,9 +223,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
       }
-      if (j < nkt[0]) issue_pv(0, j);
-      if (j + 1 < nkt[0]) issue_s(0, j + 1);
-      if (j < nkt[1]) issue_pv(1, j);
+      if (j < nkt[0]) issue_pv(W0, j);
+      if (j + 1 < nkt[0]) issue_s(W0, j + 1);
+      if (j < nkt[1]) issue_pv(W1, j);
       if (lane == 0) umma_commit(&s.v_empty[st]);
       __syncwarp();
     }
