@@ -240,6 +240,15 @@ MURMUR_API murmur_status_t murmur_decode_step_host(murmur_cache_t* cache, const 
                                                    const void* k_new_host, const void* v_new_host,
                                                    const void* q_host, void* out_host, float sm_scale, void* stream);
 
+/* CUDA graphs.  Every state transition of a step runs on the device, so a captured murmur_decode_step (or the
+ * murmur_decode_step_layers calls of one step) can be REPLAYED: capture the call(s) once with fixed k_new / v_new / q /
+ * out buffers (after at least one un-captured step, so that one-time kernel attributes are set), refill the buffers and
+ * replay once per decode step.  Replays bypass the host-side validation (the kernels keep the device error word: page
+ * exhaustion or max_blocks_per_seq raise it and the step does nothing) and the host mirror of lengths and free pages.
+ * Call murmur_mirror_sync (synchronises `stream`) before the next non-replayed call on the handle; it re-reads lengths
+ * and the free-stack height from the device.  Sequences may not begin or end inside a replayed stretch. */
+MURMUR_API murmur_status_t murmur_mirror_sync(murmur_cache_t* cache, void* stream);
+
 /* ---- chunking (host only) ------------------------------------------------------------------ */
 /* Greedy merge of VAD speech segments into chunks of span <= max_len seconds (c = 300 s).
  *   seg_start, seg_end : HOST float[n_segments], seconds, sorted and non-overlapping

@@ -33,7 +33,7 @@ STATUS_NAMES = {0: "MURMUR_OK", 1: "MURMUR_ERR_INVALID_ARG", 2: "MURMUR_ERR_STAT
 EXPORTED_SYMBOLS = [
     "murmur_pool_bytes", "murmur_workspace_bytes", "murmur_cache_create", "murmur_cache_destroy",
     "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
-    "murmur_decode_step", "murmur_decode_step_layers", "murmur_decode_step_chunked", "murmur_decode_step_host", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
+    "murmur_decode_step", "murmur_decode_step_layers", "murmur_decode_step_chunked", "murmur_decode_step_host", "murmur_mirror_sync", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
     "murmur_profile_scratch_bytes", "murmur_attn_profile",
     "murmur_decode_attn_windowed", "murmur_prefill_attn", "murmur_chunk_plan",
@@ -97,6 +97,7 @@ def lib() -> C.CDLL:
     L.murmur_decode_step.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, C.c_float, vp]
     L.murmur_decode_step_layers.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, i32, i32, C.c_float, vp]
     L.murmur_decode_step_chunked.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, i32, C.c_float, vp]
+    L.murmur_mirror_sync.argtypes = [vp, vp]
     L.murmur_decode_step_host.argtypes = [vp, vp, i32, vp, vp, vp, vp, C.c_float, vp]
     L.murmur_seq_get_state.argtypes = [vp, i32, vp, vp]
     L.murmur_kv_get_retained.argtypes = [vp, i32, vp, i32, vp, vp]
@@ -315,6 +316,10 @@ class MurmurCache:
                                                       q.data_ptr(), out.data_ptr(),
                                                       lse.data_ptr() if lse is not None else None, layers_per_launch,
                                                       C.c_float(sm_scale), _stream()))
+
+    def mirror_sync(self):
+        """After replaying captured steps (CUDA graph): re-reads lengths and the free-page count from the device."""
+        self._check(self.L.murmur_mirror_sync(self.h, _stream()))
 
     def decode_step_host(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor,
                          out: torch.Tensor, sm_scale: Optional[float] = None):

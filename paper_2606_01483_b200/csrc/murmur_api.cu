@@ -990,6 +990,35 @@ murmur_status_t murmur_kv_gather(murmur_cache_t* c, int32_t seq, const int32_t* 
   return MURMUR_OK;
 }
 
+// Re-reads the integer state the host mirror shadows (lengths, free-stack height) from the device.
+murmur_status_t murmur_mirror_sync(murmur_cache_t* c, void* stream) {
+  if (!c) return MURMUR_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  MM_CUDA(c, cudaStreamSynchronize(s));
+  std::vector<SeqDev> dev(c->desc.max_seqs);
+  MM_CUDA(c, cudaMemcpy(dev.data(), c->view.seqs, dev.size() * sizeof(SeqDev), cudaMemcpyDeviceToHost));
+  int32_t top = 0;
+  MM_CUDA(c, cudaMemcpy(&top, c->view.ctrl + kCtrlFreeTop, 4, cudaMemcpyDeviceToHost));
+  for (int i = 0; i < c->desc.max_seqs; ++i) {
+    HostSeq& hs = c->seqs[i];
+    const SeqDev& sd = dev[i];
+    if (!hs.active || !sd.active) continue;  // sequences begin and end through the API only
+    if (hs.indexed) {
+      hs.idx_blocks = sd.idx_blocks;
+      hs.idx_max_len = sd.idx_max_len;
+      continue;
+    }
+    if (sd.len != hs.sp.len) {  // steps ran on the device that the mirror has not seen: every step ends with its eviction
+      hs.sp.len = sd.len;
+      hs.evict_len = sd.len;
+      hs.freed_blocks = dead_block_count(hs.sp, c->desc.page_size);
+    }
+  }
+  c->free_pages = top;
+  c->stats.free_pages = c->free_pages;
+  return MURMUR_OK;
+}
+
 murmur_status_t murmur_get_last_error(murmur_cache_t* c, int32_t* device_err_out, void* stream) {
   if (!c || !device_err_out) return MURMUR_ERR_INVALID_ARG;
   MM_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));

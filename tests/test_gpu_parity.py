@@ -689,6 +689,66 @@ def test_bulk_append_130_sequences_two_layers(dev):
     assert sbs.gpu.last_error() == 0
     sbs.close()
 
+# -------------------------------------------------------------------------------- CUDA graph replay
+@pytest.mark.parametrize("layered", [False, True])
+def test_decode_step_cuda_graph_replay(dev, layered):
+    """One captured decode step (one launch, or the per-layer-range launches of a step) replayed 40 times with
+    refilled input buffers on a ragged page-16 batch (windows slide, pages are allocated and freed inside the
+    replays), then murmur_mirror_sync: integer state bit-exact, every replay's output within tolerance, and the
+    handle usable through the normal calls afterwards."""
+    specs = [seq_spec(8, 70 + 9 * i, 80, 32 if i % 2 else 48, 16 if i % 3 else 32, n_sink_out=2 + i % 3) for i in range(4)]
+    cfg = workloads.config5().with_seqs(specs).with_layers(3)
+    a = _mk(cfg, dev)
+    ids = list(range(cfg.batch))
+    a.bulk_prefill(ids, 1)
+    a.fused_step(ids)  # un-captured step first: one-time kernel attributes are set outside the capture
+    if layered:
+        a.layer_range_step(ids, [(0, 1), (1, 3)])
+    L = cfg.geom.n_layers
+    k_buf = torch.empty(L, len(ids), 4, 128, dtype=torch.bfloat16, device=dev)
+    v_buf = torch.empty_like(k_buf)
+    q_buf = torch.empty(L, len(ids), 28, 128, dtype=torch.bfloat16, device=dev)
+    out_buf = torch.empty_like(q_buf)
+
+    def fill():
+        ks, vs = [], []
+        for i in ids:
+            u = a.t_of(i)
+            k, v = a.data[i].out_kv(u, u + 1)
+            ks.append(k)
+            vs.append(v)
+            a._store(i, k, v)
+        k_buf.copy_(torch.cat(ks, dim=1))
+        v_buf.copy_(torch.cat(vs, dim=1))
+        a.oracle.append(ids, [1] * len(ids))
+        a.oracle.evict(ids)
+        q_buf.copy_(a.queries(ids))
+
+    fill()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        if layered:
+            a.gpu.decode_step_layers(ids, k_buf[0:1], v_buf[0:1], q_buf[0:1], out_buf[0:1], 0, 1, None, a.scale)
+            a.gpu.decode_step_layers(ids, k_buf[1:3], v_buf[1:3], q_buf[1:3], out_buf[1:3], 1, 3, None, a.scale)
+        else:
+            a.gpu.decode_step(ids, k_buf, v_buf, q_buf, out_buf, None, a.scale)
+    for step in range(40):
+        if step:
+            fill()
+        g.replay()
+        torch.cuda.synchronize()
+        if step % 4 == 0 or step >= 36:
+            a.check_attention(ids, q_buf, out_buf)
+    a.gpu.mirror_sync()
+    a.check_integer_state(ids)
+    # and on through the ordinary calls
+    q, out, lse = a.fused_step(ids, want_lse=True)
+    a.check_integer_state(ids)
+    a.check_attention(ids, q, out, lse)
+    a.close()
+
+
 # -------------------------------------------------------------------------------- per-layer windows
 def test_decode_attn_windowed_per_layer_groups(dev):
     """murmur_decode_attn_windowed: layers 0-1 attend a tighter window than layers 2-3 while residency
