@@ -75,6 +75,7 @@ struct __align__(128) SmemLayout {
                                  // eviction of the same step may unmap that very block)
   int blk_total;                      // step mode: pages this step's append pops
   int abort;
+  int chain_ok;                       // step mode: the predecessor's integer state was seen complete before it ended
 };
 static_assert(sizeof(SmemLayout) <= 227 * 1024, "shared memory budget");
 
@@ -127,6 +128,8 @@ struct AttnParams {
   const uint16_t* v_new;
   int write_only;         // step mode, layers after the first of a step issued in layer ranges: the integer state is
                           // already committed (slot reserved, eviction done) - only write this range's rows + attend
+  int chain;              // step mode: the previous launch of the stream was a step launch of this handle ...
+  unsigned chain_expect;  // ... and kCtrlStepDone reads this once all of its keeper warps are done
   int has_window;         // murmur_decode_attn_windowed: attend over the A(t) of THIS policy instead of the sequence's
   int w_s, d, k_s, w_o, k_o;
   int seq_base, n_seqs_total, layer_begin, n_layers_call;
@@ -203,7 +206,31 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   __syncthreads();
   // Everything above touches only this CTA's shared memory; from here on the kernel reads what
   // earlier kernels of the stream wrote and writes buffers the previous launch may still use.
-  pdl_wait();
+  //
+  // Chained steps.  When the previous launch of the stream was a step launch of this handle, waiting for it to
+  // END (griddepcontrol.wait: all its CTAs done and flushed) would leave HBM idle through its tail, the flush
+  // and this launch's set-up.  But everything this launch READS - lengths, tile tables, block tables, the free
+  // stack, the rows the previous step appended - is final as soon as all of the previous launch's KEEPER warps
+  // are done, which is early in that launch: every keeper adds 1 to kCtrlStepDone when it is (release), and
+  // this CTA starts reading when the counter reaches the value the host expects (acquire).  Set-up, tile
+  // generation, the K/V stream and the products run ahead; every WRITE this launch makes (output, split-K
+  // partials and counters, the keepers' scatter / commit / evict) still sits behind griddepcontrol.wait.  The
+  // counter is only a go-ahead: if it does not show the expected value in time (a replayed CUDA graph, whose
+  // launches the host did not count), the CTA falls back to griddepcontrol.wait, which is always sufficient.
+  bool chained = false;
+  if (kStep && prm.chain) {
+    if (tid == 0) {
+      int ok = 0;
+      for (int it = 0; it < 4096 && !ok; ++it) {
+        ok = ((unsigned)ld_acquire(&c.ctrl[kCtrlStepDone]) == prm.chain_expect) ? 1 : 0;
+        if (!ok) __nanosleep(64);
+      }
+      s.chain_ok = ok;
+    }
+    __syncthreads();
+    chained = s.chain_ok != 0;
+  }
+  if (!chained) pdl_wait();
 #ifdef MURMUR_TRACE
   if (tid == 0) {
     trace[0] = globaltimer_ns();
@@ -279,7 +306,11 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // zeroed Q rows vs later bulk copies
   __syncthreads();
   if (s.abort) {
-    if (tid == 0) atomicCAS(&c.ctrl[kCtrlError], 0, s.abort);
+    if (tid == 0) {
+      pdl_wait();
+      atomicCAS(&c.ctrl[kCtrlError], 0, s.abort);
+      if (kStep) atomicAdd(&c.ctrl[kCtrlStepDone], 1);  // a successor must not wait for a keeper that never runs
+    }
     return;
   }
 
@@ -291,6 +322,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     // All the old state this CTA needs is in shared memory now: take the ticket first.
     // (write-only layer ranges change no integer state: no ticket, no table products, no commit)
     const bool wo = prm.write_only != 0;
+    if (chained) pdl_wait();  // everything a keeper does is a write
     int last = 0;
     if (lane == 0 && !wo) last = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
     last = __shfl_sync(0xffffffffu, last, 0);
@@ -333,6 +365,10 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       __syncwarp();
       evict_free_warp(c, list.ids, n_seqs, s.len, free_top - s.blk_total);
     }
+    __threadfence();  // release: this keeper's table products, rows and (last keeper) commit + freed pages ...
+    asm volatile("fence.proxy.async;" ::: "memory");  // (the successor reads the scattered rows with bulk copies)
+    __syncwarp();
+    if (lane == 0) atomicAdd(&c.ctrl[kCtrlStepDone], 1);  // ... before the count a chained successor waits for
     return;
   }
 
@@ -666,6 +702,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 
     if (w4 == 0) {
       // ---- the group's first warp finishes the item: output, or split-K partial ----
+      if (kStep && chained) pdl_wait();  // first global write of this warp (no-op once the predecessor has ended)
       const int layer_c = cur.layer;
       const size_t out_row0 = ((size_t)layer_c * prm.n_seqs_total + prm.seq_base + cur.i) * c.n_q + (size_t)cur.h * G;
       // lane (lrow, lcol) holds O^T[d][head] for d = 16 dt + lrow (+ 8), head = lcol (+ 1)
@@ -789,7 +826,7 @@ cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_bas
 // reserved the slots and run the eviction.
 cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void* k_new, const void* v_new,
                             const void* q, void* out, float* lse, float sm_scale, int layer_begin, int layer_end,
-                            bool write_only, int grid, bool pdl, cudaStream_t st, LaunchInfo* info) {
+                            bool write_only, int grid, bool pdl, long long chain_expect, cudaStream_t st, LaunchInfo* info) {
   AttnParams prm{};
   prm.q = reinterpret_cast<const uint16_t*>(q);
   prm.out = reinterpret_cast<uint16_t*>(out);
@@ -801,6 +838,8 @@ cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void*
   prm.layer_begin = layer_begin;
   prm.n_layers_call = layer_end - layer_begin;
   prm.write_only = write_only ? 1 : 0;
+  prm.chain = (pdl && chain_expect >= 0) ? 1 : 0;
+  prm.chain_expect = (unsigned)chain_expect;
   prm.sm_scale = sm_scale;
   return launch_mma<true>(c, list, prm, grid, pdl, st, info);
 }

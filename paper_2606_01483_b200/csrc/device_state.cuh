@@ -30,7 +30,7 @@ constexpr int kStepTraceWords = 16;      // globaltimer stamps of the step prolo
 constexpr int kTimelineWords = 4;        // globaltimer at CTA start, at CTA end, SM id, tiles processed
 
 // ctrl word indices
-enum { kCtrlFreeTop = 0, kCtrlError = 1, kCtrlAppendTicket = 2, kCtrlWords = 8 };
+enum { kCtrlFreeTop = 0, kCtrlError = 1, kCtrlAppendTicket = 2, kCtrlStepDone = 3, kCtrlWords = 8 };
 
 // The maximal intervals of A(t) held in six fixed slots (all indexing static, so the whole thing
 // lives in registers): slot i is a run iff bit i of `mask` is set; merged neighbours are folded
@@ -210,9 +210,11 @@ cudaError_t launch_attn_generic(const CacheView& c, const SeqList& list, int seq
 cudaError_t launch_attn_mma(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,
                             void* out, float* lse, int layer_begin, int layer_end, float sm_scale, int grid,
                             bool pdl, const SeqParams* window, cudaStream_t st, LaunchInfo* info);
+// chain_expect >= 0: the previous launch on this handle's stream was a step launch; kCtrlStepDone reads that value
+// once all of ITS keeper warps are done (see decode_attn_mma.cu, "chained steps").
 cudaError_t launch_step_mma(const CacheView& c, const SeqList& list, const void* k_new, const void* v_new,
                             const void* q, void* out, float* lse, float sm_scale, int layer_begin, int layer_end,
-                            bool write_only, int grid, bool pdl, cudaStream_t st, LaunchInfo* info);
+                            bool write_only, int grid, bool pdl, long long chain_expect, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_prefill_attn(const CacheView& c, int seq, int pos_begin, int n_tok, const void* q, void* out,
                                 float* lse, int layer_begin, int layer_end, float sm_scale, cudaStream_t st,
                                 LaunchInfo* info);

@@ -118,6 +118,8 @@ struct murmur_cache {
   murmur_stats_t stats;
   cudaError_t last_cuda;
   uint8_t* ws;
+  bool chain_ok = false;        // the last launch through this handle was a (counted) step launch: the next may chain
+  uint32_t step_done = 0;       // value kCtrlStepDone reaches once every step launch counted so far is through its keepers
   IdxView idx{nullptr, nullptr, 0};        // indexed-mode tables (murmur_indexed_enable)
   unsigned long long* idx_moved = nullptr;  // device counter of rows moved by the last index-set eviction
 };
@@ -135,7 +137,10 @@ murmur_status_t cuda_fail(murmur_cache* c, cudaError_t e) {
     if (e__ != cudaSuccess) return cuda_fail((c), e__);   \
   } while (0)
 
-void note(murmur_cache* c, const LaunchInfo& li) { c->stats.kernel_launches += li.launches; }
+void note(murmur_cache* c, const LaunchInfo& li) {
+  c->stats.kernel_launches += li.launches;
+  c->chain_ok = false;  // any launch that is not a step launch breaks the chain (the step path sets it again)
+}
 
 inline int32_t blocks_for(int32_t len, int32_t p) { return (len + p - 1) / p; }
 
@@ -507,9 +512,17 @@ static murmur_status_t step_layers_impl(murmur_cache_t* c, const int32_t* seq_id
     for (int i = 0; i < n_seqs; ++i) list.ids[i] = seq_ids[i];
     const int grid = c->attn_grid_opt > 0 ? c->attn_grid_opt : c->sm_count;
     LaunchInfo li{};
+    // chained steps (decode_attn_mma.cu): only between launches the host has counted - not while capturing a graph
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    const bool capturing = cudaStreamIsCapturing((cudaStream_t)stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone;
+    const long long chain_expect = (c->chain_ok && !capturing && c->pdl_opt != 0) ? (long long)c->step_done : -1;
     MM_CUDA(c, launch_step_mma(c->view, list, k_new, v_new, q, out, lse, sm_scale, layer_begin, layer_end, !opens, grid,
-                               c->pdl_opt != 0, (cudaStream_t)stream, &li));
+                               c->pdl_opt != 0, chain_expect, (cudaStream_t)stream, &li));
     note(c, li);
+    if (!capturing) {
+      c->step_done += (uint32_t)li.grid;
+      c->chain_ok = true;
+    }
     if (opens) {
       const int32_t p = c->desc.page_size;
       for (int i = 0; i < n_seqs; ++i) {  // host mirror of the append (validated by check_step) ...
@@ -1016,6 +1029,10 @@ murmur_status_t murmur_mirror_sync(murmur_cache_t* c, void* stream) {
   }
   c->free_pages = top;
   c->stats.free_pages = c->free_pages;
+  int32_t done = 0;  // replayed step launches counted on the device only
+  MM_CUDA(c, cudaMemcpy(&done, c->view.ctrl + kCtrlStepDone, 4, cudaMemcpyDeviceToHost));
+  c->step_done = (uint32_t)done;
+  c->chain_ok = false;
   return MURMUR_OK;
 }
 
