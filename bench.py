@@ -728,7 +728,11 @@ def run_murmur(args):
                 "how": ("steady state: region A time / K launches (one launch per step, CUDA events around the K "
                         "steps; consecutive launches overlap their set-up)" if one_launch
                         else "mean of per-launch CUDA event pairs (region B2)"),
-                "frac_of_nominal_8000": achieved / 8000.0}
+                "frac_of_nominal_8000": achieved / 8000.0,
+                "frac_isolated_launch": alg_bytes / ((t_stepk if one_launch else t_att) * 1e-6) / 1e9 / peak,
+                "note": ("peak is a COPY figure (read + write streams); this kernel only reads K/V, and back-to-back "
+                         "launches overlap one step's set-up and drain with the neighbours' streams, so frac can pass "
+                         "1.0: frac_of_nominal_8000 is the same bytes/time against the HBM3e data-sheet rate")}
 
     # ---- oracle: parity of the timed outputs, CPU baseline, replay, protocol, other workloads -----
     cpu_baseline = parity = replay = protocol = others = index_sets = None

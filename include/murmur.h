@@ -387,8 +387,9 @@ MURMUR_API murmur_status_t murmur_get_last_error(murmur_cache_t* cache, int32_t*
 /* Profiling builds only (library compiled with -DMURMUR_TRACE: `python -m paper_2606_01483_b200.build --trace`);
  * the production kernels carry no time stamps and the production library does not export these. */
 #define MURMUR_TRACE_API MURMUR_API
-/* Per-CTA trace of the LAST tensor-core attention launch: out is HOST uint64[n][4] = {globaltimer ns when
- * the CTA started its work, at CTA end, SM id, tiles processed}; *n_out = CTAs of that launch (0 if the
+/* Per-CTA trace of the LAST tensor-core attention launch: out is HOST uint64[n][8] = {globaltimer ns when
+ * the CTA started its work (after the chain / dependency wait), at CTA end, SM id, tiles processed, ns at kernel
+ * entry, set-up done, keeper past its dependency wait, keeper done}; *n_out = CTAs of that launch (0 if the
  * last launch was the generic variant). */
 MURMUR_TRACE_API murmur_status_t murmur_debug_attn_timeline(murmur_cache_t* cache, uint64_t* out, int32_t cap_ctas,
                                                             int32_t* n_out, void* stream);

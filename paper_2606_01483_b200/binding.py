@@ -446,11 +446,12 @@ class MurmurCache:
         return e.value
 
     def attn_timeline(self) -> np.ndarray:
-        """uint64 [n_ctas, 4] = (start ns, end ns, SM id, tiles) of the last tensor-core attention launch.
+        """uint64 [n_ctas, 8] = (start ns, end ns, SM id, tiles, entry ns, set-up done, keeper begin, keeper end) of the
+        last tensor-core attention launch.
         Needs a profiling build of the library (python -m paper_2606_01483_b200.build --trace)."""
         if not hasattr(self.L, "murmur_debug_attn_timeline"):
             raise MurmurError(5, "library built without MURMUR_TRACE")
-        a = np.zeros((1024, 4), dtype=np.uint64)
+        a = np.zeros((1024, 8), dtype=np.uint64)
         n = C.c_int32(0)
         self._check(self.L.murmur_debug_attn_timeline(self.h, a.ctypes.data, 1024, C.byref(n), _stream()))
         return a[: n.value].copy()

@@ -70,7 +70,8 @@ struct __align__(128) SmemLayout {
   TileGen tg[kMaxSeqsAttn];      // runs + tile offsets of each sequence (closed form of the policy at that length)
   int old_nblk[kMaxSeqsAttn];    // blocks mapped in the block table when the kernel starts
   int newpage[kMaxSeqsAttn];     // step mode: page this step's append maps for the new block, else -1
-  uint8_t newatt[kMaxSeqsAttn];  // step mode: 1 if this step's token is in the retained set
+  uint8_t newatt[kMaxSeqsAttn];  // step mode: bit 0 = this step's token is in the retained set; bit 1 = the tile
+                                 // table at this length was found ready (an evict / a step ran at length - 1)
   int tokpage[kMaxSeqsAttn];     // step mode: page this step's token is written to (read BEFORE the ticket: the
                                  // eviction of the same step may unmap that very block)
   int blk_total;                      // step mode: pages this step's append pops
@@ -184,6 +185,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   const int p = c.p, plog = c.p_log2;
 #ifdef MURMUR_TRACE
   unsigned long long* trace = c.timeline + (size_t)blockIdx.x * kTimelineWords;
+  const unsigned long long t_entry = globaltimer_ns();
 #endif
   pdl_launch_dependents();
 
@@ -237,6 +239,8 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     trace[1] = 0ull;
     trace[2] = smid();
     trace[3] = 0ull;
+    trace[4] = t_entry;
+    trace[5] = trace[6] = trace[7] = 0ull;
   }
 #endif
   // ---- per-sequence state: policy + length -> tile count; step mode: the length after this step ----
@@ -258,6 +262,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       const int xb = (sp.len - 1) >> plog;
       s.tokpage[i] = xb < old_nblk ? c.block_table[(size_t)list.ids[i] * c.max_blocks + xb] : -1;
     }
+    bool tg_ready = false;
     // the tile table at this length was written by the last evict / decode step (SeqDev.tg);
     // generate it here only if it is missing (e.g. a bulk append that was not followed by an evict)
     if (!kStep && prm.has_window) {  // per-call window (e.g. per-layer windows): tables generated here
@@ -265,6 +270,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       s.tg[i] = make_tilegen(sp, p, plog);
     } else if (ld_acquire(&sd.tg_len[sp.len & 1]) == sp.len) {  // the length validates the table stored before it
       s.tg[i] = sd.tg[sp.len & 1];
+      tg_ready = true;
     } else {
       s.tg[i] = make_tilegen(sp, p, plog);
     }
@@ -272,7 +278,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 #pragma unroll
     for (int k = 0; k < 6; ++k)
       if (s.tg[i].rr.mask >> k & 1u) last_b = max(last_b, s.tg[i].rr.b[k]);
-    s.newatt[i] = (kStep && last_b == sp.len) ? 1 : 0;
+    s.newatt[i] = (uint8_t)(((kStep && last_b == sp.len) ? 1 : 0) | (tg_ready ? 2 : 0));
   }
   __syncthreads();
   if (warp == 0) {  // prefix sums over <= 64 sequences (two per lane): tiles, and (step mode) new-block demand
@@ -316,16 +322,22 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
 
   const uint8_t* kpool = reinterpret_cast<const uint8_t*>(c.k_pool);
   const uint8_t* vpool = reinterpret_cast<const uint8_t*>(c.v_pool);
+#ifdef MURMUR_TRACE
+  if (tid == 0) trace[5] = globaltimer_ns();
+#endif
 
   if (kStep && warp == kConsumerWarps + kGroups) {
     // ===================================== keeper warp =====================================
     // All the old state this CTA needs is in shared memory now: take the ticket first.
     // (write-only layer ranges change no integer state: no ticket, no table products, no commit)
     const bool wo = prm.write_only != 0;
-    if (chained) pdl_wait();  // everything a keeper does is a write
-    int last = 0;
-    if (lane == 0 && !wo) last = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
-    last = __shfl_sync(0xffffffffu, last, 0);
+    // Chained launch: the predecessor is still running, but all of ITS keepers are done, so nothing of it reads
+    // SeqDev / the table products / the ticket any more (its warps work from shared memory and, lazily, from
+    // block-table entries of blocks that are live at its length).  What may run before griddepcontrol.wait is
+    // therefore: the table products, the ticket and the commit (a new block-table entry the predecessor never
+    // looks at).  What must wait for its end: unmapping + pushing the pages that die at THIS length (the
+    // predecessor may still stream them), and everything that reads this call's inputs - k_new / v_new may have
+    // been produced by other work of the stream, which only griddepcontrol.wait orders before us.
     // (1) the eviction's table products for the post-append state, spread over the CTAs
     for (int task = (int)blockIdx.x; task < (wo ? 0 : 2 * n_seqs); task += (int)gridDim.x) {
       const int role = 1 + task / n_seqs, i = task % n_seqs;
@@ -334,41 +346,83 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       sp.len = s.len[i];                                 // the length (committed at some point of this launch) is ours
       evict_task(c, list.ids[i], sp, role, lk);
     }
-    // (2) this step's K/V rows into the pools: one half-warp per 256-byte row (pre-swizzled)
-    {
-      const int half = lane >> 4, sub = lane & 15;
-      const unsigned per_kv = (unsigned)prm.n_layers_call * (unsigned)n_seqs * (unsigned)n_kv;
-      for (unsigned u = 2u * blockIdx.x + half; u < 2u * per_kv; u += 2u * gridDim.x) {
-        const unsigned is_v = u >= per_kv, r = is_v ? u - per_kv : u;
-        const unsigned r2 = r / (unsigned)n_kv, h = r - r2 * (unsigned)n_kv;
-        const unsigned lc = r2 / (unsigned)n_seqs, i = r2 - lc * (unsigned)n_seqs;
-        const int slot = (s.len[i] - 1) & (p - 1);
-        const int page = s.tokpage[i];
-        if (page < 0) {
-          // write-only range: the eviction of this step (run with the first range) may already have
-          // freed the block of a token that is dead on arrival (w_out = 0) - its rows are dropped
-          if (!(wo && !s.newatt[i])) atomicCAS(&c.ctrl[kCtrlError], 0, 2);
-          continue;
-        }
-        const uint4 val = reinterpret_cast<const uint4*>(is_v ? prm.v_new : prm.k_new)[(size_t)r * 16 + sub];
-        uint8_t* pool = reinterpret_cast<uint8_t*>(is_v ? c.v_pool : c.k_pool);
-        reinterpret_cast<uint4*>(pool + row_offset(c, prm.layer_begin + (int)lc, page, (int)h, slot))[sub ^ (slot & 7)] = val;
-      }
-    }
-    // (3) last CTA through the ticket: commit the append, then free the dead pages
+    int last = 0;
+    if (lane == 0 && !wo) last = (atomicAdd(&c.ctrl[kCtrlAppendTicket], 1) == (int)gridDim.x - 1);
+    last = __shfl_sync(0xffffffffu, last, 0);
+    // (2) last CTA through the ticket (every CTA has its old state in shared memory by now): commit the append and
+    // look up the pages that die at this length.  Sequences whose tile table was found ready (newatt bit 1: an
+    // evict or a step ran at length - 1 and freed everything dead THERE) only need the blocks that are dead now
+    // and were not then - one or two per step; lane j takes sequences 2 j and 2 j + 1, all loads in flight at once.
+    FreeCand fc0, fc1;
+    bool fast = true;
     if (last) {
       for (int i = lane; i < n_seqs; i += 32) {
         c.seqs[list.ids[i]].len = s.len[i];
         if (s.newpage[i] >= 0) c.block_table[(size_t)list.ids[i] * c.max_blocks + s.old_nblk[i]] = s.newpage[i];
       }
       if (lane == 0) c.ctrl[kCtrlAppendTicket] = 0;
-      __syncwarp();
-      evict_free_warp(c, list.ids, n_seqs, s.len, free_top - s.blk_total);
+      const bool ok0 = free_candidates(c, list.ids, n_seqs, 2 * lane, s.len, s.newatt, s.old_nblk, s.newpage, fc0);
+      const bool ok1 = free_candidates(c, list.ids, n_seqs, 2 * lane + 1, s.len, s.newatt, s.old_nblk, s.newpage, fc1);
+      fast = __all_sync(0xffffffffu, ok0 && ok1);
+    }
+    if (chained) pdl_wait();
+#ifdef MURMUR_TRACE
+    if (lane == 0) trace[6] = globaltimer_ns();
+#endif
+    // (3) this step's K/V rows into the pools: one half-warp per 256-byte row (pre-swizzled), four rows in flight
+    {
+      const int half = lane >> 4, sub = lane & 15;
+      const unsigned per_kv = (unsigned)prm.n_layers_call * (unsigned)n_seqs * (unsigned)n_kv;
+      const unsigned stride = 2u * gridDim.x;
+      for (unsigned u0 = 2u * blockIdx.x + half; u0 < 2u * per_kv; u0 += 4u * stride) {
+        uint4 val[4];
+        uint4* dst[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const unsigned u = u0 + (unsigned)k * stride;
+          dst[k] = nullptr;
+          if (u >= 2u * per_kv) continue;
+          const unsigned is_v = u >= per_kv, r = is_v ? u - per_kv : u;
+          const unsigned r2 = r / (unsigned)n_kv, h = r - r2 * (unsigned)n_kv;
+          const unsigned lc = r2 / (unsigned)n_seqs, i = r2 - lc * (unsigned)n_seqs;
+          const int slot = (s.len[i] - 1) & (p - 1);
+          const int page = s.tokpage[i];
+          if (page < 0) {
+            // write-only range: the eviction of this step (run with the first range) may already have
+            // freed the block of a token that is dead on arrival (w_out = 0) - its rows are dropped
+            if (!(wo && !(s.newatt[i] & 1))) atomicCAS(&c.ctrl[kCtrlError], 0, 2);
+            continue;
+          }
+          val[k] = reinterpret_cast<const uint4*>(is_v ? prm.v_new : prm.k_new)[(size_t)r * 16 + sub];
+          uint8_t* pool = reinterpret_cast<uint8_t*>(is_v ? c.v_pool : c.k_pool);
+          dst[k] = reinterpret_cast<uint4*>(pool + row_offset(c, prm.layer_begin + (int)lc, page, (int)h, slot)) + (sub ^ (slot & 7));
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (dst[k] != nullptr) *dst[k] = val[k];
+      }
+    }
+    // (4) last keeper: push + unmap the dead pages (sequences in call order, blocks ascending - DESIGN.md C3)
+    if (last) {
+      const int top0 = free_top - s.blk_total;
+      if (fast) {
+        int e0, e1;
+        const int total_free = warp_scan2(fc0.n, fc1.n, e0, e1, lane);
+        free_push(c, list.ids, 2 * lane, fc0, top0 + e0);
+        free_push(c, list.ids, 2 * lane + 1, fc1, top0 + e1);
+        if (lane == 0) c.ctrl[kCtrlFreeTop] = top0 + total_free;
+      } else {
+        __syncwarp();
+        evict_free_warp(c, list.ids, n_seqs, s.len, top0);
+      }
     }
     __threadfence();  // release: this keeper's table products, rows and (last keeper) commit + freed pages ...
     asm volatile("fence.proxy.async;" ::: "memory");  // (the successor reads the scattered rows with bulk copies)
     __syncwarp();
     if (lane == 0) atomicAdd(&c.ctrl[kCtrlStepDone], 1);  // ... before the count a chained successor waits for
+#ifdef MURMUR_TRACE
+    if (lane == 0) trace[7] = globaltimer_ns();
+#endif
     return;
   }
 
@@ -416,7 +470,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
       ti.row_end = td.row_end;
       // step mode: this step's token (if attended) is the last row of the item's last tile; it is not
       // in the pool yet and is handled apart (newrow), so the tile ends one row earlier
-      const int row_end_pool = td.row_end - ((kStep && s.newatt[cc.i] && tix == s.tg[cc.i].n_tiles - 1) ? 1 : 0);
+      const int row_end_pool = td.row_end - ((kStep && (s.newatt[cc.i] & 1) && tix == s.tg[cc.i].n_tiles - 1) ? 1 : 0);
       ti.row_end = row_end_pool;
       ti.tx = (uint32_t)(row_end_pool - td.row_begin) * kRowBytes;
       const int layer = prm.layer_begin + cc.layer;
@@ -447,12 +501,16 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     if (lane < cnt) ti = prep(cur, cur.k + lane);
     while (remaining > 0) {
       // ---- issue the current batch ----
-      if (base == 0 && lane == 0) {  // first batch of an item (or of this range's segment of it)
-        // stage its G query rows and, in step mode, this step's K / V rows of the item when this
-        // segment ends with the item's last tile (natural layout, straight from k_new / v_new)
+      // first batch of an item (or of this range's segment of it): stage its G query rows and, in step mode, this
+      // step's K / V rows of the item when this segment ends with the item's last tile (natural layout, straight
+      // from k_new / v_new).  These are the call's INPUTS: in a chained launch they are read only after
+      // griddepcontrol.wait (other work of the stream may have produced them) - for the first item that wait is
+      // put off until the ring is full, so the K/V stream starts while the predecessor drains.
+      auto load_q = [&]() {
+        if (kStep && chained) pdl_wait();
         const int qb = item_no & 1;
         mbar_wait(&s.q_empty[gg][qb], ((item_no >> 1) & 1) ^ 1);
-        const bool mini = kStep && s.newatt[cur.i] && (cur.k + seg == s.tg[cur.i].n_tiles);
+        const bool mini = kStep && (s.newatt[cur.i] & 1) && (cur.k + seg == s.tg[cur.i].n_tiles);
         const size_t seq_row = (size_t)cur.layer * prm.n_seqs_total + prm.seq_base + cur.i;
         mbar_expect_tx(&s.q_full[gg][qb], (uint32_t)((G + (mini ? 2 : 0)) * kRowBytes));
         bulk_g2s(&s.q[gg][qb][0], prm.q + (seq_row * c.n_q + (size_t)cur.h * G) * kHeadDim, (uint32_t)(G * kRowBytes),
@@ -462,9 +520,13 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
           bulk_g2s(&s.newrow[gg][qb][0][0], prm.k_new + off, (uint32_t)kRowBytes, &s.q_full[gg][qb]);
           bulk_g2s(&s.newrow[gg][qb][1][0], prm.v_new + off, (uint32_t)kRowBytes, &s.q_full[gg][qb]);
         }
-      }
+      };
+      const bool first_batch = base == 0 && lane == 0;
+      const bool defer_q = kStep && chained && item_no == 0;
+      if (first_batch && !defer_q) load_q();
       for (int j = 0; j < cnt; ++j) {
         const int st = kGroups * sub + gg;
+        if (first_batch && defer_q && j == kSub) load_q();  // the ring is full: tile j needs a stage back
         if (lane == j) {
           mbar_wait(&s.empty[st], ph ^ 1u);
           s.meta[st][0] = ti.row_begin;
@@ -485,6 +547,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
           ph ^= 1u;
         }
       }
+      if (first_batch && defer_q && cnt <= kSub) load_q();
       // ---- advance, and prepare the next batch while the ring (just filled) drains ----
       base += cnt;
       if (base >= seg) {  // item (or this range's segment of it) done
@@ -554,7 +617,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     __syncwarp();
     // step mode: the group's first warp also processes this step's token at the end of the item, from
     // the same double buffer as the queries - it hands the buffer back only then
-    const bool mini = kStep && w4 == 0 && s.newatt[cur.i] && (cur.k + seg == nt_i);
+    const bool mini = kStep && w4 == 0 && (s.newatt[cur.i] & 1) && (cur.k + seg == nt_i);
     if (lane == 0 && !mini) mbar_arrive(&s.q_empty[grp][qb]);
 
     float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;

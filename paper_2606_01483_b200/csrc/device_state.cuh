@@ -27,7 +27,7 @@ constexpr int kOStride = 132;            // floats per head row in split-K parti
 constexpr int kPartialFloats = 36 * 32;   // split-K partial in MMA fragment layout: o[32] + m[2] + l[2] per lane, [reg][lane]
 constexpr int kMaxAttnGrid = 1024;       // upper bound on CTAs of the persistent attention kernel
 constexpr int kStepTraceWords = 16;      // globaltimer stamps of the step prologue (after the per-CTA entries)
-constexpr int kTimelineWords = 4;        // globaltimer at CTA start, at CTA end, SM id, tiles processed
+constexpr int kTimelineWords = 8;        // globaltimer at CTA start, at CTA end, SM id, tiles processed; entry, set-up done, keeper begin, keeper end
 
 // ctrl word indices
 enum { kCtrlFreeTop = 0, kCtrlError = 1, kCtrlAppendTicket = 2, kCtrlStepDone = 3, kCtrlWords = 8 };

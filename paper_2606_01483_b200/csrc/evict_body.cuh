@@ -308,6 +308,75 @@ __device__ __forceinline__ void evict_free_warp(const CacheView& c, const int32_
   if (lane == 0) c.ctrl[kCtrlFreeTop] = top;
 }
 
+// Product 0 of a decode step, the short way.  When everything that was dead at length - 1 has been freed (the
+// caller knows: an evict or a step ran there), the pages to free at `len` are the blocks inside the dead ranges
+// at len that were outside the dead ranges at len - 1 - the windows move a few positions per step, so that is
+// 0..2 blocks per sequence.  One THREAD looks up one sequence (kFreeCand block-table loads, all independent), so a
+// warp has the candidates of 64 sequences after one round trip, where evict_free_warp makes two per sequence.
+constexpr int kFreeCand = 4;
+struct FreeCand {
+  int32_t b[kFreeCand], pg[kFreeCand];  // newly dead blocks (ascending) and their pages (-1: not mapped)
+  int32_t n;                            // pages to push
+};
+
+// Returns false when the short way does not apply to sequence i (table not ready, or more than kFreeCand newly dead
+// blocks): the caller then runs evict_free_warp for the whole call.  i >= n gives an empty candidate list.
+// old_nblk / newpage: the block this step's commit maps (it may be written to the table concurrently).
+__device__ __forceinline__ bool free_candidates(const CacheView& c, const int32_t* ids, int n, int i, const int* len_sh,
+                                                const uint8_t* flags, const int* old_nblk, const int* newpage,
+                                                FreeCand& fc) {
+#pragma unroll
+  for (int k = 0; k < kFreeCand; ++k) fc.b[k] = fc.pg[k] = -1;
+  fc.n = 0;
+  if (i >= n) return true;
+  if (!(flags[i] & 2)) return false;
+  SeqParams sp = load_params(c.seqs[ids[i]]);
+  sp.len = len_sh[i];
+  const DeadRanges dn = dead_block_ranges(sp, c.p_log2);
+  sp.len -= 1;
+  const DeadRanges dold = dead_block_ranges(sp, c.p_log2);
+  int cnt = 0;
+  bool ok = true;
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    const int hi = r ? dn.hi1 : dn.hi0;
+    int b = r ? dn.lo1 : dn.lo0;
+    while (b < hi) {
+      if (b >= dold.lo0 && b < dold.hi0) { b = dold.hi0; continue; }
+      if (b >= dold.lo1 && b < dold.hi1) { b = dold.hi1; continue; }
+      if (cnt == kFreeCand) { ok = false; break; }
+#pragma unroll
+      for (int k = 0; k < kFreeCand; ++k)
+        if (k == cnt) fc.b[k] = b;
+      ++cnt;
+      ++b;
+    }
+  }
+  if (!ok) return false;
+  const int32_t* tab = c.block_table + (size_t)ids[i] * c.max_blocks;
+#pragma unroll
+  for (int k = 0; k < kFreeCand; ++k) {
+    const int b = fc.b[k];
+    if (b >= 0) fc.pg[k] = b < old_nblk[i] ? tab[b] : (b == old_nblk[i] ? newpage[i] : -1);
+  }
+#pragma unroll
+  for (int k = 0; k < kFreeCand; ++k) fc.n += fc.pg[k] >= 0;
+  return true;
+}
+
+// Pushes the candidates of sequence i at free_stack[at ...] and unmaps them (i may be past the list: fc.n == 0).
+__device__ __forceinline__ void free_push(const CacheView& c, const int32_t* ids, int i, const FreeCand& fc, int at) {
+  if (fc.n == 0) return;
+  int32_t* tab = c.block_table + (size_t)ids[i] * c.max_blocks;
+#pragma unroll
+  for (int k = 0; k < kFreeCand; ++k) {
+    if (fc.pg[k] >= 0) {
+      c.free_stack[at++] = fc.pg[k];
+      tab[fc.b[k]] = -1;
+    }
+  }
+}
+
 // The whole eviction in one CTA (stand-alone kernel).
 __device__ __forceinline__ void evict_body(const CacheView& c, const int32_t* ids, int n, const SeqParams* sp_sh,
                                            int free_top0, int* s_ndead, int* s_off) {
