@@ -11,17 +11,22 @@
 // that share K/V: every 128-key K/V tile is staged once and used by both (M = 256 rows per staged tile).
 // Heaviest pairs (latest queries) are launched first.
 //
-// Per CTA, 10 warps:
+// Per CTA, 12 warps in three warpgroups (register budgets re-balanced with setmaxnreg: the softmax warps hold a
+// whole 128-key score row in registers):
 //   warp 0      TMA producer: Q blocks (tensor map over q, 128-byte swizzle written by the copy engine) and
 //               the K/V tiles, one box per (page, d-half) straight from the paged pools.  The pools' rows are
 //               stored pre-swizzled (16-byte chunk c of slot s at c ^ (s & 7), device_state.cuh); a
 //               [p slots][64 bf16] box of one d-half therefore lands as exactly the 128-byte-swizzled tile
 //               image tcgen05.mma expects - the decode kernels' layout needs no re-tiling.
-//   warp 1      MMA issuer (one lane): S_w = Q_w K^T (SS, both operands K-major) and O_w += P_w V (A = P from
-//               tensor memory, B = V MN-major), completion signalled with tcgen05.commit.  Issue order per
-//               tile j:  S(1,j)  PV(0,j)  S(0,j+1)  PV(1,j) - the two row blocks run half a period apart, so
-//               one warpgroup's softmax has the other's MMAs to hide under.
-//   warps 2-5 / 6-9   softmax warpgroup of row block 0 / 1: thread = row = TMEM lane.  Scores are read with
+//   warp 1      MMA issuer (ONE thread for the whole tile loop): S_w = Q_w K^T (SS, both operands K-major) and
+//               O_w += P_w V (A = P from tensor memory, B = V MN-major), completion signalled with tcgen05.commit.
+//               Issue order per tile j:  S(1,j)  PV(0,j)  S(0,j+1)  PV(1,j) - the two row blocks run half a period
+//               apart, so one warpgroup's softmax has the other's MMAs to hide under.  tcgen05.mma issue does not
+//               run ahead of the tensor pipe: every instruction the issuing thread executes between two MMAs is
+//               tensor-pipe idle time (profiles/r02_prefill_ncu.md, rate probes), so the loop holds nothing but
+//               the waits it needs, descriptor increments and the commits.
+//   warps 2-3   idle (they fill the issuer's warpgroup; setmaxnreg is per warpgroup)
+//   warps 4-7 / 8-11   softmax warpgroup of row block 0 / 1: thread = row = TMEM lane.  Scores are read with
 //               tcgen05.ld, masked on the diagonal, exponentiated in the exp2 domain; P is written back as
 //               bf16 over the first half of the S columns (tcgen05.st).  The running maximum is only raised
 //               when it grows by more than 2^8 (the accumulator is then rescaled in tensor memory), so the
@@ -42,16 +47,17 @@ constexpr int kBM = 128;                      // query rows per row block (TMEM 
 constexpr int kBN = 128;                      // keys per K/V tile
 constexpr int kHalfBytes = kBN * 128;         // one d-half of a 128-row tile: [128][64 bf16] = 16 KB
 constexpr int kUStages = 2;
-constexpr int kUThreads = 320;
+constexpr int kUThreads = 384;                // 3 warpgroups
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleLog2 = 8.f;           // raise the reference maximum only past 2^8
+constexpr int kRegsSoftmax = 224, kRegsOther = 56;  // 256 x 224 + 128 x 56 = 64512 = 384 x 168
 
 struct __align__(1024) USmem {
   uint8_t q[2][2][kHalfBytes];                // [row block][d-half]
   uint8_t k[kUStages][2][kHalfBytes];         // [stage][d-half]
   uint8_t v[kUStages][2][kHalfBytes];
   unsigned long long q_full, k_full[kUStages], v_full[kUStages], k_empty[kUStages], v_empty[kUStages];
-  unsigned long long s_ready[2], p_ready[2], o_done[2];
+  unsigned long long s_ready[2], p_half[2][2], o_done[2], v_clean;
   uint32_t tmem_base;
 };
 
@@ -61,6 +67,30 @@ struct UParams {
   int seq, pos_begin, n_tok, layer_begin;
   float sm_scale;
 };
+
+// packed fp32 pairs (sm_100a): halve the FFMA / FADD issue slots of the softmax
+__device__ __forceinline__ unsigned long long pack2f(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2f(unsigned long long v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsigned long long b) {
+  unsigned long long d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+template <int N>
+__device__ __forceinline__ void set_regs_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void set_regs_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
 __global__ void __launch_bounds__(kUThreads, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
@@ -91,6 +121,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
   }
   const int n_kt = max(nkt[0], nkt[1]);
   const int x_last = max(xl[0], act[1] ? xl[1] : 0);
+  // rows at or beyond the sequence length (inside the last mapped page) hold whatever the pool holds: their P is
+  // 0, but 0 * NaN would poison O - the producer warp zeroes them in the last tile before PV may read it
+  const int first_bad = len - (n_kt - 1) * kBN;
+  const bool need_clean = first_bad < kBN;
 
   // ---- set-up: barriers, tensor memory, finite K/V stages ------------------------------------------
   if (tid == 0) {
@@ -103,9 +137,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     }
     for (int w = 0; w < 2; ++w) {
       mbar_init(&s.s_ready[w], 1);
-      mbar_init(&s.p_ready[w], 4);  // one arrival per softmax warp
+      mbar_init(&s.p_half[w][0], 4);  // one arrival per softmax warp
+      mbar_init(&s.p_half[w][1], 4);
       mbar_init(&s.o_done[w], 1);
     }
+    mbar_init(&s.v_clean, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k);
@@ -129,116 +165,131 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
   }
   constexpr uint32_t tb = 0u;
 
-  if (warp == 0) {
-    // ============================== TMA producer ==============================
-    if (lane == 0) {
-      mbar_expect_tx(&s.q_full, (uint32_t)((act[0] + act[1]) * 2 * kHalfBytes));
-#pragma unroll
-      for (int w = 0; w < 2; ++w)
-        if (act[w])
-          for (int h = 0; h < 2; ++h) tma_load_4d(&s.q[w][h][0], &tm_q, 64 * h, hq[w], x0[w] - prm.pos_begin, lc, &s.q_full);
-      const int32_t* tab = c.block_table + (size_t)prm.seq * c.max_blocks;
-      const int ppt = kBN >> plog;  // pages per tile
-      for (int j = 0; j < n_kt; ++j) {
-        const int st = j % kUStages;
-        const uint32_t ph = (uint32_t)(j / kUStages) & 1u;
-        mbar_wait(&s.k_empty[st], ph ^ 1u);
-        const int rows = min(kBN, x_last + 1 - j * kBN);   // keys beyond x_last are never needed
-        const int pages = (rows + p - 1) >> plog;           // whole pages (all mapped: x_last < len)
-        const uint32_t bytes = (uint32_t)pages * (uint32_t)p * kRowBytes;
-        mbar_expect_tx(&s.k_full[st], bytes);
-        for (int pg = 0; pg < pages; ++pg) {
-          const int page = tab[j * ppt + pg];
-          for (int h = 0; h < 2; ++h) tma_load_5d(&s.k[st][h][pg * p * 128], &tm_k, 64 * h, 0, kvh, page, layer, &s.k_full[st]);
-        }
-        mbar_wait(&s.v_empty[st], ph ^ 1u);
-        mbar_expect_tx(&s.v_full[st], bytes);
-        for (int pg = 0; pg < pages; ++pg) {
-          const int page = tab[j * ppt + pg];
-          for (int h = 0; h < 2; ++h) tma_load_5d(&s.v[st][h][pg * p * 128], &tm_v, 64 * h, 0, kvh, page, layer, &s.v_full[st]);
-        }
-      }
-    }
-  } else if (warp == 1) {
-    // ============================== MMA issuer ==============================
-    const uint32_t idesc_s = umma_idesc_bf16(kBM, kBN, 0, 0);   // S = Q K^T: A, B K-major
-    const uint32_t idesc_o = umma_idesc_bf16(kBM, 128, 0, 1);   // O += P V: A from TMEM, B (V) MN-major, N = d = 128
-    mbar_wait(&s.q_full, 0u);
-    // Issue order (the two row blocks half a period apart, so that one warpgroup's softmax always runs
-    // under the other's MMAs):  S(0,0);  then per tile j:  S(1,j)  PV(0,j)  S(0,j+1)  PV(1,j).
-    // S_w aliases P_w: S(w,j+1) is issued after PV(w,j), and tcgen05.mma executes in issue order.
-    // Descriptors: one base per operand tile, the k-steps only add to the start-address field.  The row block is a
-    // compile-time constant of each call so that descriptors and TMEM addresses are formed on the uniform datapath:
-    // the issuing warp shares its scheduler with softmax warps, and every extra instruction (or register -> uniform
-    // register move) between two tcgen05.mma shows up as tensor-pipe idle time.
-    constexpr std::integral_constant<int, 0> W0{};
-    constexpr std::integral_constant<int, 1> W1{};
-    auto issue_s = [&](auto wc, int j) {  // S_w = Q_w K_j^T
-      constexpr int w = decltype(wc)::value;
-      const int st = j % kUStages;
-      mbar_wait(&s.k_full[st], (uint32_t)(j / kUStages) & 1u);
-      tc_fence_after();
+  if (warp < 4) {
+    set_regs_dec<kRegsOther>();
+    if (warp == 0) {
+      // ============================== TMA producer ==============================
       if (lane == 0) {
-        const uint64_t qd0 = smem_desc_kmajor(smem_u32(&s.q[w][0][0])), qd1 = smem_desc_kmajor(smem_u32(&s.q[w][1][0]));
-        const uint64_t kd0 = smem_desc_kmajor(smem_u32(&s.k[st][0][0])), kd1 = smem_desc_kmajor(smem_u32(&s.k[st][1][0]));
+        mbar_expect_tx(&s.q_full, (uint32_t)((act[0] + act[1]) * 2 * kHalfBytes));
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk) umma_ss(tb + 128u * w, qd0 + 2u * kk, kd0 + 2u * kk, idesc_s, kk ? 1u : 0u);  // +32 bytes per k-step
-#pragma unroll
-        for (int kk = 0; kk < 4; ++kk) umma_ss(tb + 128u * w, qd1 + 2u * kk, kd1 + 2u * kk, idesc_s, 1u);
-        umma_commit(&s.s_ready[w]);
+        for (int w = 0; w < 2; ++w)
+          if (act[w])
+            for (int h = 0; h < 2; ++h) tma_load_4d(&s.q[w][h][0], &tm_q, 64 * h, hq[w], x0[w] - prm.pos_begin, lc, &s.q_full);
+        const int32_t* tab = c.block_table + (size_t)prm.seq * c.max_blocks;
+        const int ppt = kBN >> plog;  // pages per tile
+        for (int j = 0; j < n_kt; ++j) {
+          const int st = j % kUStages;
+          const uint32_t ph = (uint32_t)(j / kUStages) & 1u;
+          mbar_wait(&s.k_empty[st], ph ^ 1u);
+          const int rows = min(kBN, x_last + 1 - j * kBN);   // keys beyond x_last are never needed
+          const int pages = (rows + p - 1) >> plog;           // whole pages (all mapped: x_last < len)
+          const uint32_t bytes = (uint32_t)pages * (uint32_t)p * kRowBytes;
+          mbar_expect_tx(&s.k_full[st], bytes);
+          for (int pg = 0; pg < pages; ++pg) {
+            const int page = tab[j * ppt + pg];
+            for (int h = 0; h < 2; ++h) tma_load_5d(&s.k[st][h][pg * p * 128], &tm_k, 64 * h, 0, kvh, page, layer, &s.k_full[st]);
+          }
+          mbar_wait(&s.v_empty[st], ph ^ 1u);
+          mbar_expect_tx(&s.v_full[st], bytes);
+          for (int pg = 0; pg < pages; ++pg) {
+            const int page = tab[j * ppt + pg];
+            for (int h = 0; h < 2; ++h) tma_load_5d(&s.v[st][h][pg * p * 128], &tm_v, 64 * h, 0, kvh, page, layer, &s.v_full[st]);
+          }
+        }
       }
       __syncwarp();
-    };
-    auto issue_pv = [&](auto wc, int j) {  // O_w += P_w V_j
-      constexpr int w = decltype(wc)::value;
-      const int st = j % kUStages;
-      mbar_wait(&s.p_ready[w], (uint32_t)j & 1u);
-      tc_fence_after();
-      if (lane == 0) {
-        const uint64_t vd = smem_desc_mnmajor(smem_u32(&s.v[st][0][0]), kHalfBytes);
-        const uint32_t acc = j ? 1u : 0u;
-        umma_ts(tb + 256u + 128u * w, tb + 128u * w, vd, idesc_o, acc);
-#pragma unroll
-        for (int kk = 1; kk < 8; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk.. (+2048 bytes = +128)
-          umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, vd + 128u * kk, idesc_o, 1u);
-        umma_commit(&s.o_done[w]);
-      }
-      __syncwarp();
-    };
-    if (nkt[0] > 0) issue_s(W0, 0);
-    for (int j = 0; j < n_kt; ++j) {
-      const int st = j % kUStages;
-      if (j < nkt[1]) issue_s(W1, j);
-      if (lane == 0) umma_commit(&s.k_empty[st]);  // K_j: both S(0,j) and S(1,j) are behind this point
-      __syncwarp();
-      mbar_wait(&s.v_full[st], (uint32_t)(j / kUStages) & 1u);
-      // rows at or beyond the sequence length (inside the last mapped page) hold whatever the pool holds:
-      // their P is 0, but 0 * NaN would poison O - zero them
-      const int first_bad = len - j * kBN;
-      if (first_bad < kBN) {
-        for (int i = lane; i < (kBN - max(first_bad, 0)) * 16; i += 32) {
-          const int r = max(first_bad, 0) + (i >> 4), ch = i & 15;
+      if (need_clean) {  // the whole warp: zero the V rows at / beyond the sequence length in the last tile
+        const int jl = n_kt - 1, st = jl % kUStages;
+        mbar_wait(&s.v_full[st], (uint32_t)(jl / kUStages) & 1u);
+        const int fb = max(first_bad, 0);
+        for (int i = lane; i < (kBN - fb) * 16; i += 32) {
+          const int r = fb + (i >> 4), ch = i & 15;
           *reinterpret_cast<uint4*>(&s.v[st][ch >> 3][r * 128 + (ch & 7) * 16]) = make_uint4(0u, 0u, 0u, 0u);
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
+        if (lane == 0) mbar_arrive(&s.v_clean);
       }
-      if (j < nkt[0]) issue_pv(W0, j);
-      if (j + 1 < nkt[0]) issue_s(W0, j + 1);
-      if (j < nkt[1]) issue_pv(W1, j);
-      if (lane == 0) umma_commit(&s.v_empty[st]);
-      __syncwarp();
+    } else if (warp == 1 && lane == 0) {
+      // ============================== MMA issuer (one thread) ==============================
+      constexpr uint32_t idesc_s = umma_idesc_bf16(kBM, kBN, 0, 0);   // S = Q K^T: A, B K-major
+      constexpr uint32_t idesc_o = umma_idesc_bf16(kBM, 128, 0, 1);   // O += P V: A from TMEM, B (V) MN-major, N = d = 128
+      // One descriptor per operand array; tiles, d-halves and k-steps only add to the 14-bit start-address field
+      // (16-byte units; everything lives below 256 KB, so no carry leaves the field).
+      const uint64_t qd = smem_desc_kmajor(smem_u32(&s.q[0][0][0]));
+      const uint64_t kd = smem_desc_kmajor(smem_u32(&s.k[0][0][0]));
+      const uint64_t vd = smem_desc_mnmajor(smem_u32(&s.v[0][0][0]), kHalfBytes);
+      constexpr uint32_t kHalfU = kHalfBytes >> 4, kTileU = 2 * kHalfU;
+      int k_seen = -1, v_seen = -1;  // tiles whose full barrier this thread has already observed
+      auto need_k = [&](int j) {
+        if (k_seen < j) {
+          mbar_wait(&s.k_full[j % kUStages], (uint32_t)(j / kUStages) & 1u);
+          k_seen = j;
+        }
+      };
+      auto need_v = [&](int j) {
+        if (v_seen < j) {
+          mbar_wait(&s.v_full[j % kUStages], (uint32_t)(j / kUStages) & 1u);
+          if (need_clean && j == n_kt - 1) mbar_wait(&s.v_clean, 0u);
+          v_seen = j;
+        }
+      };
+      auto issue_s = [&](auto wc, int j) {  // S_w = Q_w K_j^T
+        constexpr int w = decltype(wc)::value;
+        need_k(j);
+        tc_fence_after();
+        const uint64_t qa = qd + (uint32_t)w * kTileU, ka = kd + (uint32_t)(j % kUStages) * kTileU;
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)  // +32 bytes per k-step inside a d-half, +16 KB for the second d-half
+          umma_ss(tb + 128u * w, qa + (kk >> 2) * kHalfU + 2u * (kk & 3), ka + (kk >> 2) * kHalfU + 2u * (kk & 3), idesc_s, kk ? 1u : 0u);
+        umma_commit(&s.s_ready[w]);
+      };
+      auto issue_pv = [&](auto wc, int j) {  // O_w += P_w V_j, in two halves of 64 keys as P arrives
+        constexpr int w = decltype(wc)::value;
+        need_v(j);
+        const uint64_t va = vd + (uint32_t)(j % kUStages) * kTileU;
+        mbar_wait(&s.p_half[w][0], (uint32_t)j & 1u);
+        tc_fence_after();
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk.. (+2048 bytes = +128)
+          umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, va + 128u * kk, idesc_o, (j | kk) ? 1u : 0u);
+        mbar_wait(&s.p_half[w][1], (uint32_t)j & 1u);
+        tc_fence_after();
+#pragma unroll
+        for (int kk = 4; kk < 8; ++kk)
+          umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, va + 128u * kk, idesc_o, 1u);
+        umma_commit(&s.o_done[w]);
+      };
+      constexpr std::integral_constant<int, 0> W0{};
+      constexpr std::integral_constant<int, 1> W1{};
+      mbar_wait(&s.q_full, 0u);
+      // Issue order (the two row blocks half a period apart, so that one warpgroup's softmax always runs
+      // under the other's MMAs):  S(0,0);  then per tile j:  S(1,j)  PV(0,j)  S(0,j+1)  PV(1,j).
+      // S_w aliases P_w: S(w,j+1) is issued after PV(w,j), and tcgen05.mma executes in issue order.
+      if (nkt[0] > 0) issue_s(W0, 0);
+      for (int j = 0; j < n_kt; ++j) {
+        const int st = j % kUStages;
+        if (j < nkt[1]) issue_s(W1, j);
+        umma_commit(&s.k_empty[st]);  // K_j: both S(0,j) and S(1,j) are behind this point
+        if (j < nkt[0]) issue_pv(W0, j);
+        if (j + 1 < nkt[0]) issue_s(W0, j + 1);
+        if (j < nkt[1]) issue_pv(W1, j);
+        umma_commit(&s.v_empty[st]);
+      }
     }
   } else {
     // ============================== softmax warpgroups ==============================
-    const int w = (warp - 2) >> 2;         // row block of this warpgroup
+    set_regs_inc<kRegsSoftmax>();
+    const int w = (warp - 4) >> 2;         // row block of this warpgroup
     const int q4 = warp & 3;               // TMEM lane quarter this warp may access
     const int row = q4 * 32 + lane;
     const int x = x0[w] + row;             // this thread's query position
     const uint32_t lane_base = tb + ((uint32_t)(q4 * 32) << 16);
     const uint32_t s_addr = lane_base + 128u * w, o_addr = lane_base + 256u + 128u * w;
     const float c2 = prm.sm_scale * 1.4426950408889634f;
-    float m = -INFINITY, l = 0.f;
+    const unsigned long long c2p = pack2f(c2, c2);
+    float m = -INFINITY;
+    unsigned long long l2 = pack2f(0.f, 0.f);
     const int n = nkt[w];
     for (int j = 0; j < n; ++j) {
       mbar_wait(&s.s_ready[w], (uint32_t)j & 1u);
@@ -261,10 +312,15 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         for (int i = 0; i < 128; ++i)
           if (y0 + i > x) sc[i] = 0xff800000u;  // -inf
       }
-      float mx = -INFINITY;
+      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
-      for (int i = 0; i < 128; ++i) mx = fmaxf(mx, __uint_as_float(sc[i]));
-      float m_new = fmaxf(m, mx);
+      for (int i = 0; i < 32; ++i) {
+        mx0 = fmaxf(mx0, __uint_as_float(sc[i]));
+        mx1 = fmaxf(mx1, __uint_as_float(sc[32 + i]));
+        mx2 = fmaxf(mx2, __uint_as_float(sc[64 + i]));
+        mx3 = fmaxf(mx3, __uint_as_float(sc[96 + i]));
+      }
+      const float m_new = fmaxf(fmaxf(m, fmaxf(mx0, mx1)), fmaxf(mx2, mx3));
       if (j == 0) {
         m = m_new;  // key 0 <= every query position: finite
       } else {
@@ -283,32 +339,41 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
             tmem_st32(o_addr + 32 * cc, o);
           }
-          l *= f;
+          float la, lb;
+          unpack2f(l2, la, lb);
+          l2 = pack2f(la * f, lb * f);
           if (need) m = m_new;
         }
       }
-      const float ms = m * c2;
+      const float ms = -m * c2;
+      const unsigned long long msp = pack2f(ms, ms);
 #pragma unroll
       for (int cc = 0; cc < 4; ++cc) {
         uint32_t pk[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-          const float p0 = ex2(fmaf(__uint_as_float(sc[32 * cc + 2 * i]), c2, -ms));
-          const float p1 = ex2(fmaf(__uint_as_float(sc[32 * cc + 2 * i + 1]), c2, -ms));
-          l += p0 + p1;
+          float e0, e1;
+          unpack2f(ffma2(pack2f(__uint_as_float(sc[32 * cc + 2 * i]), __uint_as_float(sc[32 * cc + 2 * i + 1])), c2p, msp), e0, e1);
+          const float p0 = ex2(e0), p1 = ex2(e1);
+          l2 = fadd2(l2, pack2f(p0, p1));
           pk[i] = pack_bf16(p0, p1);
         }
         tmem_st16(s_addr + 16 * cc, pk);
+        if (cc & 1) {  // 64 keys of P are in tensor memory: PV may start on them
+          tmem_wait_st();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&s.p_half[w][cc >> 1]);
+        }
       }
-      tmem_wait_st();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&s.p_ready[w]);
     }
     if (n > 0) {
       // ---- epilogue: O / l -> bf16 -> out ----
       mbar_wait(&s.o_done[w], (uint32_t)(n - 1) & 1u);
       tc_fence_after();
+      float la, lb;
+      unpack2f(l2, la, lb);
+      const float l = la + lb;
       const float inv = 1.f / l;
       const bool valid = x <= xl[w];
       const size_t orow = ((size_t)lc * prm.n_tok + (size_t)(x - prm.pos_begin)) * c.n_q + hq[w];
