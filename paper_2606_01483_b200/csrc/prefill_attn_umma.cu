@@ -57,7 +57,7 @@ struct __align__(1024) USmem {
   uint8_t k[kUStages][2][kHalfBytes];         // [stage][d-half]
   uint8_t v[kUStages][2][kHalfBytes];
   unsigned long long q_full, k_full[kUStages], v_full[kUStages], k_empty[kUStages], v_empty[kUStages];
-  unsigned long long s_ready[2], p_half[2][2], o_done[2], v_clean;
+  unsigned long long s_ready[2], p_half[2][2], o_half[2], o_done[2], v_clean;
   uint32_t tmem_base;
 };
 
@@ -87,6 +87,41 @@ __device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsign
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
   return d;
 }
+#ifdef MURMUR_PFTRACE
+// Profiling builds only (-DMURMUR_PFTRACE): clock stamps of the issuing thread and of one lane per softmax
+// warpgroup, for the heaviest work item of (KV head 0, first layer of the call).
+__device__ long long g_pftrace[3][2048];
+#define PFT(role, idx) do { if (trace_cta && (idx) < 2048) g_pftrace[role][idx] = clock64(); } while (0)
+#else
+#define PFT(role, idx) do { } while (0)
+#endif
+
+// exp2 of a packed pair on the FMA pipes (the SFUs do 16 exp2 per clock and SM: as many cycles per 128-key tile
+// as its two MMA groups, so part of the exponentials is taken off them): x = n + f with n = round(x), f in
+// [-1/2, 1/2]; 2^f by a cubic (minimax in relative error, 7.5e-5 - P is rounded to bf16, 2^-9, right after);
+// 2^n by adding n to the exponent field.  x + 1.5 * 2^23 leaves round(x) in the low mantissa bits.
+__device__ __forceinline__ unsigned long long ex2_fma2(unsigned long long x2) {
+  float x0, x1;
+  unpack2f(x2, x0, x1);
+  const unsigned long long xc = pack2f(fmaxf(x0, -125.f), fmaxf(x1, -125.f));  // keeps 2^n normal (and -inf finite)
+  const unsigned long long magic = pack2f(12582912.f, 12582912.f);
+  const unsigned long long t = fadd2(xc, magic);
+  const unsigned long long nf = fadd2(t, pack2f(-12582912.f, -12582912.f));
+  const unsigned long long f = ffma2(nf, pack2f(-1.f, -1.f), xc);
+  unsigned long long q = ffma2(f, pack2f(0.05517132207751274f, 0.05517132207751274f), pack2f(0.24261054396629333f, 0.24261054396629333f));
+  q = ffma2(q, f, pack2f(0.6932609677314758f, 0.6932609677314758f));
+  q = ffma2(q, f, pack2f(0.9999281167984009f, 0.9999281167984009f));
+  float q0, q1, t0, t1;
+  unpack2f(q, q0, q1);
+  unpack2f(t, t0, t1);
+  return pack2f(__uint_as_float(__float_as_uint(q0) + (__float_as_uint(t0) << 23)),
+                __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23)));
+}
+#ifndef MURMUR_PF_EMU_OF_8
+#define MURMUR_PF_EMU_OF_8 3
+#endif
+constexpr int kEmuOf8 = MURMUR_PF_EMU_OF_8;   // of every 8 pairs, this many take the FMA route
+
 template <int N>
 __device__ __forceinline__ void set_regs_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N>
@@ -107,6 +142,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
   const int pair = n_pairs - 1 - (int)blockIdx.x;  // heaviest first
   const int pos_end = prm.pos_begin + prm.n_tok;
   const int len = c.seqs[prm.seq].len;
+#ifdef MURMUR_PFTRACE
+  const bool trace_cta = blockIdx.x == 1 && blockIdx.y == 0 && blockIdx.z == 0;
+#endif
 
   int act[2], hq[2], x0[2], xl[2], nkt[2];
 #pragma unroll
@@ -140,6 +178,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       mbar_init(&s.p_half[w][0], 4);  // one arrival per softmax warp
       mbar_init(&s.p_half[w][1], 4);
       mbar_init(&s.o_done[w], 1);
+      mbar_init(&s.o_half[w], 1);
     }
     mbar_init(&s.v_clean, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -210,8 +249,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         __syncwarp();
         if (lane == 0) mbar_arrive(&s.v_clean);
       }
-    } else if (warp == 1 && lane == 0) {
-      // ============================== MMA issuer (one thread) ==============================
+    } else if (warp == 1) {
+      // ============================== MMA issuer ==============================
+      // The whole warp walks the loop (waits, tile arithmetic: all warp-uniform, so descriptors and tensor-memory
+      // addresses are formed on the uniform datapath); one elected lane issues.
+      const bool leader = elect_one();
       constexpr uint32_t idesc_s = umma_idesc_bf16(kBM, kBN, 0, 0);   // S = Q K^T: A, B K-major
       constexpr uint32_t idesc_o = umma_idesc_bf16(kBM, 128, 0, 1);   // O += P V: A from TMEM, B (V) MN-major, N = d = 128
       // One descriptor per operand array; tiles, d-halves and k-steps only add to the 14-bit start-address field
@@ -238,27 +280,44 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         constexpr int w = decltype(wc)::value;
         need_k(j);
         tc_fence_after();
+        PFT(0, 16 * j + (w ? 0 : 6) + 0);
         const uint64_t qa = qd + (uint32_t)w * kTileU, ka = kd + (uint32_t)(j % kUStages) * kTileU;
+        if (leader) {
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)  // +32 bytes per k-step inside a d-half, +16 KB for the second d-half
-          umma_ss(tb + 128u * w, qa + (kk >> 2) * kHalfU + 2u * (kk & 3), ka + (kk >> 2) * kHalfU + 2u * (kk & 3), idesc_s, kk ? 1u : 0u);
-        umma_commit(&s.s_ready[w]);
+          for (int kk = 0; kk < 8; ++kk)  // +32 bytes per k-step inside a d-half, +16 KB for the second d-half
+            umma_ss(tb + 128u * w, qa + (kk >> 2) * kHalfU + 2u * (kk & 3), ka + (kk >> 2) * kHalfU + 2u * (kk & 3), idesc_s, kk ? 1u : 0u);
+          umma_commit(&s.s_ready[w]);
+        }
+        __syncwarp();
+        PFT(0, 16 * j + (w ? 0 : 6) + 1);
       };
       auto issue_pv = [&](auto wc, int j) {  // O_w += P_w V_j, in two halves of 64 keys as P arrives
         constexpr int w = decltype(wc)::value;
         need_v(j);
         const uint64_t va = vd + (uint32_t)(j % kUStages) * kTileU;
+        PFT(0, 16 * j + (w ? 8 : 2) + 0);
         mbar_wait(&s.p_half[w][0], (uint32_t)j & 1u);
         tc_fence_after();
+        PFT(0, 16 * j + (w ? 8 : 2) + 1);
+        if (leader) {
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk.. (+2048 bytes = +128)
-          umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, va + 128u * kk, idesc_o, (j | kk) ? 1u : 0u);
+          for (int kk = 0; kk < 4; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk.. (+2048 bytes = +128)
+            umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, va + 128u * kk, idesc_o, (j | kk) ? 1u : 0u);
+          umma_commit(&s.o_half[w]);  // (a rescale triggered by the second half waits for these)
+        }
+        __syncwarp();
+        PFT(0, 16 * j + (w ? 8 : 2) + 2);
         mbar_wait(&s.p_half[w][1], (uint32_t)j & 1u);
         tc_fence_after();
+        PFT(0, 16 * j + (w ? 8 : 2) + 3);
+        if (leader) {
 #pragma unroll
-        for (int kk = 4; kk < 8; ++kk)
-          umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, va + 128u * kk, idesc_o, 1u);
-        umma_commit(&s.o_done[w]);
+          for (int kk = 4; kk < 8; ++kk)
+            umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, va + 128u * kk, idesc_o, 1u);
+          umma_commit(&s.o_done[w]);
+        }
+        __syncwarp();
+        PFT(0, 16 * j + 12 + w);
       };
       constexpr std::integral_constant<int, 0> W0{};
       constexpr std::integral_constant<int, 1> W1{};
@@ -270,11 +329,13 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       for (int j = 0; j < n_kt; ++j) {
         const int st = j % kUStages;
         if (j < nkt[1]) issue_s(W1, j);
-        umma_commit(&s.k_empty[st]);  // K_j: both S(0,j) and S(1,j) are behind this point
+        if (leader) umma_commit(&s.k_empty[st]);  // K_j: both S(0,j) and S(1,j) are behind this point
+        __syncwarp();
         if (j < nkt[0]) issue_pv(W0, j);
         if (j + 1 < nkt[0]) issue_s(W0, j + 1);
         if (j < nkt[1]) issue_pv(W1, j);
-        umma_commit(&s.v_empty[st]);
+        if (leader) umma_commit(&s.v_empty[st]);
+        __syncwarp();
       }
     }
   } else {
@@ -291,80 +352,99 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     float m = -INFINITY;
     unsigned long long l2 = pack2f(0.f, 0.f);
     const int n = nkt[w];
+    // The reference maximum m of a row is LAZY: a half tile (64 keys) is exponentiated against the m left by the
+    // halves before it and only when it tops m by more than 2^8 are O and l rescaled first - so no pass over the
+    // whole 128-key row precedes the first exp2, the second half's tcgen05.ld hides under the first half's
+    // exponentials, and l and O always share one reference (exact in the end).
     for (int j = 0; j < n; ++j) {
+      if (q4 == 0 && lane == 0) PFT(1 + w, 8 * j + 0);
       mbar_wait(&s.s_ready[w], (uint32_t)j & 1u);
       tc_fence_after();
-      uint32_t sc[128];
+      if (q4 == 0 && lane == 0) PFT(1 + w, 8 * j + 1);
+      uint32_t sc[2][64];
       {
-        uint32_t(&a0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[0]);
-        uint32_t(&a1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[32]);
-        uint32_t(&a2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[64]);
-        uint32_t(&a3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[96]);
+        uint32_t(&a0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[0][0]);
+        uint32_t(&a1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[0][32]);
         tmem_ld32(s_addr, a0);
         tmem_ld32(s_addr + 32, a1);
-        tmem_ld32(s_addr + 64, a2);
-        tmem_ld32(s_addr + 96, a3);
         tmem_wait_ld();
+        uint32_t(&a2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[1][0]);
+        uint32_t(&a3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[1][32]);
+        tmem_ld32(s_addr + 64, a2);   // lands while the first half is exponentiated
+        tmem_ld32(s_addr + 96, a3);
       }
+      if (q4 == 0 && lane == 0) PFT(1 + w, 8 * j + 2);
       const int y0 = j * kBN;
-      if (y0 + kBN - 1 > x0[w]) {  // the tile reaches past the first row's position: causal mask
+      const bool diag = y0 + kBN - 1 > x0[w];  // the tile reaches past the first row's position: causal mask
 #pragma unroll
-        for (int i = 0; i < 128; ++i)
-          if (y0 + i > x) sc[i] = 0xff800000u;  // -inf
-      }
-      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+      for (int h = 0; h < 2; ++h) {
+        if (h == 1) tmem_wait_ld();
+        if (diag) {
 #pragma unroll
-      for (int i = 0; i < 32; ++i) {
-        mx0 = fmaxf(mx0, __uint_as_float(sc[i]));
-        mx1 = fmaxf(mx1, __uint_as_float(sc[32 + i]));
-        mx2 = fmaxf(mx2, __uint_as_float(sc[64 + i]));
-        mx3 = fmaxf(mx3, __uint_as_float(sc[96 + i]));
-      }
-      const float m_new = fmaxf(fmaxf(m, fmaxf(mx0, mx1)), fmaxf(mx2, mx3));
-      if (j == 0) {
-        m = m_new;  // key 0 <= every query position: finite
-      } else {
-        const bool need = (m_new - m) * c2 > kRescaleLog2;
-        if (__any_sync(0xffffffffu, need)) {
-          // rescale O (and l) of the rows whose reference maximum moves; PV of the previous tile must have landed
-          mbar_wait(&s.o_done[w], (uint32_t)(j - 1) & 1u);
-          tc_fence_after();
-          const float f = need ? ex2((m - m_new) * c2) : 1.f;
+          for (int i = 0; i < 64; ++i)
+            if (y0 + 64 * h + i > x) sc[h][i] = 0xff800000u;  // -inf
+        }
+        float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
-          for (int cc = 0; cc < 4; ++cc) {
-            uint32_t o[32];
-            tmem_ld32(o_addr + 32 * cc, o);
-            tmem_wait_ld();
+        for (int i = 0; i < 32; ++i) {
+          mx0 = fmaxf(mx0, __uint_as_float(sc[h][i]));
+          mx1 = fmaxf(mx1, __uint_as_float(sc[h][32 + i]));
+        }
+        const float hmax = fmaxf(mx0, mx1);
+        if (j == 0 && h == 0) {
+          m = hmax;  // key 0 <= every query position: finite; nothing accumulated yet
+        } else {
+          const bool need = (hmax - m) * c2 > kRescaleLog2;
+          if (__any_sync(0xffffffffu, need)) {
+            // rescale O and l of the rows whose reference moves.  Everything issued into O_w so far must have landed:
+            // PV(w, j-1) has (S(w, j) was issued behind it), the first half of PV(w, j) is waited for.
+            if (h == 1) mbar_wait(&s.o_half[w], (uint32_t)j & 1u);
+            tc_fence_after();
+            const float f = need ? ex2((m - hmax) * c2) : 1.f;
 #pragma unroll
-            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
-            tmem_st32(o_addr + 32 * cc, o);
+            for (int cc = 0; cc < 4; ++cc) {
+              uint32_t o[32];
+              tmem_ld32(o_addr + 32 * cc, o);
+              tmem_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+              tmem_st32(o_addr + 32 * cc, o);
+            }
+            float la, lb;
+            unpack2f(l2, la, lb);
+            l2 = pack2f(la * f, lb * f);
+            if (need) m = hmax;
           }
-          float la, lb;
-          unpack2f(l2, la, lb);
-          l2 = pack2f(la * f, lb * f);
-          if (need) m = m_new;
         }
-      }
-      const float ms = -m * c2;
-      const unsigned long long msp = pack2f(ms, ms);
+        const float ms = -m * c2;
+        const unsigned long long msp = pack2f(ms, ms);
 #pragma unroll
-      for (int cc = 0; cc < 4; ++cc) {
-        uint32_t pk[16];
+        for (int cc = 0; cc < 2; ++cc) {
+          uint32_t pk[16];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          float e0, e1;
-          unpack2f(ffma2(pack2f(__uint_as_float(sc[32 * cc + 2 * i]), __uint_as_float(sc[32 * cc + 2 * i + 1])), c2p, msp), e0, e1);
-          const float p0 = ex2(e0), p1 = ex2(e1);
-          l2 = fadd2(l2, pack2f(p0, p1));
-          pk[i] = pack_bf16(p0, p1);
+          for (int i = 0; i < 16; ++i) {
+            const unsigned long long e2 = ffma2(pack2f(__uint_as_float(sc[h][32 * cc + 2 * i]), __uint_as_float(sc[h][32 * cc + 2 * i + 1])), c2p, msp);
+            float p0, p1;
+            if ((i & 7) < kEmuOf8) {
+              const unsigned long long pp = ex2_fma2(e2);
+              unpack2f(pp, p0, p1);
+              l2 = fadd2(l2, pp);
+            } else {
+              float e0, e1;
+              unpack2f(e2, e0, e1);
+              p0 = ex2(e0), p1 = ex2(e1);
+              l2 = fadd2(l2, pack2f(p0, p1));
+            }
+            pk[i] = pack_bf16(p0, p1);
+          }
+          tmem_st16(s_addr + 32 * h + 16 * cc, pk);
         }
-        tmem_st16(s_addr + 16 * cc, pk);
-        if (cc & 1) {  // 64 keys of P are in tensor memory: PV may start on them
-          tmem_wait_st();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&s.p_half[w][cc >> 1]);
-        }
+        // 64 keys of P are in tensor memory: PV may start on them
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&s.p_half[w][h]);
+        if (q4 == 0 && lane == 0) PFT(1 + w, 8 * j + 4 + h);
       }
     }
     if (n > 0) {
@@ -447,3 +527,10 @@ cudaError_t launch_prefill_attn_umma(const CacheView& c, int seq, int pos_begin,
 }
 
 }  // namespace murmur
+
+#ifdef MURMUR_PFTRACE
+extern "C" __attribute__((visibility("default"))) int murmur_debug_pftrace(long long* host_out) {
+  cudaDeviceSynchronize();
+  return (int)cudaMemcpyFromSymbol(host_out, murmur::g_pftrace, sizeof(long long) * 3 * 2048);
+}
+#endif

@@ -84,6 +84,31 @@ def test_prefill_chunked_unaligned_ranges_and_layer_range(dev):
     c.close()
 
 
+@pytest.mark.parametrize("page", [16, 64])
+def test_prefill_moving_row_maximum(dev, page):
+    """Scores that keep growing along the key axis: every row's reference maximum moves by far more than 2^8
+    again and again, in first and in second halves of the 128-key tiles (the kernel's lazy-maximum rescale of
+    O and l, incl. the case where the first half of the same tile's PV is already in flight)."""
+    L, n_tok = 1, 700
+    c = _cache(dev, L, n_tok, page)
+    k, v = _rand((L, n_tok, 4, 128), 21, dev), _rand((L, n_tok, 4, 128), 22, dev)
+    q = _rand((L, n_tok, 28, 128), 23, dev)
+    # a common direction u in q and k; its weight in k jumps at positions spread over both tile halves
+    u = torch.zeros(128, device=dev)
+    u[:8] = 1.0
+    q = (q.float() + 6.0 * u).to(torch.bfloat16)
+    step = torch.zeros(n_tok, device=dev)
+    for pos, amp in ((40, 2.0), (100, 4.0), (130, 6.0), (200, 8.0), (330, 10.0), (447, 12.0), (448, 14.0), (600, 16.0), (699, 18.0)):
+        step[pos:] = amp
+    k = (k.float() + step[None, :, None, None] * u).to(torch.bfloat16)
+    c.kv_append([0], [n_tok], k, v)
+    lse = torch.empty(L, n_tok, 28, dtype=torch.float32, device=dev)
+    out = c.prefill_attn(0, 0, n_tok, q, lse=lse)
+    _check(out, lse, q, k, v, 0, None, 1 / math.sqrt(128))
+    assert c.last_error() == 0
+    c.close()
+
+
 def test_prefill_config2_size_sampled_rows(dev):
     # one 300 s chunk: 64 prefix + 2250 speech tokens, 2 layers; rows around tile / page boundaries and the end
     cfg = workloads.config2().with_layers(2)
