@@ -47,17 +47,18 @@ constexpr int kBM = 128;                      // query rows per row block (TMEM 
 constexpr int kBN = 128;                      // keys per K/V tile
 constexpr int kHalfBytes = kBN * 128;         // one d-half of a 128-row tile: [128][64 bf16] = 16 KB
 constexpr int kUStages = 2;
-constexpr int kUThreads = 384;                // 3 warpgroups
+constexpr int kUThreads = 640;                // 5 warpgroups: {producer, issuer, 2 idle}, 2 x 2 softmax
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleLog2 = 8.f;           // raise the reference maximum only past 2^8
-constexpr int kRegsSoftmax = 224, kRegsOther = 56;  // 256 x 224 + 128 x 56 = 64512 = 384 x 168
+constexpr int kRegsSoftmax = 104, kRegsOther = 56;  // 512 x 104 + 128 x 56 = 60416 <= 640 x 96 (what the launch allocates)
 
 struct __align__(1024) USmem {
   uint8_t q[2][2][kHalfBytes];                // [row block][d-half]
   uint8_t k[kUStages][2][kHalfBytes];         // [stage][d-half]
   uint8_t v[kUStages][2][kHalfBytes];
   unsigned long long q_full, k_full[kUStages], v_full[kUStages], k_empty[kUStages], v_empty[kUStages];
-  unsigned long long s_ready[2], p_half[2][2], o_half[2], o_done[2], v_clean;
+  unsigned long long s_ready[2], p_ready[2], o_done[2], v_clean;
+  float mxch[2][2][kBM], lxch[2][2][kBM];  // row maxima / row sums exchanged between the two warps of a row
   uint32_t tmem_base;
 };
 
@@ -175,10 +176,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     }
     for (int w = 0; w < 2; ++w) {
       mbar_init(&s.s_ready[w], 1);
-      mbar_init(&s.p_half[w][0], 4);  // one arrival per softmax warp
-      mbar_init(&s.p_half[w][1], 4);
+      mbar_init(&s.p_ready[w], 8);  // one arrival per softmax warp
       mbar_init(&s.o_done[w], 1);
-      mbar_init(&s.o_half[w], 1);
     }
     mbar_init(&s.v_clean, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -291,29 +290,18 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         __syncwarp();
         PFT(0, 16 * j + (w ? 0 : 6) + 1);
       };
-      auto issue_pv = [&](auto wc, int j) {  // O_w += P_w V_j, in two halves of 64 keys as P arrives
+      auto issue_pv = [&](auto wc, int j) {  // O_w += P_w V_j
         constexpr int w = decltype(wc)::value;
         need_v(j);
         const uint64_t va = vd + (uint32_t)(j % kUStages) * kTileU;
         PFT(0, 16 * j + (w ? 8 : 2) + 0);
-        mbar_wait(&s.p_half[w][0], (uint32_t)j & 1u);
+        mbar_wait(&s.p_ready[w], (uint32_t)j & 1u);
         tc_fence_after();
         PFT(0, 16 * j + (w ? 8 : 2) + 1);
         if (leader) {
 #pragma unroll
-          for (int kk = 0; kk < 4; ++kk)  // 16 keys per instruction: P columns 8 kk.., V rows 16 kk.. (+2048 bytes = +128)
-            umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, va + 128u * kk, idesc_o, (j | kk) ? 1u : 0u);
-          umma_commit(&s.o_half[w]);  // (a rescale triggered by the second half waits for these)
-        }
-        __syncwarp();
-        PFT(0, 16 * j + (w ? 8 : 2) + 2);
-        mbar_wait(&s.p_half[w][1], (uint32_t)j & 1u);
-        tc_fence_after();
-        PFT(0, 16 * j + (w ? 8 : 2) + 3);
-        if (leader) {
-#pragma unroll
-          for (int kk = 4; kk < 8; ++kk)
-            umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk, va + 128u * kk, idesc_o, 1u);
+          for (int kk = 0; kk < 8; ++kk)  // 16 keys per instruction: P of keys 0..63 at columns 0..31, of keys 64..127 at columns 64..95; V rows 16 kk.. (+2048 bytes = +128)
+            umma_ts(tb + 256u + 128u * w, tb + 128u * w + 8u * kk + (kk >= 4 ? 32u : 0u), va + 128u * kk, idesc_o, (j | kk) ? 1u : 0u);
           umma_commit(&s.o_done[w]);
         }
         __syncwarp();
@@ -340,130 +328,141 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     }
   } else {
     // ============================== softmax warpgroups ==============================
+    // 16 warps: row block w = 8 warps = two per tensor-memory lane quarter; of a pair, warp `hs` owns the key
+    // columns [64 hs, 64 hs + 64) of every row of its quarter.  (Two warps per scheduler per row block: one
+    // warp alone runs the exp2 chain at a fraction of the SFU rate.)
     set_regs_inc<kRegsSoftmax>();
-    const int w = (warp - 4) >> 2;         // row block of this warpgroup
+    const int sw = warp - 4;
+    const int w = sw >> 3;                 // row block of this warp
+    const int hs = (sw >> 2) & 1;          // key half of this warp
     const int q4 = warp & 3;               // TMEM lane quarter this warp may access
     const int row = q4 * 32 + lane;
     const int x = x0[w] + row;             // this thread's query position
     const uint32_t lane_base = tb + ((uint32_t)(q4 * 32) << 16);
-    const uint32_t s_addr = lane_base + 128u * w, o_addr = lane_base + 256u + 128u * w;
+    const uint32_t s_addr = lane_base + 128u * w + 64u * hs;            // this thread's 64 score columns
+    const uint32_t o_addr = lane_base + 256u + 128u * w + 64u * hs;     // this thread's half of the O row
+    const int pair_bar = 1 + w * 4 + q4;   // named barrier of the two warps that share these rows
     const float c2 = prm.sm_scale * 1.4426950408889634f;
     const unsigned long long c2p = pack2f(c2, c2);
     float m = -INFINITY;
     unsigned long long l2 = pack2f(0.f, 0.f);
     const int n = nkt[w];
-    // The reference maximum m of a row is LAZY: a half tile (64 keys) is exponentiated against the m left by the
-    // halves before it and only when it tops m by more than 2^8 are O and l rescaled first - so no pass over the
-    // whole 128-key row precedes the first exp2, the second half's tcgen05.ld hides under the first half's
-    // exponentials, and l and O always share one reference (exact in the end).
     for (int j = 0; j < n; ++j) {
-      if (q4 == 0 && lane == 0) PFT(1 + w, 8 * j + 0);
+      if (q4 == 0 && lane == 0 && hs == 0) PFT(1 + w, 8 * j + 0);
       mbar_wait(&s.s_ready[w], (uint32_t)j & 1u);
       tc_fence_after();
-      if (q4 == 0 && lane == 0) PFT(1 + w, 8 * j + 1);
-      uint32_t sc[2][64];
+      if (q4 == 0 && lane == 0 && hs == 0) PFT(1 + w, 8 * j + 1);
+      // pass 1: this thread's 64 scores -> their maximum (the scores are read again in pass 2: tensor memory is
+      // closer than the registers a 64-value row segment would cost every one of the 512 softmax threads)
+      const bool diag = j * kBN + kBN - 1 > x0[w];  // the tile reaches past the first row's position: causal mask
+      const int y0 = j * kBN + 64 * hs;
+      float hmax;
       {
-        uint32_t(&a0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[0][0]);
-        uint32_t(&a1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[0][32]);
+        uint32_t sc[64];
+        uint32_t(&a0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[0]);
+        uint32_t(&a1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[32]);
         tmem_ld32(s_addr, a0);
         tmem_ld32(s_addr + 32, a1);
         tmem_wait_ld();
-        uint32_t(&a2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[1][0]);
-        uint32_t(&a3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sc[1][32]);
-        tmem_ld32(s_addr + 64, a2);   // lands while the first half is exponentiated
-        tmem_ld32(s_addr + 96, a3);
-      }
-      if (q4 == 0 && lane == 0) PFT(1 + w, 8 * j + 2);
-      const int y0 = j * kBN;
-      const bool diag = y0 + kBN - 1 > x0[w];  // the tile reaches past the first row's position: causal mask
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        if (h == 1) tmem_wait_ld();
         if (diag) {
 #pragma unroll
           for (int i = 0; i < 64; ++i)
-            if (y0 + 64 * h + i > x) sc[h][i] = 0xff800000u;  // -inf
+            if (y0 + i > x) sc[i] = 0xff800000u;  // -inf
         }
         float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
-          mx0 = fmaxf(mx0, __uint_as_float(sc[h][i]));
-          mx1 = fmaxf(mx1, __uint_as_float(sc[h][32 + i]));
+          mx0 = fmaxf(mx0, __uint_as_float(sc[i]));
+          mx1 = fmaxf(mx1, __uint_as_float(sc[32 + i]));
         }
-        const float hmax = fmaxf(mx0, mx1);
-        if (j == 0 && h == 0) {
-          m = hmax;  // key 0 <= every query position: finite; nothing accumulated yet
-        } else {
-          const bool need = (hmax - m) * c2 > kRescaleLog2;
-          if (__any_sync(0xffffffffu, need)) {
-            // rescale O and l of the rows whose reference moves.  Everything issued into O_w so far must have landed:
-            // PV(w, j-1) has (S(w, j) was issued behind it), the first half of PV(w, j) is waited for.
-            if (h == 1) mbar_wait(&s.o_half[w], (uint32_t)j & 1u);
-            tc_fence_after();
-            const float f = need ? ex2((m - hmax) * c2) : 1.f;
-#pragma unroll
-            for (int cc = 0; cc < 4; ++cc) {
-              uint32_t o[32];
-              tmem_ld32(o_addr + 32 * cc, o);
-              tmem_wait_ld();
-#pragma unroll
-              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
-              tmem_st32(o_addr + 32 * cc, o);
-            }
-            float la, lb;
-            unpack2f(l2, la, lb);
-            l2 = pack2f(la * f, lb * f);
-            if (need) m = hmax;
-          }
-        }
-        const float ms = -m * c2;
-        const unsigned long long msp = pack2f(ms, ms);
-#pragma unroll
-        for (int cc = 0; cc < 2; ++cc) {
-          uint32_t pk[16];
-#pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            const unsigned long long e2 = ffma2(pack2f(__uint_as_float(sc[h][32 * cc + 2 * i]), __uint_as_float(sc[h][32 * cc + 2 * i + 1])), c2p, msp);
-            float p0, p1;
-            if ((i & 7) < kEmuOf8) {
-              const unsigned long long pp = ex2_fma2(e2);
-              unpack2f(pp, p0, p1);
-              l2 = fadd2(l2, pp);
-            } else {
-              float e0, e1;
-              unpack2f(e2, e0, e1);
-              p0 = ex2(e0), p1 = ex2(e1);
-              l2 = fadd2(l2, pack2f(p0, p1));
-            }
-            pk[i] = pack_bf16(p0, p1);
-          }
-          tmem_st16(s_addr + 32 * h + 16 * cc, pk);
-        }
-        // 64 keys of P are in tensor memory: PV may start on them
-        tmem_wait_st();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&s.p_half[w][h]);
-        if (q4 == 0 && lane == 0) PFT(1 + w, 8 * j + 4 + h);
+        hmax = fmaxf(mx0, mx1);
       }
+      // row maximum = max over the two halves of the row
+      s.mxch[w][hs][row] = hmax;
+      asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
+      const float m_new = fmaxf(m, fmaxf(hmax, s.mxch[w][hs ^ 1][row]));
+      if (j == 0) {
+        m = m_new;  // key 0 <= every query position: finite
+      } else {
+        const bool need = (m_new - m) * c2 > kRescaleLog2;   // same decision in both warps of the pair
+        if (__any_sync(0xffffffffu, need)) {
+          // rescale (this thread's half of) O and l of the rows whose reference maximum moves; PV(w, j-1) has
+          // landed: S(w, j) was issued behind it
+          const float f = need ? ex2((m - m_new) * c2) : 1.f;
+#pragma unroll
+          for (int cc = 0; cc < 2; ++cc) {
+            uint32_t o[32];
+            tmem_ld32(o_addr + 32 * cc, o);
+            tmem_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+            tmem_st32(o_addr + 32 * cc, o);
+          }
+          float la, lb;
+          unpack2f(l2, la, lb);
+          l2 = pack2f(la * f, lb * f);
+          if (need) m = m_new;
+        }
+      }
+      if (q4 == 0 && lane == 0 && hs == 0) PFT(1 + w, 8 * j + 2);
+      // pass 2: P = exp2(c2 s - c2 m) as bf16 pairs, written over the first 32 of this thread's OWN 64 score
+      // columns (keys 64 hs + 32 cc .. at columns 64 hs + 16 cc ..): no thread writes what another still reads
+      const float ms = -m * c2;
+      const unsigned long long msp = pack2f(ms, ms);
+#pragma unroll
+      for (int cc = 0; cc < 2; ++cc) {
+        uint32_t sc[32];
+        tmem_ld32(s_addr + 32 * cc, sc);
+        tmem_wait_ld();
+        if (diag) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i)
+            if (y0 + 32 * cc + i > x) sc[i] = 0xff800000u;
+        }
+        uint32_t pk[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const unsigned long long e2 = ffma2(pack2f(__uint_as_float(sc[2 * i]), __uint_as_float(sc[2 * i + 1])), c2p, msp);
+          float p0, p1;
+          if ((i & 7) < kEmuOf8) {
+            const unsigned long long pp = ex2_fma2(e2);
+            unpack2f(pp, p0, p1);
+            l2 = fadd2(l2, pp);
+          } else {
+            float e0, e1;
+            unpack2f(e2, e0, e1);
+            p0 = ex2(e0), p1 = ex2(e1);
+            l2 = fadd2(l2, pack2f(p0, p1));
+          }
+          pk[i] = pack_bf16(p0, p1);
+        }
+        tmem_st16(s_addr + 16 * cc, pk);
+      }
+      tmem_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&s.p_ready[w]);
+      if (q4 == 0 && lane == 0 && hs == 0) PFT(1 + w, 8 * j + 4);
     }
     if (n > 0) {
-      // ---- epilogue: O / l -> bf16 -> out ----
-      mbar_wait(&s.o_done[w], (uint32_t)(n - 1) & 1u);
-      tc_fence_after();
+      // ---- epilogue: O / l -> bf16 -> out (each thread its half of the row) ----
       float la, lb;
       unpack2f(l2, la, lb);
-      const float l = la + lb;
+      s.lxch[w][hs][row] = la + lb;
+      asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
+      const float l = la + lb + s.lxch[w][hs ^ 1][row];
+      mbar_wait(&s.o_done[w], (uint32_t)(n - 1) & 1u);
+      tc_fence_after();
       const float inv = 1.f / l;
       const bool valid = x <= xl[w];
       const size_t orow = ((size_t)lc * prm.n_tok + (size_t)(x - prm.pos_begin)) * c.n_q + hq[w];
 #pragma unroll
-      for (int cc = 0; cc < 4; ++cc) {
+      for (int cc = 0; cc < 2; ++cc) {
         uint32_t o[32];
         tmem_ld32(o_addr + 32 * cc, o);
         tmem_wait_ld();
         if (valid) {
-          uint4* dst = reinterpret_cast<uint4*>(prm.out + orow * kHeadDim + 32 * cc);
+          uint4* dst = reinterpret_cast<uint4*>(prm.out + orow * kHeadDim + 64 * hs + 32 * cc);
 #pragma unroll
           for (int v4 = 0; v4 < 4; ++v4) {
             uint4 val;
@@ -475,7 +474,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
           }
         }
       }
-      if (valid && prm.lse != nullptr) prm.lse[orow] = m * prm.sm_scale + __logf(l);
+      if (valid && hs == 0 && prm.lse != nullptr) prm.lse[orow] = m * prm.sm_scale + __logf(l);
     }
   }
   // ---- teardown: the single-lane roles diverged - reconverge before the aligned CTA barrier ----------
