@@ -219,8 +219,8 @@ cudaError_t launch_prefill_attn(const CacheView& c, int seq, int pos_begin, int 
                                 float* lse, int layer_begin, int layer_end, float sm_scale, cudaStream_t st,
                                 LaunchInfo* info);
 cudaError_t launch_prefill_attn_umma(const CacheView& c, int seq, int pos_begin, int n_tok, const void* q, void* out,
-                                     float* lse, int layer_begin, int layer_end, float sm_scale, cudaStream_t st,
-                                     LaunchInfo* info);
+                                     float* lse, int layer_begin, int layer_end, float sm_scale, int sm_count,
+                                     cudaStream_t st, LaunchInfo* info);
 // member_mask (optional): uint8 [layers][n_seqs][n_kv][stride], set to 1 at the positions that belong to the mass
 // set of ANY query head of the group; out may then be null.
 cudaError_t launch_attn_profile(const CacheView& c, const SeqList& list, int seq_base, int n_seqs_total, const void* q,

@@ -661,7 +661,7 @@ murmur_status_t murmur_prefill_attn(murmur_cache_t* c, int32_t seq, int32_t pos_
   } else {  // tcgen05 + tensor memory (the tensor maps need 16-byte aligned bases)
     if (((uintptr_t)q | (uintptr_t)out) & 15) return MURMUR_ERR_INVALID_ARG;
     MM_CUDA(c, launch_prefill_attn_umma(c->view, seq, pos_begin, pos_end - pos_begin, q, out, lse, layer_begin,
-                                        layer_end, sm_scale, (cudaStream_t)stream, &li));
+                                        layer_end, sm_scale, c->sm_count, (cudaStream_t)stream, &li));
   }
   note(c, li);
   return MURMUR_OK;
