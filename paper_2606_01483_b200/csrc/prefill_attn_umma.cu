@@ -52,20 +52,21 @@ constexpr int kBM = 128;                      // query rows per row block (TMEM 
 constexpr int kBN = 128;                      // keys per K/V tile
 constexpr int kHalfBytes = kBN * 128;         // one d-half of a 128-row tile: [128][64 bf16] = 16 KB
 constexpr int kUStages = 2;
-constexpr int kUThreads = 640;                // 5 warpgroups: {producer, issuer, 2 idle}, 4 x softmax
+constexpr int kUThreads = 768;                // 6 warpgroups: {producer, issuer, 2 idle}, 4 x softmax, epilogue
 constexpr int kSoftmaxWarps = 16;
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleLog2 = 8.f;           // raise the reference maximum only past 2^8
-constexpr int kRegsSoftmax = 104, kRegsOther = 56;  // 512 x 104 + 128 x 56 = 60416 <= 640 x 96 (what the launch allocates)
+constexpr int kRegsSoftmax = 88, kRegsOther = 48, kRegsEpilogue = 72;  // 512 x 88 + 128 x 48 + 128 x 72 = 60416 <= 768 x 80 (what the launch allocates)
 
 struct __align__(1024) USmem {
   uint8_t q[2][2][kHalfBytes];                // [row block][d-half]
   uint8_t k[kUStages][2][kHalfBytes];         // [stage][d-half]
   uint8_t v[kUStages][2][kHalfBytes];
   uint8_t ostage[4][32 * 128];                // per lane quarter: [32 rows][64 bf16] of one d-half on its way out (TMA store)
-  float mxch[2][2][4][kBM], lxch[2][4][kBM];  // row maxima [row block][tile parity] / row sums of the four warps of a row
+  float mxch[2][4][kBM];                      // row maxima of the four warps of a row, [exchange parity]
+  float lfin[2][2][4][kBM], mfin[2][2][kBM];  // an item's row sums (four partials) and reference maxima on their way to the epilogue, [item parity][row block]
   unsigned long long q_full, q_empty, k_full[kUStages], v_full[kUStages], k_empty[kUStages], v_empty[kUStages];
-  unsigned long long s_ready[2], p_ready[2], o_done[2], o_free[2], v_clean;
+  unsigned long long s_ready[2], p_ready[2], o_done[2], o_free[2], l_ready[2], v_clean, xch[4];
   uint32_t tmem_base;
 };
 
@@ -202,9 +203,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       mbar_init(&s.s_ready[w], 1);
       mbar_init(&s.p_ready[w], kSoftmaxWarps);  // one arrival per softmax warp
       mbar_init(&s.o_done[w], 1);
-      mbar_init(&s.o_free[w], kSoftmaxWarps);
+      mbar_init(&s.o_free[w], 4);               // the four epilogue warps
+      mbar_init(&s.l_ready[w], kSoftmaxWarps);
     }
     mbar_init(&s.v_clean, 1);
+    for (int i = 0; i < 4; ++i) mbar_init(&s.xch[i], 4);  // the four warps of a lane quarter
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k);
@@ -391,7 +394,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         PFT(0, 8 * n_it + 2);
       }
     }
-  } else {
+  } else if (warp < 4 + kSoftmaxWarps) {
     // ============================== softmax warps ==============================
     set_regs_inc<kRegsSoftmax>();
     const int sw = warp - 4;
@@ -399,11 +402,12 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const int q4 = warp & 3;               // TMEM lane quarter this warp may access
     const int row = q4 * 32 + lane;
     const uint32_t lane_base = tb + ((uint32_t)(q4 * 32) << 16);
-    const int quad_bar = 1 + q4;           // named barrier of the four warps that share these rows
     const float c2 = prm.sm_scale * 1.4426950408889634f;
     const unsigned long long c2p = pack2f(c2, c2);
     uint32_t n_s[2] = {0u, 0u};            // score tiles consumed per row block (barrier parities)
     [[maybe_unused]] uint32_t n_done = 0;
+    uint32_t n_x = 0;                      // maximum exchanges of this lane quarter so far (parity of xch)
+    uint32_t n_fin[2] = {0u, 0u};          // items handed to the epilogue per row block (parity of lfin / mfin)
     for (int id = first; id < n_items; id += stride) {
       const Item it = make_item(id, c, prm, len);
       float m_[2] = {-INFINITY, -INFINITY};
@@ -436,15 +440,52 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
           mx0 = fmaxf(mx0, __uint_as_float(sc[i]));
           mx1 = fmaxf(mx1, __uint_as_float(sc[16 + i]));
         }
-        // row maximum = max over the four column quarters
+        // row maximum = max over the four column quarters, exchanged through shared memory.  The exchange is
+        // asynchronous (an mbarrier, one arrival per warp of the quarter): the exponentials are computed at once
+        // against the row's CURRENT reference m and kept in registers; by the time they are done the other
+        // quarters' maxima are there, and only if the row's maximum tops m by more than 2^8 (rare) are O and l
+        // rescaled and the exponentials redone.  The first tile of an item has no reference yet and waits.
         PFD(n_done == kTraceItem && warp == 4, 1 + w, 8 * j + 2);
-        float(*mxq)[kBM] = s.mxch[w][j & 1];
+        float(*mxq)[kBM] = s.mxch[n_x & 1];
         mxq[cq][row] = fmaxf(mx0, mx1);
-        asm volatile("bar.sync %0, 128;" ::"r"(quad_bar) : "memory");
-        const float m_new = fmaxf(fmaxf(m, fmaxf(mxq[0][row], mxq[1][row])), fmaxf(mxq[2][row], mxq[3][row]));
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&s.xch[q4]);
+        const uint32_t xph = n_x & 1u;
+        ++n_x;
+        auto row_max = [&]() {
+          mbar_wait(&s.xch[q4], xph);
+          return fmaxf(fmaxf(mxq[0][row], mxq[1][row]), fmaxf(mxq[2][row], mxq[3][row]));
+        };
+        uint32_t pk[16];
+        auto exponentials = [&](float mref, unsigned long long lin) {
+          // P = exp2(c2 s - c2 m) as bf16 pairs; returns l + their sum
+          const float ms = -mref * c2;
+          const unsigned long long msp = pack2f(ms, ms);
+#pragma unroll
+          for (int i = 0; i < 16; ++i) {
+            const unsigned long long e2 = ffma2(pack2f(__uint_as_float(sc[2 * i]), __uint_as_float(sc[2 * i + 1])), c2p, msp);
+            float p0, p1;
+            if ((i & 7) < kEmuOf8) {
+              const unsigned long long pp = ex2_fma2(e2);
+              unpack2f(pp, p0, p1);
+              lin = fadd2(lin, pp);
+            } else {
+              float e0, e1;
+              unpack2f(e2, e0, e1);
+              p0 = ex2(e0), p1 = ex2(e1);
+              lin = fadd2(lin, pack2f(p0, p1));
+            }
+            pk[i] = pack_bf16(p0, p1);
+          }
+          return lin;
+        };
         if (j == 0) {
-          m = m_new;  // key 0 <= every query position: finite
+          m = row_max();  // key 0 <= every query position: finite
+          l2 = exponentials(m, l2);
         } else {
+          const unsigned long long l_try = exponentials(m, l2);
+          PFD(n_done == kTraceItem && warp == 4, 1 + w, 8 * j + 3);
+          const float m_new = fmaxf(m, row_max());
           const bool need = (m_new - m) * c2 > kRescaleLog2;   // same decision in all four warps of the row
           if (__any_sync(0xffffffffu, need)) {
             // rescale (this thread's quarter of) O and l of the rows whose reference maximum moves; PV(w, j-1) has
@@ -458,32 +499,14 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             tmem_st32(o_addr, o);
             float la, lb;
             unpack2f(l2, la, lb);
-            l2 = pack2f(la * f, lb * f);
             if (need) m = m_new;
-          }
-        }
-        PFD(n_done == kTraceItem && warp == 4, 1 + w, 8 * j + 3);
-        // P = exp2(c2 s - c2 m) as bf16 pairs, written over the first 16 of this thread's OWN 32 score columns
-        // (keys 32 cq .. at columns 32 cq ..): no thread writes what another still reads
-        const float ms = -m * c2;
-        const unsigned long long msp = pack2f(ms, ms);
-        uint32_t pk[16];
-#pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          const unsigned long long e2 = ffma2(pack2f(__uint_as_float(sc[2 * i]), __uint_as_float(sc[2 * i + 1])), c2p, msp);
-          float p0, p1;
-          if ((i & 7) < kEmuOf8) {
-            const unsigned long long pp = ex2_fma2(e2);
-            unpack2f(pp, p0, p1);
-            l2 = fadd2(l2, pp);
+            l2 = exponentials(m, pack2f(la * f, lb * f));
           } else {
-            float e0, e1;
-            unpack2f(e2, e0, e1);
-            p0 = ex2(e0), p1 = ex2(e1);
-            l2 = fadd2(l2, pack2f(p0, p1));
+            l2 = l_try;
           }
-          pk[i] = pack_bf16(p0, p1);
         }
+        // P goes over the first 16 of this thread's OWN 32 score columns (keys 32 cq .. at columns 32 cq ..): no
+        // thread writes what another still reads
         PFD(n_done == kTraceItem && warp == 4, 1 + w, 8 * j + 4);
         tmem_st16(s_addr, pk);
         tmem_wait_st();
@@ -492,59 +515,18 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         if (lane == 0) mbar_arrive(&s.p_ready[w]);
         PFD(n_done == kTraceItem && warp == 4, 1 + w, 8 * j + 5);
       };
-      auto finish = [&](auto wc) {
-        // ---- epilogue of a row block: O / l -> bf16 -> out (each thread its quarter of the row) ----
+      auto hand_over = [&](auto wc) {
+        // the row block's partial row sums and reference maxima go to the epilogue warps; this warp moves on
         constexpr int w = decltype(wc)::value;
-        const int n = it.nkt[w];
-        if (n == 0) return;
-        const int x = it.x0[w] + row;
-        const uint32_t o_addr = lane_base + 256u + 128u * w + 32u * cq;
+        if (it.nkt[w] == 0) return;
+        const uint32_t par = n_fin[w] & 1u;
+        ++n_fin[w];
         float la, lb;
         unpack2f(l_[w], la, lb);
-        s.lxch[w][cq][row] = la + lb;
-        asm volatile("bar.sync %0, 128;" ::"r"(quad_bar) : "memory");
-        if (warp == 4) PFT(1, 8 * n_done + 3 + 2 * w);
-        const float l = (s.lxch[w][0][row] + s.lxch[w][1][row]) + (s.lxch[w][2][row] + s.lxch[w][3][row]);
-        mbar_wait(&s.o_done[w], (n_s[w] - 1u) & 1u);   // the item's last PV of this row block
-        tc_fence_after();
-        if (warp == 4) PFT(1, 8 * n_done + 4 + 2 * w);
-        uint32_t o[32];
-        tmem_ld32(o_addr, o);
-        tmem_wait_ld();
-        tc_fence_before();
+        s.lfin[par][w][cq][row] = la + lb;
+        if (cq == 0) s.mfin[par][w][row] = m_[w];
         __syncwarp();
-        if (lane == 0) mbar_arrive(&s.o_free[w]);      // O_w may be overwritten by the next item
-        const float inv = 1.f / l;
-        if (cq == 0 && x <= it.xl[w] && prm.lse != nullptr) {
-          const size_t orow = ((size_t)it.lc * prm.n_tok + (size_t)(x - prm.pos_begin)) * c.n_q + it.hq[w];
-          prm.lse[orow] = m_[w] * prm.sm_scale + __logf(l);
-        }
-        // out rows are 7 KB apart: 32 lanes storing 16 bytes each would touch 32 lines per instruction.  The four
-        // warps of a lane quarter stage [32 rows][64 bf16] of one d-half (128-byte swizzle) and one TMA store writes
-        // it as 32 full 128-byte row segments; rows past the end of the call's range are clipped by the tensor map.
-        uint8_t* stage = s.ostage[q4];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          if ((cq >> 1) == h) {
-#pragma unroll
-            for (int v4 = 0; v4 < 4; ++v4) {
-              uint4 val;
-              val.x = pack_bf16(__uint_as_float(o[8 * v4 + 0]) * inv, __uint_as_float(o[8 * v4 + 1]) * inv);
-              val.y = pack_bf16(__uint_as_float(o[8 * v4 + 2]) * inv, __uint_as_float(o[8 * v4 + 3]) * inv);
-              val.z = pack_bf16(__uint_as_float(o[8 * v4 + 4]) * inv, __uint_as_float(o[8 * v4 + 5]) * inv);
-              val.w = pack_bf16(__uint_as_float(o[8 * v4 + 6]) * inv, __uint_as_float(o[8 * v4 + 7]) * inv);
-              *reinterpret_cast<uint4*>(stage + lane * 128 + ((((cq & 1) * 4 + v4) ^ (lane & 7)) << 4)) = val;
-            }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          }
-          asm volatile("bar.sync %0, 128;" ::"r"(quad_bar) : "memory");
-          if (cq == 0 && lane == 0) {
-            tma_store_4d(&tm_o, stage, 64 * h, it.hq[w], it.x0[w] - prm.pos_begin + 32 * q4, it.lc);
-            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging slice has been read
-          }
-          asm volatile("bar.sync %0, 128;" ::"r"(quad_bar) : "memory");
-        }
+        if (lane == 0) mbar_arrive(&s.l_ready[w]);
       };
       constexpr std::integral_constant<int, 0> W0{};
       constexpr std::integral_constant<int, 1> W1{};
@@ -554,10 +536,75 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         if (j < it.nkt[1]) tile(W1, j);
       }
       if (warp == 4) PFT(1, 8 * n_done + 1);
-      finish(W0);
-      finish(W1);
+      hand_over(W0);
+      hand_over(W1);
       if (warp == 4) PFT(1, 8 * n_done + 2);
       ++n_done;
+    }
+  } else {
+    // ============================== epilogue warps ==============================
+    // One warp per tensor-memory lane quarter: O_w / l -> bf16 -> out for the quarter's 32 rows, off the softmax
+    // warps' path (they are already on the next item's first tiles).  out rows are 7 KB apart - 32 lanes storing 16
+    // bytes each would touch 32 lines per instruction - so a warp stages [32 rows][64 bf16] of one d-half in shared
+    // memory (128-byte swizzle) and one TMA store writes it as 32 full 128-byte row segments; rows past the end of
+    // the call's range are clipped by the tensor map.
+    set_regs_dec<kRegsEpilogue>();
+    const int q4 = warp & 3;
+    const int row = q4 * 32 + lane;
+    const uint32_t lane_base = tb + ((uint32_t)(q4 * 32) << 16);
+    uint8_t* stage = s.ostage[q4];
+    uint32_t n_pv[2] = {0u, 0u}, n_fin[2] = {0u, 0u};
+    for (int id = first; id < n_items; id += stride) {
+      const Item it = make_item(id, c, prm, len);
+#pragma unroll
+      for (int w = 0; w < 2; ++w) {
+        if (it.nkt[w] == 0) continue;
+        n_pv[w] += (uint32_t)it.nkt[w];
+        const uint32_t par = n_fin[w] & 1u;
+        ++n_fin[w];
+        mbar_wait(&s.l_ready[w], par);
+        const float l = (s.lfin[par][w][0][row] + s.lfin[par][w][1][row]) + (s.lfin[par][w][2][row] + s.lfin[par][w][3][row]);
+        const float m = s.mfin[par][w][row];
+        mbar_wait(&s.o_done[w], (n_pv[w] - 1u) & 1u);   // the item's last PV of this row block
+        tc_fence_after();
+        const float inv = 1.f / l;
+        const int x = it.x0[w] + row;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+          for (int cc = 0; cc < 2; ++cc) {
+            uint32_t o[32];
+            tmem_ld32(lane_base + 256u + 128u * w + 64u * h + 32u * cc, o);
+            tmem_wait_ld();
+            if (h == 1 && cc == 1) {  // O_w is in registers / on its way out: the next item may overwrite it
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive(&s.o_free[w]);
+            }
+#pragma unroll
+            for (int v4 = 0; v4 < 4; ++v4) {
+              uint4 val;
+              val.x = pack_bf16(__uint_as_float(o[8 * v4 + 0]) * inv, __uint_as_float(o[8 * v4 + 1]) * inv);
+              val.y = pack_bf16(__uint_as_float(o[8 * v4 + 2]) * inv, __uint_as_float(o[8 * v4 + 3]) * inv);
+              val.z = pack_bf16(__uint_as_float(o[8 * v4 + 4]) * inv, __uint_as_float(o[8 * v4 + 5]) * inv);
+              val.w = pack_bf16(__uint_as_float(o[8 * v4 + 6]) * inv, __uint_as_float(o[8 * v4 + 7]) * inv);
+              *reinterpret_cast<uint4*>(stage + lane * 128 + (((cc * 4 + v4) ^ (lane & 7)) << 4)) = val;
+            }
+          }
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          __syncwarp();
+          if (lane == 0) {
+            tma_store_4d(&tm_o, stage, 64 * h, it.hq[w], it.x0[w] - prm.pos_begin + 32 * q4, it.lc);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging slice has been read
+          }
+          __syncwarp();
+        }
+        if (x <= it.xl[w] && prm.lse != nullptr) {
+          const size_t orow = ((size_t)it.lc * prm.n_tok + (size_t)(x - prm.pos_begin)) * c.n_q + it.hq[w];
+          prm.lse[orow] = m * prm.sm_scale + __logf(l);
+        }
+      }
     }
   }
   // ---- teardown: the single-lane roles diverged - reconverge before the aligned CTA barrier ----------
