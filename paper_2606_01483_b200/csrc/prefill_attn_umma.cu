@@ -155,7 +155,7 @@ __device__ __forceinline__ unsigned long long ex2_fma2(unsigned long long x2) {
                 __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23)));
 }
 #ifndef MURMUR_PF_EMU_OF_8
-#define MURMUR_PF_EMU_OF_8 3
+#define MURMUR_PF_EMU_OF_8 1
 #endif
 constexpr int kEmuOf8 = MURMUR_PF_EMU_OF_8;   // of every 8 pairs, this many take the FMA route
 
