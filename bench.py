@@ -973,12 +973,13 @@ def run_index_set_eviction(dev, torch) -> dict:
            "select_us_per_sequence": e0.elapsed_time(e1) * 1e3 / cfg.batch,
            "evict_indexed_wall_us_per_sequence": t_def * 1e6 / cfg.batch,
            "decode_attn_indexed_us": e2.elapsed_time(e3) * 1e3 / 10,
+           "decode_attn_indexed_gbs": rows * 512 / (e2.elapsed_time(e3) * 1e-3 / 10) / 1e9,
            "pages_freed": int(wb.cache.stats()["free_pages"]) - 2,
            "parity_sequence_0": {"slab_tables_and_rows_bit_exact": bool(rows_ok), "max_abs": mx, "mean_abs": mean,
                                  "ok": bool(rows_ok and mx <= 2e-2 and mean <= 2e-3)},
            "device_error_word": wb.cache.last_error(),
-           "note": "first path: FFMA attention over the slabs; the point of the line is the cache-management cost "
-                   "(PAPER.md:154, 214) next to what it buys"}
+           "note": "attention over the slabs: streaming tensor-core kernel, one CTA per (layer, sequence, KV head) slab; "
+                   "the point of the line is the cache-management cost (PAPER.md:154, 214) next to what it buys"}
     wb.close()
     del wb
     torch.cuda.empty_cache()
@@ -1048,9 +1049,12 @@ def run_prefill(args):
     tfs = flops / (ms * 1e-3) / 1e12
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            peak, peak_src = float(json.load(f)["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst: the kernel is timed alone)"
+            pk = json.load(f)
+        peak, peak_src = float(pk["bf16_tflops"]), ("measured (MEASURED_PEAKS.json bf16_tflops, the BURST figure - the conservative "
+                                                     "denominator: K launches back to back run into the power cap like the sustained one)")
+        peak_sus = float(pk["bf16_tflops_sustained"]) if "bf16_tflops_sustained" in pk else None
     except Exception:
-        peak, peak_src = 1590.0, "fallback (B200_PROFILING.md 1.59 PFLOP/s)"
+        peak, peak_src, peak_sus = 1590.0, "fallback (B200_PROFILING.md 1.59 PFLOP/s)", None
     # oracle: sampled rows (first, tile / page boundaries, last) of 3 layers, all heads, fp64
     from oracle import attention as o_attn
 
@@ -1083,7 +1087,8 @@ def run_prefill(args):
         "tflops": tfs, "tokens_per_s": n / (ms * 1e-3),
         "roofline": {"bound": "tensor", "kernel": "prefill_umma_kernel (tcgen05.mma, accumulators in TMEM, TMA-fed)",
                      "achieved": tfs, "peak": peak, "unit": "TFLOP/s", "frac": tfs / peak, "traffic": None,
-                     "peak_source": peak_src, "algorithmic_flops_per_launch": flops,
+                     "peak_source": peak_src, "peak_sustained": peak_sus,
+                     "frac_of_sustained_peak": (tfs / peak_sus) if peak_sus else None, "algorithmic_flops_per_launch": flops,
                      "how": "causal flops 4 d sum_x (x + 1) per head and layer / mean launch duration (CUDA events, %d launches)" % K},
         "mma_sync_kernel_ms": ms_old, "speedup_vs_mma_sync": ms_old / ms,
         "max_abs_diff_vs_mma_sync": float((out.float() - out_old.float()).abs().max()),

@@ -26,7 +26,8 @@ LIB = os.path.join(_HERE, "libmurmur.so")
 OBJ_DIR = os.path.join(_HERE, "_obj")
 
 SOURCES = ["murmur_api.cu", "kv_append.cu", "kv_evict.cu", "decode_attn_generic.cu", "decode_attn_mma.cu",
-           "attn_profile.cu", "prefill_attn.cu", "prefill_attn_umma.cu", "chunk_plan.cu", "kv_indexed.cu"]
+           "attn_profile.cu", "prefill_attn.cu", "prefill_attn_umma.cu", "chunk_plan.cu", "kv_indexed.cu",
+           "decode_attn_indexed.cu"]
 HEADERS = ["device_state.cuh", "policy_math.cuh", "evict_body.cuh", "ptx_utils.cuh", "umma_utils.cuh"]
 
 NVCC_FLAGS = [

@@ -234,6 +234,8 @@ cudaError_t launch_indexed_append(const CacheView& c, const IdxView& ix, const S
                                   const void* v_new, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_indexed_attn(const CacheView& c, const IdxView& ix, const SeqList& list, const void* q, void* out,
                                 float* lse, float sm_scale, cudaStream_t st, LaunchInfo* info);
+cudaError_t launch_indexed_attn_mma(const CacheView& c, const IdxView& ix, const SeqList& list, const void* q, void* out,
+                                float* lse, float sm_scale, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_indexed_gather(const CacheView& c, const IdxView& ix, int seq, void* k_out, void* v_out, int cap_out,
                                   cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_indexed_seq_end(const CacheView& c, int seq, cudaStream_t st, LaunchInfo* info);

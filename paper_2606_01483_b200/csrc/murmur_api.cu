@@ -848,7 +848,15 @@ murmur_status_t murmur_decode_attn_indexed(murmur_cache_t* c, const int32_t* seq
   list.n = n_seqs;
   for (int i = 0; i < n_seqs; ++i) list.ids[i] = seq_ids[i];
   LaunchInfo li{};
-  MM_CUDA(c, launch_indexed_attn(c->view, c->idx, list, q, out, lse, sm_scale, (cudaStream_t)stream, &li));
+  // tensor cores whenever a page holds whole 16-row MMA slices (same rule and option as the positional call)
+  int variant = c->attn_variant_opt;
+  if (variant == MURMUR_ATTN_AUTO) variant = (c->desc.page_size >= 16) ? MURMUR_ATTN_MMA : MURMUR_ATTN_GENERIC;
+  if (variant == MURMUR_ATTN_MMA && c->desc.page_size < 16) return MURMUR_ERR_UNSUPPORTED;
+  if (variant == MURMUR_ATTN_MMA) {
+    MM_CUDA(c, launch_indexed_attn_mma(c->view, c->idx, list, q, out, lse, sm_scale, (cudaStream_t)stream, &li));
+  } else {
+    MM_CUDA(c, launch_indexed_attn(c->view, c->idx, list, q, out, lse, sm_scale, (cudaStream_t)stream, &li));
+  }
   note(c, li);
   c->stats.attn_calls += 1;
   return MURMUR_OK;

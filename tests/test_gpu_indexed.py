@@ -59,17 +59,25 @@ def _check_indexed(sbs, oix, i, q=None):
     assert sbs.gpu.stats()["free_pages"] == len(sbs.oracle.free_stack)
     assert sbs.gpu.last_error() == 0
     if q is not None:
-        lse = torch.empty(L, 1, sbs.cfg.geom.n_q_heads, dtype=torch.float32, device=sbs.device)
-        out = sbs.gpu.decode_attn_indexed([i], q, lse=lse, sm_scale=sbs.scale)
-        got = out.float().cpu().numpy().astype(np.float64)
+        from paper_2606_01483_b200 import MURMUR_ATTN_AUTO, MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA
+        from paper_2606_01483_b200.binding import MURMUR_OPT_ATTN_VARIANT
+
         qb = workloads.to_bits(q)
-        errs = []
-        for l in range(L):
-            o_ref, lse_ref = o_ix.attend_indexed(qb[l, 0], kb[l], vb[l], [oix.positions(i, l, h) for h in range(H)], sbs.scale)
-            errs.append(np.abs(got[l, 0] - o_ref))
-            assert np.max(np.abs(lse[l, 0].cpu().numpy() - lse_ref)) < 2e-3
-        e = np.stack(errs)
-        assert e.max() <= 2e-2 and e.mean() <= 2e-3, (e.max(), e.mean())
+        refs = [o_ix.attend_indexed(qb[l, 0], kb[l], vb[l], [oix.positions(i, l, h) for h in range(H)], sbs.scale) for l in range(L)]
+        # both kernels: tensor cores (streaming mma.sync kernel, pages of >= 16 rows) and the FFMA path
+        for variant in (MURMUR_ATTN_MMA, MURMUR_ATTN_GENERIC):
+            sbs.gpu.set_option(MURMUR_OPT_ATTN_VARIANT, variant)
+            lse = torch.empty(L, 1, sbs.cfg.geom.n_q_heads, dtype=torch.float32, device=sbs.device)
+            out = sbs.gpu.decode_attn_indexed([i], q, lse=lse, sm_scale=sbs.scale)
+            got = out.float().cpu().numpy().astype(np.float64)
+            errs = []
+            for l in range(L):
+                o_ref, lse_ref = refs[l]
+                errs.append(np.abs(got[l, 0] - o_ref))
+                assert np.max(np.abs(lse[l, 0].cpu().numpy() - lse_ref)) < 2e-3, variant
+            e = np.stack(errs)
+            assert np.isfinite(got).all() and e.max() <= 2e-2 and e.mean() <= 2e-3, (variant, e.max(), e.mean())
+        sbs.gpu.set_option(MURMUR_OPT_ATTN_VARIANT, MURMUR_ATTN_AUTO)
 
 
 @pytest.mark.parametrize("seed,page", [(0, 16), (1, 16), (2, 64), (3, 32)])
