@@ -8,7 +8,9 @@ only the stale ones) and linked into one shared library.
     python -m paper_2606_01483_b200.build [-v] [--trace]
 
 ``--trace`` (or MURMUR_TRACE=1 in the environment) compiles the per-CTA ``globaltimer`` stamps and
-the two ``murmur_debug_*`` exports in (profiling builds only; see include/murmur.h).
+the two ``murmur_debug_*`` exports in (profiling builds only; see include/murmur.h).  ``--pftrace`` compiles
+the prefill kernel's clock stamps in (``-DMURMUR_PFTRACE``: per-item and per-tile stamps of CTA 0's issuer and
+of one softmax warp, read back with ``murmur_debug_pftrace`` / ``murmur_debug_pftile``; profiles/r02_prefill_ncu.md).
 """
 from __future__ import annotations
 
@@ -112,6 +114,7 @@ def build(force: bool = False, verbose: bool = False, extra: Sequence[str] = (),
 
 
 if __name__ == "__main__":
-    build(force="-f" in sys.argv, verbose=True, extra=["-Xptxas", "-v"] if "-v" in sys.argv else [],
+    build(force="-f" in sys.argv, verbose=True,
+          extra=(["-Xptxas", "-v"] if "-v" in sys.argv else []) + (["-DMURMUR_PFTRACE=1"] if "--pftrace" in sys.argv else []),
           trace="--trace" in sys.argv)
     print(LIB)
