@@ -136,6 +136,39 @@ def test_random_index_sets_compaction_append_and_attention(dev, seed, page):
     sbs.close()
 
 
+@pytest.mark.parametrize("page", [16, 64])
+def test_long_ragged_slabs_attention(dev, page):
+    """Slabs of very different lengths (1 row ... ~700 rows = 11 tiles of 64: the 4-stage ring of the streaming
+    tensor-core kernel wraps several times, groups get odd and even tile counts, the last tile is partial), windows
+    off so that everything is resident; then a few head-ragged appends across a tile boundary."""
+    from workloads import WINDOW_OFF
+
+    rng = random.Random(77 + page)
+    L, H = 2, 4
+    specs = [seq_spec(8, 650, 40, WINDOW_OFF, WINDOW_OFF)]
+    cfg = Config(f"idxlong{page}", 140, Geometry(n_layers=L), page, tuple(specs))
+    sbs = _mk(cfg, dev, extra_tokens=64)
+    sbs.gpu.indexed_enable()
+    oix = o_ix.OracleIndexedCache(sbs.oracle, L, H)
+    sbs.bulk_prefill([0], 30)
+    st = sbs.oracle.seqs[0]
+    resident = sorted(x for x in o_policy.resident_positions(st.P, st.S, st.M, st.t, st.pol) if x < st.length)
+    sizes = [len(resident), 1, 63, 64, 65, 191, 256, 449]
+    sel = [[sorted(rng.sample(resident, sizes[(l * H + h) % len(sizes)])) for h in range(H)] for l in range(L)]
+    pos_d, cnt_d = _sets_to_device(sel, L, H, dev)
+    moved = sbs.gpu.kv_evict_indexed(0, pos_d, cnt_d)
+    assert moved == 512 * oix.evict_indexed(0, sel)
+    _check_indexed(sbs, oix, 0, sbs.data[0].q_step(31).unsqueeze(1).contiguous())
+    for k in range(3):  # 63 -> 66, 64 -> 67, 191 -> 194, 256 -> 259 rows: across tile and page boundaries
+        u = 30 + k
+        kn, vn = sbs.data[0].out_kv(u, u + 1)
+        sbs._store(0, kn, vn)
+        sbs.gpu.kv_append_indexed([0], kn.contiguous(), vn.contiguous())
+        oix.append_indexed([0])
+        _check_indexed(sbs, oix, 0, sbs.data[0].q_step(u + 1).unsqueeze(1).contiguous())
+    sbs.close()
+
+
 def test_mass_sets_are_valid_and_drive_an_eviction(dev):
     """murmur_select_mass_sets: every query head keeps >= frac of its Eq. 1 mass inside its KV head's set (checked with the
     oracle's fp64 weights), prompts and the newest positions are in, the set sizes are those of the oracle up to the
