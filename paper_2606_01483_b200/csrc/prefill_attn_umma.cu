@@ -16,7 +16,7 @@
 // already streams the next item's Q and K/V and the issuer its first score tiles.  (One CTA per item cost ~10 us of
 // launch, set-up, pipeline fill and drain per item - as much as the item's tensor-core time.)
 //
-// Per CTA, 20 warps in five warpgroups (register budgets re-balanced with setmaxnreg):
+// Per CTA, 24 warps in six warpgroups (register budgets re-balanced with setmaxnreg):
 //   warp 0      TMA producer: Q blocks (tensor map over q, 128-byte swizzle written by the copy engine) and
 //               the K/V tiles, one box per (page, d-half) straight from the paged pools.  The pools' rows are
 //               stored pre-swizzled (16-byte chunk c of slot s at c ^ (s & 7), device_state.cuh); a
@@ -36,6 +36,8 @@
 //               of it on the FMA pipes), P written back as bf16 over the first 16 of the thread's OWN 32 score
 //               columns (tcgen05.st).  The reference maximum is raised only when it grows by more than 2^8 (O is
 //               then rescaled in tensor memory): rare, and exact in the end - l and O share one reference.
+//   warps 20-23 epilogue, one per lane quarter: O_w / l -> bf16 -> 4 KB staging slice -> TMA store, while the
+//               softmax warps are already on the next item's first tiles.
 // Tensor memory (512 columns): S_0, S_1 (128 fp32 columns each, P_w inside S_w), O_0, O_1.
 #include <cuda_bf16.h>
 
