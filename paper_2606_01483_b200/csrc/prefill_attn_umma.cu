@@ -67,7 +67,7 @@ struct __align__(1024) USmem {
   uint8_t ostage[4][32 * 128];                // per lane quarter: [32 rows][64 bf16] of one d-half on its way out (TMA store)
   float mxch[2][4][kBM];                      // row maxima of the four warps of a row, [exchange parity]
   float lfin[2][2][4][kBM], mfin[2][2][kBM];  // an item's row sums (four partials) and reference maxima on their way to the epilogue, [item parity][row block]
-  unsigned long long q_full, q_empty, k_full[kUStages], v_full[kUStages], k_empty[kUStages], v_empty[kUStages];
+  unsigned long long q_full[2], q_empty[2], k_full[kUStages], v_full[kUStages], k_empty[kUStages], v_empty[kUStages];
   unsigned long long s_ready[2], p_ready[2], o_done[2], o_free[2], l_ready[2], v_clean, xch[4];
   uint32_t tmem_base;
 };
@@ -193,8 +193,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
 
   // ---- set-up: barriers, tensor memory, finite K/V stages ------------------------------------------
   if (tid == 0) {
-    mbar_init(&s.q_full, 1);
-    mbar_init(&s.q_empty, 1);
+    for (int w = 0; w < 2; ++w) {
+      mbar_init(&s.q_full[w], 1);
+      mbar_init(&s.q_empty[w], 1);
+    }
     for (int i = 0; i < kUStages; ++i) {
       mbar_init(&s.k_full[i], 1);
       mbar_init(&s.v_full[i], 1);
@@ -242,7 +244,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       const int32_t* tab = c.block_table + (size_t)prm.seq * c.max_blocks;
       const int ppt = kBN >> plog;  // pages per tile
       int t = 0;                    // K/V tiles staged so far (ring position, across items)
-      uint32_t n_it = 0;
+      uint32_t n_it = 0, n_qw[2] = {0u, 0u};   // items; items with row block w active (parity of q_empty[w])
       for (int id = first; id < n_items; id += stride, ++n_it) {
         const Item it = make_item(id, c, prm, len);
         const int layer = prm.layer_begin + it.lc;
@@ -267,15 +269,20 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
             }
             ++t;
           };
-          // the item's first K/V tile goes into the ring while the previous item is still using Q
+          // Q_w has its own hand-over: the previous item's last score tile of row block w frees it - for row block 0
+          // that is two MMA groups before the item ends, so Q_0 and the first K/V tile (the ring slot frees at about
+          // the same time) are there for the successor's first score tile to be issued under the tail
+          auto load_q = [&](int w) {
+            if (!it.act[w]) return;
+            mbar_wait(&s.q_empty[w], (n_qw[w] & 1u) ^ 1u);
+            ++n_qw[w];
+            mbar_expect_tx(&s.q_full[w], (uint32_t)(2 * kHalfBytes));
+            for (int h = 0; h < 2; ++h)
+              tma_load_4d(&s.q[w][h][0], &tm_q, 64 * h, it.hq[w], it.x0[w] - prm.pos_begin, it.lc, &s.q_full[w]);
+          };
+          load_q(0);
           stage_tile(0);
-          mbar_wait(&s.q_empty, (n_it & 1u) ^ 1u);  // the previous item's score MMAs are done with Q
-          mbar_expect_tx(&s.q_full, (uint32_t)((it.act[0] + it.act[1]) * 2 * kHalfBytes));
-#pragma unroll
-          for (int w = 0; w < 2; ++w)
-            if (it.act[w])
-              for (int h = 0; h < 2; ++h)
-                tma_load_4d(&s.q[w][h][0], &tm_q, 64 * h, it.hq[w], it.x0[w] - prm.pos_begin, it.lc, &s.q_full);
+          load_q(1);
           if (id + stride < n_items) {  // the NEXT item's Q on its way into L2 (it comes from HBM: q is read once)
             const Item nx = make_item(id + stride, c, prm, len);
 #pragma unroll
@@ -314,6 +321,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       int k_seen = -1, v_seen = -1;      // ring positions whose full barrier this warp has already observed
       uint32_t n_pv[2] = {0u, 0u};       // PV groups issued per row block (parity of p_ready)
       uint32_t n_it = 0, n_itw[2] = {0u, 0u}, n_clean = 0;
+      uint32_t n_qw[2] = {0u, 0u};       // items with row block w active whose Q this warp has taken (parity of q_full[w])
+      bool s00_early = false;            // this item's S(0,0) was already issued under the previous item's tail
       for (int id = first; id < n_items; id += stride, ++n_it) {
         const Item it = make_item(id, c, prm, len);
         auto need_k = [&](int j) {
@@ -371,23 +380,52 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         constexpr std::integral_constant<int, 0> W0{};
         constexpr std::integral_constant<int, 1> W1{};
         PFT(0, 8 * n_it + 0);
-        mbar_wait(&s.q_full, n_it & 1u);
-        PFT(0, 8 * n_it + 1);
         PFV(0, 8 * n_it + 3, it.n_kt);
         // Issue order (the two row blocks half a period apart, so that one block's softmax always runs
         // under the other's MMAs):  S(0,0);  then per tile j:  S(1,j)  PV(0,j)  S(0,j+1)  PV(1,j).
         // P_w lives inside S_w: S(w,j+1) is issued after PV(w,j), and tcgen05.mma executes in issue order.
-        if (it.nkt[0] > 0) issue_s(W0, 0);
+        // Row block 0 always exists (e = 2 pair < n_rb).
+        if (!s00_early) {
+          mbar_wait(&s.q_full[0], n_qw[0] & 1u);
+          issue_s(W0, 0);
+        }
+        s00_early = false;
+        ++n_qw[0];
+        if (it.nkt[0] == 1) {
+          if (leader) umma_commit(&s.q_empty[0]);  // that was row block 0's last score tile of the item: Q_0 may go
+          __syncwarp();
+        }
+        PFT(0, 8 * n_it + 1);
+        const bool has_next = id + stride < n_items;
         for (int j = 0; j < it.n_kt; ++j) {
           const int st = (t0 + j) % kUStages;
-          if (j < it.nkt[1]) issue_s(W1, j);
+          if (j < it.nkt[1]) {
+            if (j == 0) {
+              mbar_wait(&s.q_full[1], n_qw[1] & 1u);
+              ++n_qw[1];
+            }
+            issue_s(W1, j);
+          }
           if (leader) {
             umma_commit(&s.k_empty[st]);  // K_j: both S(0,j) and S(1,j) are behind this point
-            if (j == it.n_kt - 1) umma_commit(&s.q_empty);  // ... and so is every score tile of the item: Q may go
+            if (j == it.nkt[1] - 1) umma_commit(&s.q_empty[1]);
           }
           __syncwarp();
           if (j < it.nkt[0]) issue_pv(W0, j);
-          if (j + 1 < it.nkt[0]) issue_s(W0, j + 1);
+          if (j + 1 < it.nkt[0]) {
+            issue_s(W0, j + 1);
+            if (j + 1 == it.nkt[0] - 1) {
+              if (leader) umma_commit(&s.q_empty[0]);
+              __syncwarp();
+            }
+          } else if (j == it.n_kt - 1 && has_next) {
+            // the slot of S(0, j+1) in the item's last round: the NEXT item's S(0,0) - its pipeline fills under this item's tail
+            // (both waits end without this warp's help: the producer was handed Q_0 and the ring slot a round ago;
+            // PV(1, j) behind them has the softmax of (1, j) to wait for anyway)
+            mbar_wait(&s.q_full[0], n_qw[0] & 1u);
+            issue_s(W0, it.n_kt);   // ring tile t0 + n_kt = the next item's tile 0
+            s00_early = true;
+          }
           if (j < it.nkt[1]) issue_pv(W1, j);
           if (leader) umma_commit(&s.v_empty[st]);
           __syncwarp();
