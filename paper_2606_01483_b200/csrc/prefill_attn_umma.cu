@@ -68,7 +68,7 @@ struct __align__(1024) USmem {
   float mxch[2][4][kBM];                      // row maxima of the four warps of a row, [exchange parity]
   float lfin[2][2][4][kBM], mfin[2][2][kBM];  // an item's row sums (four partials) and reference maxima on their way to the epilogue, [item parity][row block]
   unsigned long long q_full[2], q_empty[2], k_full[kUStages], v_full[kUStages], k_empty[kUStages], v_empty[kUStages];
-  unsigned long long s_ready[2], p_ready[2], o_done[2], o_free[2], l_ready[2], v_clean, xch[4];
+  unsigned long long s_ready[2], p_ready[2], o_done[2], o_free[2], l_ready[2], l_free[2], v_clean[2], xch[4];
   uint32_t tmem_base;
 };
 
@@ -209,8 +209,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       mbar_init(&s.o_done[w], 1);
       mbar_init(&s.o_free[w], 4);               // the four epilogue warps
       mbar_init(&s.l_ready[w], kSoftmaxWarps);
+      mbar_init(&s.l_free[w], 4);               // the four epilogue warps
+      mbar_init(&s.v_clean[w], 1);
     }
-    mbar_init(&s.v_clean, 1);
     for (int i = 0; i < 4; ++i) mbar_init(&s.xch[i], 4);  // the four warps of a lane quarter
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     tma_prefetch_desc(&tm_q);
@@ -245,6 +246,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
       const int ppt = kBN >> plog;  // pages per tile
       int t = 0;                    // K/V tiles staged so far (ring position, across items)
       uint32_t n_it = 0, n_qw[2] = {0u, 0u};   // items; items with row block w active (parity of q_empty[w])
+      uint32_t n_clean = 0;                    // tiles cleaned so far
       for (int id = first; id < n_items; id += stride, ++n_it) {
         const Item it = make_item(id, c, prm, len);
         const int layer = prm.layer_begin + it.lc;
@@ -303,7 +305,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
           }
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           __syncwarp();
-          if (lane == 0) mbar_arrive(&s.v_clean);
+          // two barriers in turn: the producer is at most two tiles - two cleaned tiles - ahead of the issuer, so
+          // neither barrier ever runs two phases ahead of its waiter (a parity wait could not tell)
+          if (lane == 0) mbar_arrive(&s.v_clean[n_clean & 1u]);
+          ++n_clean;
         }
       }
     } else if (warp == 1) {
@@ -336,7 +341,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
           const int t = t0 + j;
           if (v_seen < t) {
             mbar_wait(&s.v_full[t % kUStages], (uint32_t)(t / kUStages) & 1u);
-            if (it.need_clean && j == it.n_kt - 1) mbar_wait(&s.v_clean, n_clean & 1u), ++n_clean;
+            if (it.need_clean && j == it.n_kt - 1) mbar_wait(&s.v_clean[n_clean & 1u], (n_clean >> 1) & 1u), ++n_clean;
             v_seen = t;
           }
         };
@@ -560,6 +565,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         constexpr int w = decltype(wc)::value;
         if (it.nkt[w] == 0) return;
         const uint32_t par = n_fin[w] & 1u;
+        // not before the epilogue has taken the previous item's: an item of a single tile needs no PV - no o_free - to
+        // get here, and l_ready must never run two phases ahead of its waiter (a parity wait could not tell)
+        mbar_wait(&s.l_free[w], par ^ 1u);
         ++n_fin[w];
         float la, lb;
         unpack2f(l_[w], la, lb);
@@ -605,6 +613,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         mbar_wait(&s.l_ready[w], par);
         const float l = (s.lfin[par][w][0][row] + s.lfin[par][w][1][row]) + (s.lfin[par][w][2][row] + s.lfin[par][w][3][row]);
         const float m = s.mfin[par][w][row];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&s.l_free[w]);
         mbar_wait(&s.o_done[w], (n_pv[w] - 1u) & 1u);   // the item's last PV of this row block
         tc_fence_after();
         const float inv = 1.f / l;

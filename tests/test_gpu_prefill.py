@@ -109,6 +109,25 @@ def test_prefill_moving_row_maximum(dev, page):
     c.close()
 
 
+def test_prefill_many_single_tile_items_per_cta(dev):
+    """100 positions x 28 layers: 448 work items of ONE 128-key tile each, three per persistent CTA back to back, every
+    one with rows past the sequence length in its last (only) tile - the hand-overs between softmax, epilogue, producer
+    and issuer that a multi-tile item spaces out all fall on top of each other.  Repeated, bit-identical every time."""
+    L, n_tok = 28, 100
+    c = _cache(dev, L, n_tok, 16)
+    k, v = _rand((L, n_tok, 4, 128), 31, dev), _rand((L, n_tok, 4, 128), 32, dev)
+    q = _rand((L, n_tok, 28, 128), 33, dev)
+    c.kv_append([0], [n_tok], k, v)
+    lse = torch.empty(L, n_tok, 28, dtype=torch.float32, device=dev)
+    out = c.prefill_attn(0, 0, n_tok, q, lse=lse)
+    _check(out, lse, q, k, v, 0, [0, 1, 31, 64, 98, 99], 1 / math.sqrt(128))
+    for _ in range(50):
+        again = c.prefill_attn(0, 0, n_tok, q)
+        assert torch.equal(again, out)
+    assert c.last_error() == 0
+    c.close()
+
+
 def test_prefill_config2_size_sampled_rows(dev):
     # one 300 s chunk: 64 prefix + 2250 speech tokens, 2 layers; rows around tile / page boundaries and the end
     cfg = workloads.config2().with_layers(2)
