@@ -297,10 +297,13 @@ def run_reference(args):
     n_sample = int(max(1, min(g.n_layers, budget_s / max(1, K + W) / per_item)))
     for _ in range(max(0, W - 1)):
         step(n_sample)
+    n_ret0 = sum(len(oc.retained(i)) for i in ids)  # outside the timed region: the same |A(t)| the CUDA arm reads off the device
     t_start = time.perf_counter()
     for _ in range(K):
         used = step(n_sample)
     el = time.perf_counter() - t_start
+    n_ret = (n_ret0 + sum(len(oc.retained(i)) for i in ids)) // 2
+    kv_bytes = n_ret * BYTES_PER_TOKEN_LAYER * g.n_layers
     us_step = el / K * (n_items_step / n_sample) * 1e6
     sample = (f"per step: Python integer bookkeeping (oracle.paged_cache append + evict) of all {cfg.batch} sequences "
               f"+ fp64 attention of sequence 0, layers 0..{n_sample - 1} (all 28 q heads); the whole time is scaled "
@@ -310,7 +313,10 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": us_step, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
         "warmup": W, "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": config_keys(cfg, int(os.environ.get("WORLD_SIZE", "1"))),
+        # the same keys and values as the CUDA arm's `config` (same workload, same t)
+        "config": dict(config_keys(cfg, int(os.environ.get("WORLD_SIZE", "1"))), retained_tokens_per_seq=n_ret // cfg.batch,
+                       t_first_timed=t0 + max(W, 1) + 1,
+                       l2="inputs larger than L2 (each step re-reads %.0f MB of K/V)" % (kv_bytes / 1e6)),
         "what": "fp64 CPU oracle (oracle/), bounded sample per step",
         "cpu_baseline": {"value": us_step, "unit": UNIT, "cores": int(used), "kind": "oracle", "sample": sample},
         "e2e": {"value": us_step, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
