@@ -58,17 +58,19 @@ HBM_FALLBACK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when 
 OTHER_WORKLOADS = ["config3a", "config3b", "config5", "sweep_128_64", "sweep_2250_1024"]
 # sources whose change invalidates an ncu traffic capture of the step kernel (profiles/traffic.md)
 KERNEL_SOURCES = ["decode_attn_mma.cu", "evict_body.cuh", "device_state.cuh", "policy_math.cuh", "ptx_utils.cuh"]
+# ... and of the prefill kernel (workload prefill_300s)
+PREFILL_SOURCES = ["prefill_attn_umma.cu", "umma_utils.cuh", "ptx_utils.cuh"]
 
 
-def kernel_source_hash() -> str:
+def kernel_source_hash(sources=None) -> str:
     h = hashlib.sha256()
-    for f in KERNEL_SOURCES:
+    for f in (sources or KERNEL_SOURCES):
         with open(os.path.join(ROOT, "paper_2606_01483_b200", "csrc", f), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
 
 
-def ncu_traffic_bytes(workload: str):
+def ncu_traffic_bytes(workload: str, sources=None):
     """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the committed
     `ncu --set full` capture (profiles/traffic.md), or None when there is no capture for this workload or
     the kernel sources have changed since it was taken (the row carries their hash)."""
@@ -78,7 +80,7 @@ def ncu_traffic_bytes(workload: str):
                 if not (ln.startswith("| `") and ln.count("|") >= 5):
                     continue
                 c = [x.strip() for x in ln.strip().strip("|").split("|")]
-                if c[0].strip("`") == workload and c[2].strip("`") == kernel_source_hash():
+                if c[0].strip("`") == workload and c[2].strip("`") == kernel_source_hash(sources):
                     return float(c[1])
     except (OSError, ValueError, IndexError):
         pass
@@ -1092,7 +1094,9 @@ def run_prefill(args):
                    "head_dim": g.head_dim, "page_size": cfg.page_size, "l2": "q + out = 2 x 464 MB per call (> 126 MB L2); K/V 133 MB"},
         "tflops": tfs, "tokens_per_s": n / (ms * 1e-3),
         "roofline": {"bound": "tensor", "kernel": "prefill_umma_kernel (tcgen05.mma, accumulators in TMEM, TMA-fed)",
-                     "achieved": tfs, "peak": peak, "unit": "TFLOP/s", "frac": tfs / peak, "traffic": None,
+                     "achieved": tfs, "peak": peak, "unit": "TFLOP/s", "frac": tfs / peak,
+                     "traffic": ncu_traffic_bytes("prefill_300s", PREFILL_SOURCES),
+                     "kernel_source_hash": kernel_source_hash(PREFILL_SOURCES),
                      "peak_source": peak_src, "peak_sustained": peak_sus,
                      "frac_of_sustained_peak": (tfs / peak_sus) if peak_sus else None, "algorithmic_flops_per_launch": flops,
                      "how": "causal flops 4 d sum_x (x + 1) per head and layer / mean launch duration (CUDA events, %d launches)" % K},
