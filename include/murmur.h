@@ -122,6 +122,10 @@ typedef struct {
                                      0 = three launches (append, evict, attention) */
 #define MURMUR_OPT_HOST_ZERO_COPY 6 /* value: 1 (default) = murmur_decode_step_host works on page-locked host buffers
                                       in place (zero-copy); 0 = always stage through device buffers */
+#define MURMUR_OPT_L2_KEEP_PCT 7   /* value: -1 (default) = automatic, else 0..100: percentage of the K/V rows a decode-
+                                      attention launch reads with L2::evict_last instead of L2::evict_first - the retained
+                                      set of step t+1 is that of step t shifted by one token, so whatever part of it fits
+                                      the L2 can be served from there on the next step; results do not depend on it */
 #define MURMUR_OPT_PREFILL_VARIANT 5 /* value: MURMUR_PREFILL_AUTO / _MMA_SYNC / _UMMA */
 #define MURMUR_PREFILL_AUTO 0     /* = MURMUR_PREFILL_UMMA */
 #define MURMUR_PREFILL_MMA_SYNC 1 /* warp-level mma.sync kernel (the round-1 path, kept as a cross-check) */

@@ -23,6 +23,7 @@ MURMUR_OPT_PDL = 3
 MURMUR_OPT_FUSE_STEP = 4
 MURMUR_OPT_PREFILL_VARIANT = 5
 MURMUR_OPT_HOST_ZERO_COPY = 6
+MURMUR_OPT_L2_KEEP_PCT = 7
 MURMUR_PREFILL_AUTO, MURMUR_PREFILL_MMA_SYNC, MURMUR_PREFILL_UMMA = 0, 1, 2
 MURMUR_ATTN_AUTO, MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA = 0, 1, 2
 

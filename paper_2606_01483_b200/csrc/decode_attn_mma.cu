@@ -455,7 +455,7 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
     // per page - so the serial part of issuing a tile (one lane at a time, ring order) is only:
     // wait for the stage, 2 expect_tx, the copies.  That serial path runs at single-warp latency
     // and has to stay well below the ~0.75 us a tile takes to stream at this CTA's share of HBM.
-    const unsigned long long kv_policy = l2_policy_evict_first();
+    const unsigned long long kv_policy = c.l2_keep > 0.f ? l2_policy_keep_fraction(c.l2_keep) : l2_policy_evict_first();
     struct TileIssue {
       unsigned long long off[4];  // byte offset of the page's first copied row in a pool (same in K and V)
       uint32_t dst[4], bytes[4];  // destination offset in the stage buffer, bytes to copy (0 = none)

@@ -94,6 +94,7 @@ struct CacheView {
   int32_t* item_counters;  // [n_layers][max_seqs][n_kv] split-K arrival counters (self-resetting)
   float* partials;       // [4 * kMaxAttnGrid][kPartialFloats]: two slots per tile range, two ranges per CTA
   unsigned long long* timeline;  // [kMaxAttnGrid][kTimelineWords] per-CTA trace of the last attention launch
+  float l2_keep;         // fraction of the K/V rows decode attention reads with L2::evict_last (the rest: evict_first)
 };
 
 #ifdef __CUDACC__

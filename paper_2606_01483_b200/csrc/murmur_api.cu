@@ -109,12 +109,14 @@ struct murmur_cache {
   std::vector<HostSeq> seqs;
   int64_t free_pages;
   int sm_count;
+  int l2_bytes = 0;
   int attn_variant_opt;
   int attn_grid_opt;
   int pdl_opt;         // programmatic dependent launch between the kernels of a step
   int fuse_step_opt;   // murmur_decode_step: append + evict in one launch
   int prefill_variant_opt;  // MURMUR_PREFILL_*
   int host_zero_copy_opt;   // murmur_decode_step_host: work on page-locked host buffers in place
+  int l2_keep_pct_opt;      // MURMUR_OPT_L2_KEEP_PCT (-1 = automatic)
   murmur_stats_t stats;
   cudaError_t last_cuda;
   uint8_t* ws;
@@ -145,6 +147,23 @@ void note(murmur_cache* c, const LaunchInfo& li) {
 inline int32_t blocks_for(int32_t len, int32_t p) { return (len + p - 1) / p; }
 
 // ids in range, active, distinct; want_indexed: 0 = positional sequences only, 1 = indexed-mode sequences only
+// Fraction of the K/V rows a decode-attention launch reads with L2::evict_last (MURMUR_OPT_L2_KEEP_PCT).  Consecutive
+// steps re-read the same retained rows (the windows move by one token), so when the retained rows of all active
+// sequences and layers are not much more than the L2 holds, half an L2 of them is pinned ahead of the rest and served
+// from there on the next step (config 3b, 151 MB per step: 29.8 -> 26.9 us).  For larger working sets any pinned
+// share measured slower than a pure evict_first stream (config 2, 575 MB: 89 -> 92-97 us), so they get none.
+constexpr double kL2KeepShare = 0.5, kL2KeepMaxWorkingSet = 1.3;  // in units of the L2 size
+float l2_keep_fraction(murmur_cache* c) {
+  if (c->l2_keep_pct_opt >= 0) return (float)c->l2_keep_pct_opt / 100.f;
+  double rows = 0;
+  for (const HostSeq& hs : c->seqs)
+    if (hs.active) rows += (double)retained_count(hs.sp);
+  const double bytes = rows * 2.0 * kRowBytes * c->desc.n_kv_heads * c->desc.n_layers;
+  if (bytes <= 0 || bytes > kL2KeepMaxWorkingSet * (double)c->l2_bytes) return 0.f;
+  const double f = kL2KeepShare * (double)c->l2_bytes / bytes;
+  return (float)(f > 1.0 ? 1.0 : f);
+}
+
 murmur_status_t check_ids(murmur_cache* c, const int32_t* ids, int32_t n, int want_indexed = 0) {
   if (!ids || n < 0) return MURMUR_ERR_INVALID_ARG;
   for (int i = 0; i < n; ++i) {
@@ -193,11 +212,13 @@ murmur_status_t murmur_cache_create(const murmur_cache_desc_t* d, murmur_cache_t
   c->fuse_step_opt = 2;
   c->prefill_variant_opt = MURMUR_PREFILL_AUTO;
   c->host_zero_copy_opt = 1;
+  c->l2_keep_pct_opt = -1;
   std::memset(&c->stats, 0, sizeof c->stats);
   c->last_cuda = cudaSuccess;
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->l2_bytes, cudaDevAttrL2CacheSize, dev);
   if (e != cudaSuccess) {
     delete c;
     return MURMUR_ERR_CUDA;
@@ -437,6 +458,7 @@ static murmur_status_t attn_impl(murmur_cache_t* c, const int32_t* seq_ids, int3
     for (int i = 0; i < list.n; ++i) list.ids[i] = seq_ids[base + i];
     LaunchInfo li{};
     if (variant == MURMUR_ATTN_MMA) {
+      c->view.l2_keep = l2_keep_fraction(c);
       MM_CUDA(c, launch_attn_mma(c->view, list, base, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, grid,
                                  c->pdl_opt != 0, window ? &win : nullptr, (cudaStream_t)stream, &li));
     } else {
@@ -516,6 +538,7 @@ static murmur_status_t step_layers_impl(murmur_cache_t* c, const int32_t* seq_id
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     const bool capturing = cudaStreamIsCapturing((cudaStream_t)stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone;
     const long long chain_expect = (c->chain_ok && !capturing && c->pdl_opt != 0) ? (long long)c->step_done : -1;
+    c->view.l2_keep = l2_keep_fraction(c);
     MM_CUDA(c, launch_step_mma(c->view, list, k_new, v_new, q, out, lse, sm_scale, layer_begin, layer_end, !opens, grid,
                                c->pdl_opt != 0, chain_expect, (cudaStream_t)stream, &li));
     note(c, li);
@@ -1093,6 +1116,10 @@ murmur_status_t murmur_set_option(murmur_cache_t* c, int32_t option, int32_t val
       return MURMUR_OK;
     case MURMUR_OPT_HOST_ZERO_COPY:
       c->host_zero_copy_opt = value != 0;
+      return MURMUR_OK;
+    case MURMUR_OPT_L2_KEEP_PCT:
+      if (value < -1 || value > 100) return MURMUR_ERR_INVALID_ARG;
+      c->l2_keep_pct_opt = value;
       return MURMUR_OK;
     case MURMUR_OPT_PREFILL_VARIANT:
       if (value < MURMUR_PREFILL_AUTO || value > MURMUR_PREFILL_UMMA) return MURMUR_ERR_INVALID_ARG;

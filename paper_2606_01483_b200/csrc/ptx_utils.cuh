@@ -43,6 +43,13 @@ __device__ __forceinline__ unsigned long long l2_policy_evict_first() {
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
   return pol;
 }
+// A `keep` fraction of the lines (chosen by address, the same every time) stays in L2 ahead of everything else, the
+// rest leaves first: the part of a decode step's K/V that fits the L2 is served from there on the next step.
+__device__ __forceinline__ unsigned long long l2_policy_keep_fraction(float keep) {
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.L2::evict_first.b64 %0, %1;" : "=l"(pol) : "f"(keep));
+  return pol;
+}
 __device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, uint32_t bytes, unsigned long long* bar,
                                               unsigned long long pol) {
   asm volatile(

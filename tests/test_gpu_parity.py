@@ -175,6 +175,43 @@ def test_split_k_grid_invariance(dev):
     sbs.close()
 
 
+def test_l2_keep_fraction_does_not_change_results(dev):
+    """MURMUR_OPT_L2_KEEP_PCT is a cache hint (which share of the K/V rows is read with L2::evict_last): automatic,
+    0, 40 and 100 % give bit-identical outputs, for the attention call and for one-launch steps."""
+    from paper_2606_01483_b200.binding import MURMUR_OPT_L2_KEEP_PCT
+
+    cfg = workloads.config2().with_layers(3).with_seqs(workloads.config2().seqs[:3])
+    ids = [0, 1, 2]
+    outs = []
+    for pct in (-1, 0, 40, 100):
+        sbs = _mk(cfg, dev)
+        sbs.gpu.set_option(MURMUR_OPT_L2_KEEP_PCT, pct)
+        sbs.bulk_prefill(ids, 300)
+        sbs.append_step(ids)
+        sbs.evict(ids)
+        q = sbs.queries(ids)
+        lse = torch.empty(q.shape[:3], dtype=torch.float32, device=dev)
+        out = sbs.gpu.decode_attn(ids, q, lse=lse, sm_scale=sbs.scale)
+        if pct == -1:
+            sbs.check_attention(ids, q, out, lse)
+        steps = []
+        for _ in range(3):
+            qs, os_, _ = sbs.fused_step(ids, want_lse=True)
+            steps.append(os_.clone())
+        sbs.check_integer_state(ids)
+        outs.append([out.clone()] + steps)
+        sbs.close()
+    for o in outs[1:]:
+        for a, b in zip(o, outs[0]):
+            assert torch.equal(a, b)
+    from paper_2606_01483_b200 import MurmurError
+
+    sbs = _mk(cfg, dev)
+    with pytest.raises(MurmurError):
+        sbs.gpu.set_option(MURMUR_OPT_L2_KEEP_PCT, 101)
+    sbs.close()
+
+
 def test_window_off_equals_full_attention(dev):
     """I1 on the GPU: windows >= lengths -> every position retained, nothing freed."""
     W = workloads.WINDOW_OFF
