@@ -69,7 +69,9 @@ typedef enum {
   MURMUR_ERR_STATE = 2,       /* sequence not active / already active / empty / max_blocks exceeded */
   MURMUR_ERR_OOM_PAGES = 3,   /* the call as a whole needs more pages than are free; nothing changed */
   MURMUR_ERR_CUDA = 4,        /* a CUDA runtime call failed */
-  MURMUR_ERR_UNSUPPORTED = 5  /* geometry outside what the kernels are built for */
+  MURMUR_ERR_UNSUPPORTED = 5, /* geometry outside what the kernels are built for */
+  MURMUR_ERR_SCRATCH_LIMIT = 6 /* murmur_attn_profile_noalloc only: the call needs more scratch than the library's
+                                  built-in MURMUR_PROFILE_NOALLOC_MAX_BYTES; nothing was launched */
 } murmur_status_t;
 
 #define MURMUR_WINDOW_OFF 0x7fffffff /* window >= any length: that region is never evicted */
@@ -307,6 +309,39 @@ MURMUR_API murmur_status_t murmur_attn_profile(murmur_cache_t* cache, const int3
                                                const void* q, const murmur_policy_t* candidate, float mass_frac,
                                                void* out, void* scratch, size_t scratch_bytes, int32_t layer_begin,
                                                int32_t layer_end, float sm_scale, void* stream);
+
+/* murmur_attn_profile for callers that have no way to get a scratch buffer.
+ *
+ * Who that is: murmur_attn_profile wants murmur_profile_scratch_bytes() of device memory from the caller, and the
+ * amount depends on how long the sequences are at the moment of the call.  Some callers cannot produce that:
+ *   - a monitoring hook inside a serving engine that handed ALL device memory to its KV pool and activation arena
+ *     at start-up and forbids (or simply fails) any later cudaMalloc;
+ *   - code running on a latency-critical decode loop, where cudaMalloc / cudaFree would stall the whole GPU (both
+ *     synchronise the device) for a profile that is sampled once in a while;
+ *   - plug-in code called from someone else's runtime (a callback, a foreign-language binding) that is given the
+ *     step's tensors but no handle to that runtime's allocator.
+ * For them the library carries its own scratch: a fixed array of MURMUR_PROFILE_NOALLOC_MAX_BYTES in the library's
+ * device image.  Every GPU that loads the library holds those bytes from load until process exit, used or not -
+ * that is why the limit is modest.  The call allocates nothing: no cudaMalloc, no cudaFree, no library routine that
+ * allocates; q and out are still the caller's.
+ *
+ * Arguments, result and errors are those of murmur_attn_profile (Fig. 5 at PAPER.md:85), without
+ * scratch / scratch_bytes.  In addition:
+ *   - MURMUR_ERR_SCRATCH_LIMIT when murmur_profile_scratch_bytes(cache, seq_ids, n_seqs, layer_begin, layer_end)
+ *     exceeds MURMUR_PROFILE_NOALLOC_MAX_BYTES; nothing is launched.  The need is (layers in the call) x n_seqs x
+ *     n_q_heads x (longest listed sequence, rounded up to 32) x 4 bytes: 8 MiB is e.g. one layer of 16 sequences of
+ *     4 600 tokens at 28 heads, or one 2 314-token sequence over all 28 layers.  Split larger jobs by layer range.
+ *   - The FIRST call on each GPU also looks up where the array lives on that GPU (with that GPU current, as for
+ *     every call on the handle).  Make that first call during set-up, before any stream capture is begun.
+ *   - The array is shared by everything in the process that uses this GPU and keeps the previous call's contents.
+ *     That is harmless for a single call (the kernel writes every element it later reads; nothing has to start at
+ *     zero), but two calls that overlap on the GPU - different streams, handles or threads - overwrite each other's
+ *     rows and both results are garbage.  Issue them on one stream or order them with events. */
+#define MURMUR_PROFILE_NOALLOC_MAX_BYTES (8u << 20)
+MURMUR_API murmur_status_t murmur_attn_profile_noalloc(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
+                                                       const void* q, const murmur_policy_t* candidate,
+                                                       float mass_frac, void* out, int32_t layer_begin,
+                                                       int32_t layer_end, float sm_scale, void* stream);
 
 /* ---- general index-set eviction: "indexed mode" --------------------------------------------
  * "The evictable tokens are not contiguous and cannot be captured by a simple positional policy. This motivates

@@ -28,7 +28,8 @@ MURMUR_PREFILL_AUTO, MURMUR_PREFILL_MMA_SYNC, MURMUR_PREFILL_UMMA = 0, 1, 2
 MURMUR_ATTN_AUTO, MURMUR_ATTN_GENERIC, MURMUR_ATTN_MMA = 0, 1, 2
 
 STATUS_NAMES = {0: "MURMUR_OK", 1: "MURMUR_ERR_INVALID_ARG", 2: "MURMUR_ERR_STATE", 3: "MURMUR_ERR_OOM_PAGES",
-                4: "MURMUR_ERR_CUDA", 5: "MURMUR_ERR_UNSUPPORTED"}
+                4: "MURMUR_ERR_CUDA", 5: "MURMUR_ERR_UNSUPPORTED", 6: "MURMUR_ERR_SCRATCH_LIMIT"}
+MURMUR_PROFILE_NOALLOC_MAX_BYTES = 8 << 20
 
 # every symbol include/murmur.h declares (checked by tests/test_abi.py)
 EXPORTED_SYMBOLS = [
@@ -36,7 +37,7 @@ EXPORTED_SYMBOLS = [
     "murmur_seq_begin", "murmur_seq_end", "murmur_kv_append", "murmur_kv_evict", "murmur_decode_attn",
     "murmur_decode_step", "murmur_decode_step_layers", "murmur_decode_step_chunked", "murmur_decode_step_host", "murmur_mirror_sync", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
-    "murmur_profile_scratch_bytes", "murmur_attn_profile",
+    "murmur_profile_scratch_bytes", "murmur_attn_profile", "murmur_attn_profile_noalloc",
     "murmur_decode_attn_windowed", "murmur_prefill_attn", "murmur_chunk_plan",
     "murmur_indexed_bytes", "murmur_indexed_enable", "murmur_select_scratch_bytes", "murmur_select_mass_sets",
     "murmur_kv_evict_indexed", "murmur_kv_append_indexed", "murmur_decode_attn_indexed", "murmur_kv_get_indexed",
@@ -116,6 +117,7 @@ def lib() -> C.CDLL:
     L.murmur_profile_scratch_bytes.argtypes = [vp, vp, i32, i32, i32]
     L.murmur_profile_scratch_bytes.restype = C.c_size_t
     L.murmur_attn_profile.argtypes = [vp, vp, i32, vp, vp, C.c_float, vp, vp, C.c_size_t, i32, i32, C.c_float, vp]
+    L.murmur_attn_profile_noalloc.argtypes = [vp, vp, i32, vp, vp, C.c_float, vp, i32, i32, C.c_float, vp]
     L.murmur_indexed_bytes.restype = C.c_size_t
     L.murmur_indexed_bytes.argtypes = [C.POINTER(CacheDesc)]
     L.murmur_indexed_enable.argtypes = [vp, vp, C.c_size_t, vp]
@@ -286,6 +288,38 @@ class MurmurCache:
                                                "k_speech", "k_text")] +
                       [(n, np.float32) for n in ("coverage", "mass_prompt", "mass_speech", "mass_text")])
         return out.cpu().numpy().view(dt).reshape(shape[:3])
+
+    def attn_profile_noalloc(self, seq_ids, q: torch.Tensor, out: torch.Tensor, candidate=None, mass_frac: float = 0.99,
+                             sm_scale: Optional[float] = None, layer_begin: int = 0, layer_end: Optional[int] = None):
+        """murmur_attn_profile_noalloc: the same profile for callers that may not allocate device memory (a hook
+        inside an engine that owns all of HBM, a latency-critical loop where cudaMalloc would stall the GPU).  The
+        scratch is a fixed MURMUR_PROFILE_NOALLOC_MAX_BYTES array inside the library, so this method allocates
+        nothing either: `out` is the caller's int32 tensor [layers, n_seqs, n_q, 12] (12 words = murmur_profile_t)
+        and is filled asynchronously on the current stream; view it with `profile_view` after synchronising.
+        Raises MurmurError(6) when the sequences are too long for the built-in array.  Calls that overlap on the
+        GPU share that array and race; the first call on a device should precede any stream capture."""
+        layer_end = self.n_layers if layer_end is None else layer_end
+        ids = _ids(seq_ids)
+        shape = (layer_end - layer_begin, len(ids), self.n_q, self.d)
+        assert q.dtype == torch.bfloat16 and q.is_cuda and q.is_contiguous() and tuple(q.shape) == shape
+        assert out.dtype == torch.int32 and out.is_cuda and out.is_contiguous() and tuple(out.shape) == shape[:3] + (12,)
+        sm_scale = 1.0 / math.sqrt(self.d) if sm_scale is None else sm_scale
+        pol = (C.c_int32 * 5)(*candidate) if candidate is not None else None
+        st = self.L.murmur_attn_profile_noalloc(self.h, ids.ctypes.data, len(ids), q.data_ptr(), pol,
+                                                C.c_float(mass_frac), out.data_ptr(), layer_begin, layer_end,
+                                                C.c_float(sm_scale), _stream())
+        if st == 6:
+            raise MurmurError(st, f"the profile needs more than the built-in {MURMUR_PROFILE_NOALLOC_MAX_BYTES} bytes of "
+                                  "scratch: use fewer layers or sequences per call, or murmur_attn_profile with your own buffer")
+        self._check(st)
+
+    @staticmethod
+    def profile_view(out: torch.Tensor) -> np.ndarray:
+        """Structured view (fields of murmur_profile_t) of an `out` tensor of attn_profile_noalloc; synchronises."""
+        dt = np.dtype([(n, np.int32) for n in ("n_resident", "n_prompt", "n_speech", "n_text", "k_mass", "k_prompt",
+                                               "k_speech", "k_text")] +
+                      [(n, np.float32) for n in ("coverage", "mass_prompt", "mass_speech", "mass_text")])
+        return out.cpu().numpy().view(dt).reshape(tuple(out.shape[:3]))
 
     def decode_step(self, seq_ids, k_new: torch.Tensor, v_new: torch.Tensor, q: torch.Tensor, out: torch.Tensor,
                     lse: Optional[torch.Tensor] = None, sm_scale: Optional[float] = None):

@@ -19,8 +19,17 @@
 //           k = #{e > tau} + (as many of the ties at tau, in ascending position, as are needed).
 #include <cuda_bf16.h>
 
+#include <mutex>
+
 #include "../../include/murmur.h"
 #include "device_state.cuh"
+
+// Built-in scratch of murmur_attn_profile_noalloc (see the end of this file and include/murmur.h).  It is part of
+// the library image: every GPU that loads libmurmur.so sets these 8 MiB of its memory aside until the process
+// exits, whether or not the call is ever made.  One array per GPU, shared by every handle, stream and thread.
+// The name below is only usable as an address in DEVICE code; host code has to ask the runtime for the array's
+// address on the current device (cudaGetSymbolAddress) - launch_attn_profile_noalloc does, once per device.
+static __device__ __align__(256) unsigned char murmur_profile_builtin_scratch[MURMUR_PROFILE_NOALLOC_MAX_BYTES];
 
 namespace murmur {
 namespace {
@@ -279,6 +288,50 @@ cudaError_t launch_attn_profile(const CacheView& c, const SeqList& list, int seq
   info->launches += 1;
   info->grid = (int)(grid.x * grid.y * grid.z);
   return cudaGetLastError();
+}
+
+// ---- the profile for callers that cannot provide scratch ------------------------------------------------------
+// Same kernel, same arguments, but the per-head score rows go to murmur_profile_builtin_scratch instead of a
+// buffer of the caller's.  Nothing is allocated here or anywhere below: one cudaGetDevice, on the first call per
+// device one cudaGetSymbolAddress, and the launch.
+//
+// What the caller must know (repeated in murmur.h):
+//   * the first call on a device looks the array's device address up; that look-up may load the module on the
+//     device, so make this first call outside any stream capture;
+//   * the array keeps whatever the previous call left in it.  The kernel needs no zeroed scratch: pass 1 writes
+//     scratch[h][x] for every head h of the group and every x < len before pass 2 reads it, and nothing beyond
+//     len is ever read, so there is nothing to clear;
+//   * two calls in flight at once on one GPU (two streams, two handles, two threads) write the same rows and
+//     corrupt each other's result.  Order them.
+namespace {
+constexpr int kMaxDevicesTracked = 64;
+std::mutex g_builtin_mu;
+float* g_builtin_ptr[kMaxDevicesTracked];  // device address of the array per device ordinal; null = not looked up yet
+}  // namespace
+
+cudaError_t launch_attn_profile_noalloc(const CacheView& c, const SeqList& list, int n_seqs_total, const void* q,
+                                        const SeqParams* candidate, float frac, void* out, long long stride,
+                                        size_t scratch_bytes_needed, int layer_begin, int layer_end, float sm_scale,
+                                        cudaStream_t st, LaunchInfo* info) {
+  if (scratch_bytes_needed > sizeof(murmur_profile_builtin_scratch)) return cudaErrorInvalidValue;  // API checks first
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevicesTracked) return cudaErrorInvalidDevice;
+  float* scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(g_builtin_mu);
+    scratch = g_builtin_ptr[dev];
+    if (scratch == nullptr) {
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, murmur_profile_builtin_scratch);  // address on the CURRENT device
+      if (e != cudaSuccess) return e;
+      if (p == nullptr) return cudaErrorInvalidSymbol;
+      g_builtin_ptr[dev] = scratch = reinterpret_cast<float*>(p);
+    }
+  }
+  return launch_attn_profile(c, list, 0, n_seqs_total, q, candidate, frac, out, scratch, stride, layer_begin,
+                             layer_end, sm_scale, nullptr, st, info);
 }
 
 }  // namespace murmur

@@ -228,6 +228,11 @@ cudaError_t launch_attn_profile(const CacheView& c, const SeqList& list, int seq
                                 const SeqParams* candidate, float frac, void* out, float* scratch, long long stride,
                                 int layer_begin, int layer_end, float sm_scale, uint8_t* member_mask, cudaStream_t st,
                                 LaunchInfo* info);
+// The same launch with the library's built-in scratch array (attn_profile.cu); allocates nothing.
+cudaError_t launch_attn_profile_noalloc(const CacheView& c, const SeqList& list, int n_seqs_total, const void* q,
+                                        const SeqParams* candidate, float frac, void* out, long long stride,
+                                        size_t scratch_bytes_needed, int layer_begin, int layer_end, float sm_scale,
+                                        cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_indexed_defrag(const CacheView& c, const IdxView& ix, int seq, const int32_t* sel_pos, const int32_t* sel_cnt,
                                   int cap_sel, bool from_positional, unsigned long long* moved_dev, cudaStream_t st,
                                   LaunchInfo* info);

@@ -735,6 +735,38 @@ murmur_status_t murmur_attn_profile(murmur_cache_t* c, const int32_t* seq_ids, i
   return MURMUR_OK;
 }
 
+// The profile with the library's built-in scratch (attn_profile.cu): for callers that cannot allocate - see murmur.h.
+// Validation is that of murmur_attn_profile; the scratch need is checked against the fixed array before any launch.
+murmur_status_t murmur_attn_profile_noalloc(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q,
+                                            const murmur_policy_t* cand, float mass_frac, void* out,
+                                            int32_t layer_begin, int32_t layer_end, float sm_scale, void* stream) {
+  if (!c || !q || !out) return MURMUR_ERR_INVALID_ARG;
+  if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch) return MURMUR_ERR_INVALID_ARG;
+  murmur_status_t st = check_ids(c, seq_ids, n_seqs);
+  if (st != MURMUR_OK) return st;
+  if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
+  if (!(sm_scale > 0.f) || !(mass_frac > 0.f) || mass_frac > 1.f) return MURMUR_ERR_INVALID_ARG;
+  if (cand && (cand->w_speech < 0 || cand->delay < 0 || cand->n_sink_speech < 0 || cand->w_out < 0 || cand->n_sink_out < 0))
+    return MURMUR_ERR_INVALID_ARG;
+  for (int i = 0; i < n_seqs; ++i)
+    if (c->seqs[seq_ids[i]].sp.len < 1) return MURMUR_ERR_STATE;
+  const size_t need = murmur_profile_scratch_bytes(c, seq_ids, n_seqs, layer_begin, layer_end);
+  if (need == 0) return MURMUR_ERR_INVALID_ARG;
+  if (need > (size_t)MURMUR_PROFILE_NOALLOC_MAX_BYTES) return MURMUR_ERR_SCRATCH_LIMIT;
+  SeqList list;
+  list.n = n_seqs;
+  for (int i = 0; i < n_seqs; ++i) list.ids[i] = seq_ids[i];
+  SeqParams cs{};
+  if (cand) {
+    cs.w_s = cand->w_speech; cs.d = cand->delay; cs.k_s = cand->n_sink_speech; cs.w_o = cand->w_out; cs.k_o = cand->n_sink_out;
+  }
+  LaunchInfo li{};
+  MM_CUDA(c, launch_attn_profile_noalloc(c->view, list, n_seqs, q, cand ? &cs : nullptr, mass_frac, out,
+                                         profile_stride(c, seq_ids, n_seqs), need, layer_begin, layer_end, sm_scale,
+                                         (cudaStream_t)stream, &li));
+  note(c, li);
+  return MURMUR_OK;
+}
 
 // ---- general index-set eviction (indexed mode) ------------------------------------------------------
 static size_t idx_len_bytes(const murmur_cache_desc_t* d) {
@@ -1154,6 +1186,7 @@ const char* murmur_status_str(murmur_status_t s) {
     case MURMUR_ERR_OOM_PAGES: return "MURMUR_ERR_OOM_PAGES";
     case MURMUR_ERR_CUDA: return "MURMUR_ERR_CUDA";
     case MURMUR_ERR_UNSUPPORTED: return "MURMUR_ERR_UNSUPPORTED";
+    case MURMUR_ERR_SCRATCH_LIMIT: return "MURMUR_ERR_SCRATCH_LIMIT";
   }
   return "MURMUR_ERR_?";
 }
