@@ -219,12 +219,18 @@ attn_mma_kernel(const __grid_constant__ CacheView c, const __grid_constant__ Seq
   // partials and counters, the keepers' scatter / commit / evict) still sits behind griddepcontrol.wait.  The
   // counter is only a go-ahead: if it does not show the expected value in time (a replayed CUDA graph, whose
   // launches the host did not count), the CTA falls back to griddepcontrol.wait, which is always sufficient.
+  // The test is "expected <= counter < expected + this launch's own CTAs" (wrap-safe), not equality: keepers of
+  // THIS launch add to the same counter, and a CTA that starts after some of them are done - a second-wave CTA when
+  // the grid exceeds the SM count, or one delayed by other work - would never see the exact value and spin out the
+  // whole time-out with the step's commit and eviction stalled behind it.  A keeper of this launch can only finish
+  // after griddepcontrol.wait, i.e. after the predecessor ended, so counter >= expected still means that every
+  // keeper of the predecessor is done; every CTA of a launch adds exactly 1, which bounds the window from above.
   bool chained = false;
   if (kStep && prm.chain) {
     if (tid == 0) {
       int ok = 0;
       for (int it = 0; it < 4096 && !ok; ++it) {
-        ok = ((unsigned)ld_acquire(&c.ctrl[kCtrlStepDone]) == prm.chain_expect) ? 1 : 0;
+        ok = ((unsigned)ld_acquire(&c.ctrl[kCtrlStepDone]) - prm.chain_expect < gridDim.x) ? 1 : 0;
         if (!ok) __nanosleep(64);
       }
       s.chain_ok = ok;

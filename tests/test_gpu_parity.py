@@ -541,6 +541,47 @@ def test_decode_step_back_to_back_without_host_sync(dev):
     a.close()
 
 
+def test_chained_steps_with_more_ctas_than_sms(dev):
+    """Chained step launches whose grid exceeds one wave (MURMUR_OPT_ATTN_GRID = 1000): a second-wave CTA starts
+    after first-wave keepers of its OWN launch have already added to the go-ahead counter, so it must accept
+    "counter >= expected", not only equality - otherwise it spins out the whole time-out (0.3 - 3 ms) on every step
+    with the step's commit stalled behind it.  Results must match the oracle, and the chained steps may not be
+    slower than a small multiple of the same steps launched without programmatic dependent launch (no chain)."""
+    from paper_2606_01483_b200 import MURMUR_OPT_ATTN_GRID, MURMUR_OPT_PDL
+
+    cfg = workloads.config2().with_layers(2)
+    a = _mk(cfg, dev)
+    ids = list(range(cfg.batch))
+    a.bulk_prefill(ids, 250)
+    a.gpu.set_option(MURMUR_OPT_ATTN_GRID, 1000)
+    keep = []
+    for k in range(12):  # back to back, no host sync: steps 1.. are chained
+        keep.append(a.fused_step(ids, want_lse=True) + ({i: list(a.oracle.retained(i)) for i in ids},))
+    torch.cuda.synchronize()
+    a.check_integer_state(ids)
+    for q, out, lse, ret in keep[-3:]:
+        a.check_attention(ids, q, out, lse, retained=ret)
+    # timing: the same device inputs every step, GPU side only (the oracle is not advanced from here on)
+    q, out, _lse, _ = keep[-1]
+    k_new = torch.randn(2, len(ids), 4, 128, device=dev).to(torch.bfloat16)
+    v_new = torch.randn(2, len(ids), 4, 128, device=dev).to(torch.bfloat16)
+    times = {}
+    for pdl in (1, 0, 1, 0):
+        a.gpu.set_option(MURMUR_OPT_PDL, pdl)
+        for _ in range(3):
+            a.gpu.decode_step(ids, k_new, v_new, q, out, None, a.scale)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(30):
+            a.gpu.decode_step(ids, k_new, v_new, q, out, None, a.scale)
+        e1.record()
+        torch.cuda.synchronize()
+        times[pdl] = min(times.get(pdl, 1e9), e0.elapsed_time(e1) / 30)
+    assert a.gpu.last_error() == 0
+    assert times[1] < 3.0 * times[0] + 0.02, f"chained {times[1] * 1e3:.1f} us/step vs unchained {times[0] * 1e3:.1f} us/step"
+    a.close()
+
+
 def test_decode_step_soak_small_pages_many_allocations(dev):
     """600 one-launch steps enqueued without host synchronisation on a page-16 cache with small
     windows: every sequence allocates a page every 16 steps while others are freed in the same launch
