@@ -124,10 +124,13 @@ typedef struct {
                                      0 = three launches (append, evict, attention) */
 #define MURMUR_OPT_HOST_ZERO_COPY 6 /* value: 1 (default) = murmur_decode_step_host works on page-locked host buffers
                                       in place (zero-copy); 0 = always stage through device buffers */
-#define MURMUR_OPT_L2_KEEP_PCT 7   /* value: -1 (default) = automatic, else 0..100: percentage of the K/V rows a decode-
-                                      attention launch reads with L2::evict_last instead of L2::evict_first - the retained
-                                      set of step t+1 is that of step t shifted by one token, so whatever part of it fits
-                                      the L2 can be served from there on the next step; results do not depend on it */
+#define MURMUR_OPT_L2_KEEP_PCT 7   /* value: 0 (default) .. 100: percentage of the K/V rows a decode-attention launch reads
+                                      with L2::evict_last instead of L2::evict_first - the retained set of step t+1 is that
+                                      of step t shifted by one token, so whatever part of it fits the L2 can be served from
+                                      there on the next step; -1 = automatic (half an L2 when the retained rows of the
+                                      sequences in the call are at most 1.3 L2 sizes, else none).  Opt-in because pinned
+                                      lines are never demoted and take L2 from whatever else runs between two attention
+                                      calls; results do not depend on it */
 #define MURMUR_OPT_PREFILL_VARIANT 5 /* value: MURMUR_PREFILL_AUTO / _MMA_SYNC / _UMMA */
 #define MURMUR_PREFILL_AUTO 0     /* = MURMUR_PREFILL_UMMA */
 #define MURMUR_PREFILL_MMA_SYNC 1 /* warp-level mma.sync kernel (the round-1 path, kept as a cross-check) */
@@ -389,7 +392,8 @@ MURMUR_API murmur_status_t murmur_kv_append_indexed(murmur_cache_t* cache, const
                                                     const void* k_new, const void* v_new, void* stream);
 /* Eq. 1 of every query head hq over the rows of slab (l, hq / group), all layers.
  *   q, out : DEVICE bf16 [n_layers][n_seqs][n_q_heads][head_dim];  lse: DEVICE fp32 [n_layers][n_seqs][n_q_heads] or NULL
- * First path (FFMA straight from the pool); the tensor-core streaming kernel serves the positional mode. */
+ * page_size >= 16: the streaming tensor-core kernel (one CTA per slab: bulk-copy ring, mma.sync, fragment-layout
+ * merge); smaller pages: FFMA straight from the pool. */
 MURMUR_API murmur_status_t murmur_decode_attn_indexed(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
                                                       const void* q, void* out, float* lse, float sm_scale, void* stream);
 /* Introspection (synchronise): the original positions held by slab (layer, kv_head), by slot; and the rows of every

@@ -147,17 +147,19 @@ void note(murmur_cache* c, const LaunchInfo& li) {
 inline int32_t blocks_for(int32_t len, int32_t p) { return (len + p - 1) / p; }
 
 // ids in range, active, distinct; want_indexed: 0 = positional sequences only, 1 = indexed-mode sequences only
-// Fraction of the K/V rows a decode-attention launch reads with L2::evict_last (MURMUR_OPT_L2_KEEP_PCT).  Consecutive
-// steps re-read the same retained rows (the windows move by one token), so when the retained rows of all active
-// sequences and layers are not much more than the L2 holds, half an L2 of them is pinned ahead of the rest and served
-// from there on the next step (config 3b, 151 MB per step: 29.8 -> 26.9 us).  For larger working sets any pinned
-// share measured slower than a pure evict_first stream (config 2, 575 MB: 89 -> 92-97 us), so they get none.
+// Fraction of the K/V rows a decode-attention launch reads with L2::evict_last (MURMUR_OPT_L2_KEEP_PCT).  The default
+// is 0: a pure evict_first stream that leaves the L2 to whatever else the engine runs between two attention calls
+// (its GEMMs and activations) - lines marked evict_last are never demoted by this library, and a benchmark of
+// back-to-back attention steps cannot see what they cost the neighbours.  Opt-in, -1 = automatic: consecutive steps
+// re-read the same retained rows (the windows move by one token), so when the retained rows of the sequences IN THE
+// CALL, over all layers, are not much more than the L2 holds, half an L2 of them is pinned ahead of the rest and
+// served from there on the next step (config 3b, 151 MB per step: 29.8 -> 26.9 us).  For larger working sets any
+// pinned share measured slower than a pure evict_first stream (config 2, 575 MB: 89 -> 92-97 us), so they get none.
 constexpr double kL2KeepShare = 0.5, kL2KeepMaxWorkingSet = 1.3;  // in units of the L2 size
-float l2_keep_fraction(murmur_cache* c) {
+float l2_keep_fraction(murmur_cache* c, const int32_t* seq_ids, int32_t n_seqs) {
   if (c->l2_keep_pct_opt >= 0) return (float)c->l2_keep_pct_opt / 100.f;
   double rows = 0;
-  for (const HostSeq& hs : c->seqs)
-    if (hs.active) rows += (double)retained_count(hs.sp);
+  for (int i = 0; i < n_seqs; ++i) rows += (double)retained_count(c->seqs[seq_ids[i]].sp);
   const double bytes = rows * 2.0 * kRowBytes * c->desc.n_kv_heads * c->desc.n_layers;
   if (bytes <= 0 || bytes > kL2KeepMaxWorkingSet * (double)c->l2_bytes) return 0.f;
   const double f = kL2KeepShare * (double)c->l2_bytes / bytes;
@@ -212,7 +214,7 @@ murmur_status_t murmur_cache_create(const murmur_cache_desc_t* d, murmur_cache_t
   c->fuse_step_opt = 2;
   c->prefill_variant_opt = MURMUR_PREFILL_AUTO;
   c->host_zero_copy_opt = 1;
-  c->l2_keep_pct_opt = -1;
+  c->l2_keep_pct_opt = 0;
   std::memset(&c->stats, 0, sizeof c->stats);
   c->last_cuda = cudaSuccess;
   int dev = 0;
@@ -458,7 +460,7 @@ static murmur_status_t attn_impl(murmur_cache_t* c, const int32_t* seq_ids, int3
     for (int i = 0; i < list.n; ++i) list.ids[i] = seq_ids[base + i];
     LaunchInfo li{};
     if (variant == MURMUR_ATTN_MMA) {
-      c->view.l2_keep = l2_keep_fraction(c);
+      c->view.l2_keep = l2_keep_fraction(c, list.ids, list.n);
       MM_CUDA(c, launch_attn_mma(c->view, list, base, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, grid,
                                  c->pdl_opt != 0, window ? &win : nullptr, (cudaStream_t)stream, &li));
     } else {
@@ -538,7 +540,7 @@ static murmur_status_t step_layers_impl(murmur_cache_t* c, const int32_t* seq_id
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     const bool capturing = cudaStreamIsCapturing((cudaStream_t)stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone;
     const long long chain_expect = (c->chain_ok && !capturing && c->pdl_opt != 0) ? (long long)c->step_done : -1;
-    c->view.l2_keep = l2_keep_fraction(c);
+    c->view.l2_keep = l2_keep_fraction(c, seq_ids, n_seqs);
     MM_CUDA(c, launch_step_mma(c->view, list, k_new, v_new, q, out, lse, sm_scale, layer_begin, layer_end, !opens, grid,
                                c->pdl_opt != 0, chain_expect, (cudaStream_t)stream, &li));
     note(c, li);
