@@ -381,7 +381,9 @@ MURMUR_API murmur_status_t murmur_select_mass_sets(murmur_cache_t* cache, int32_
  * The compaction is in place (rows only move towards lower addresses); *bytes_moved_out (HOST, may be NULL) = bytes of
  * K/V rows that changed address - the cost of cache management made countable.  A positional
  * sequence must have been evicted since its last append (its live page list is the source).  SYNCHRONISES the stream
- * (the set sizes are read back for the page accounting).  A position that is not held raises the device error word. */
+ * (the set sizes are read back for the page accounting).  The sets are validated on the device before any row moves:
+ * a set that is empty, larger than cap, not strictly ascending, or names a position its slab does not hold returns
+ * MURMUR_ERR_INVALID_ARG with the sequence, its rows, its pages and its mode unchanged. */
 MURMUR_API murmur_status_t murmur_kv_evict_indexed(murmur_cache_t* cache, int32_t seq, const int32_t* sel_pos,
                                                    const int32_t* sel_cnt, int32_t cap, int64_t* bytes_moved_out,
                                                    void* stream);

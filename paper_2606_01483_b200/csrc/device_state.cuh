@@ -233,6 +233,10 @@ cudaError_t launch_attn_profile_noalloc(const CacheView& c, const SeqList& list,
                                         const SeqParams* candidate, float frac, void* out, long long stride,
                                         size_t scratch_bytes_needed, int layer_begin, int layer_end, float sm_scale,
                                         cudaStream_t st, LaunchInfo* info);
+// Read-only validation of index sets (sizes, strict order, membership); *bad_dev must be 0 on entry.
+cudaError_t launch_indexed_validate(const CacheView& c, const IdxView& ix, int seq, const int32_t* sel_pos,
+                                    const int32_t* sel_cnt, int cap_sel, bool from_positional, int* bad_dev,
+                                    cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_indexed_defrag(const CacheView& c, const IdxView& ix, int seq, const int32_t* sel_pos, const int32_t* sel_cnt,
                                   int cap_sel, bool from_positional, unsigned long long* moved_dev, cudaStream_t st,
                                   LaunchInfo* info);

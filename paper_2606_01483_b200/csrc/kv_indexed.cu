@@ -117,6 +117,49 @@ indexed_defrag_kernel(const __grid_constant__ CacheView c, const __grid_constant
   if (sub == 0 && n_moved) atomicAdd(moved, n_moved);
 }
 
+// Read-only check of the index sets before anything moves: every set has 1 .. min(cap_sel, table capacity) elements,
+// is strictly ascending, names only positions its slab holds, and fits the blocks the sequence keeps.  The first
+// violation's code lands in *bad (1 = size / order, 2 = a position that is not held); the defrag is launched only when
+// the host has read 0 there - an in-place compaction cannot be undone once rows have been overwritten.
+__global__ void __launch_bounds__(kIdxThreads)
+indexed_validate_kernel(const __grid_constant__ CacheView c, const __grid_constant__ IdxView ix, int seq,
+                        const int32_t* __restrict__ sel_pos, const int32_t* __restrict__ sel_cnt, int cap_sel,
+                        int from_positional, int* __restrict__ bad) {
+  const int slab = blockIdx.x;
+  const int plog = c.p_log2;
+  const SeqDev& sd = c.seqs[seq];
+  const int32_t* sel = sel_pos + (size_t)slab * cap_sel;
+  const int n_new = sel_cnt[slab];
+  if (n_new < 1 || n_new > cap_sel || n_new > ix.cap) {
+    if (threadIdx.x == 0) atomicCAS(bad, 0, 1);
+    return;
+  }
+  const int32_t* pos = ix.pos + ((size_t)seq * c.n_layers * c.n_kv + slab) * ix.cap;
+  const int n_old = from_positional ? 0 : ix.len[(size_t)seq * c.n_layers * c.n_kv + slab];
+  const int32_t* lblocks = c.live_blocks + (size_t)seq * c.max_blocks;
+  const int n_live = sd.n_live;
+  const int blocks_kept = from_positional ? n_live : sd.idx_blocks;
+  if (((n_new - 1) >> plog) >= blocks_kept) {  // the last destination slot has no page
+    if (threadIdx.x == 0) atomicCAS(bad, 0, 2);
+    return;
+  }
+  int err = 0;
+  for (int s = threadIdx.x; s < n_new; s += kIdxThreads) {
+    const int x = sel[s];
+    if (s > 0 && sel[s - 1] >= x) err = err ? err : 1;
+    bool held;
+    if (from_positional) {
+      const int k = upper_index(lblocks, n_live, x >> plog);
+      held = x >= 0 && x < sd.len && k >= 0 && lblocks[k] == (x >> plog);
+    } else {
+      const int so = upper_index(pos, n_old, x);
+      held = so >= 0 && pos[so] == x;
+    }
+    if (!held) err = err ? err : 2;
+  }
+  if (err) atomicCAS(bad, 0, err);
+}
+
 // After the slabs: keep blocks 0 .. ceil(max len / p) - 1, push the surplus pages (ascending), switch the mode.
 __global__ void indexed_commit_kernel(const __grid_constant__ CacheView c, const __grid_constant__ IdxView ix, int seq,
                                       int from_positional) {
@@ -408,6 +451,15 @@ select_compact_kernel(const __grid_constant__ CacheView c, int seq, const uint8_
 }
 
 }  // namespace
+
+cudaError_t launch_indexed_validate(const CacheView& c, const IdxView& ix, int seq, const int32_t* sel_pos,
+                                    const int32_t* sel_cnt, int cap_sel, bool from_positional, int* bad_dev,
+                                    cudaStream_t st, LaunchInfo* info) {
+  indexed_validate_kernel<<<c.n_layers * c.n_kv, kIdxThreads, 0, st>>>(c, ix, seq, sel_pos, sel_cnt, cap_sel,
+                                                                       from_positional ? 1 : 0, bad_dev);
+  info->launches += 1;
+  return cudaGetLastError();
+}
 
 cudaError_t launch_indexed_defrag(const CacheView& c, const IdxView& ix, int seq, const int32_t* sel_pos, const int32_t* sel_cnt,
                                   int cap_sel, bool from_positional, unsigned long long* moved_dev, cudaStream_t st,

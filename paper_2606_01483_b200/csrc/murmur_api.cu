@@ -836,7 +836,17 @@ murmur_status_t murmur_kv_evict_indexed(murmur_cache_t* c, int32_t seq, const in
   cudaStream_t s = (cudaStream_t)stream;
   const int n_slabs = c->desc.n_layers * c->desc.n_kv_heads;
   std::vector<int32_t> cnt(n_slabs);
+  // The sets are checked on the device BEFORE anything moves (sizes, strict ascending order, every position held by
+  // its slab): the compaction is in place, so a bad set found half-way could not be undone.  The verdict word shares
+  // the 256-byte block of the moved-rows counter and is read in the synchronisation that fetches the set sizes.
+  int* bad_dev = reinterpret_cast<int*>(c->idx_moved) + 4;
+  int32_t bad = 0;
+  LaunchInfo lv{};
+  MM_CUDA(c, cudaMemsetAsync(bad_dev, 0, 4, s));
+  MM_CUDA(c, launch_indexed_validate(c->view, c->idx, seq, sel_pos, sel_cnt, cap, !hs.indexed, bad_dev, s, &lv));
+  note(c, lv);
   MM_CUDA(c, cudaMemcpyAsync(cnt.data(), sel_cnt, (size_t)n_slabs * 4, cudaMemcpyDeviceToHost, s));
+  MM_CUDA(c, cudaMemcpyAsync(&bad, bad_dev, 4, cudaMemcpyDeviceToHost, s));
   MM_CUDA(c, cudaStreamSynchronize(s));
   const int32_t held = hs.indexed ? hs.idx_max_len : hs.sp.len;  // a slab cannot grow by eviction
   int32_t mx = 0;
@@ -844,6 +854,7 @@ murmur_status_t murmur_kv_evict_indexed(murmur_cache_t* c, int32_t seq, const in
     if (cnt[i] < 1 || cnt[i] > cap || cnt[i] > held) return MURMUR_ERR_INVALID_ARG;
     mx = cnt[i] > mx ? cnt[i] : mx;
   }
+  if (bad != 0) return MURMUR_ERR_INVALID_ARG;  // nothing moved, no page freed, the sequence keeps its mode
   const int32_t p = c->desc.page_size;
   const int32_t blocks_held = hs.indexed ? hs.idx_blocks : blocks_for(hs.sp.len, p) - hs.freed_blocks;
   const int32_t nb_new = blocks_for(mx, p);

@@ -244,8 +244,57 @@ def test_indexed_error_behaviour(dev):
     with pytest.raises(MurmurError) as e:
         c.kv_append([0], [1], k1, k1.clone())
     assert e.value.status == 2
+    # bad sets are refused BEFORE anything moves: state, rows, pages and mode stay as they were
+    before = [c.indexed_positions(0, l, h).tolist() for l in range(2) for h in range(4)]
+    free_before = list(c.free_stack())
     pos2 = pos.clone()
-    pos2[0, 0, 2] = 30  # position 30 is not held by slab (0, 0) any more: device error word
-    c.kv_evict_indexed(0, pos2, cnt)
-    assert c.last_error() != 0
+    pos2[0, 0, 2] = 30  # position 30 is not held by slab (0, 0) any more
+    pos3 = pos.clone()
+    pos3[1, 2, 1], pos3[1, 2, 2] = 2, 1  # not ascending
+    pos4 = pos.clone()
+    pos4[1, 3, 1] = 0  # a repeated position
+    for badpos in (pos2, pos3, pos4):
+        with pytest.raises(MurmurError) as e:
+            c.kv_evict_indexed(0, badpos, cnt)
+        assert e.value.status == 1
+        assert [c.indexed_positions(0, l, h).tolist() for l in range(2) for h in range(4)] == before
+        assert list(c.free_stack()) == free_before and c.last_error() == 0
+    two = torch.full((2, 4), 2, dtype=torch.int32, device=dev)
+    c.kv_evict_indexed(0, pos, two)  # a good set still goes through afterwards
+    assert c.indexed_positions(0, 0, 0).tolist() == [0, 1]
+    assert c.last_error() == 0
+    c.close()
+
+
+def test_bad_index_set_on_a_positional_sequence_changes_nothing(dev):
+    """The first murmur_kv_evict_indexed of a sequence (positional -> indexed): a set naming an evicted position or a
+    position beyond the length is refused, the sequence stays positional and its rows are untouched."""
+    from paper_2606_01483_b200 import MurmurCache, MurmurError
+
+    c = MurmurCache(2, 28, 4, 128, 16, max_seqs=1, max_blocks_per_seq=8, n_pages=10, device=dev)
+    c.seq_begin(0, 4, 60, 0, (16, 0, 0, 8, 1))  # speech window 16 of 60: whole blocks behind it are freed
+    g = torch.Generator().manual_seed(11)
+    kv = torch.randn(2, 100, 4, 128, generator=g).to(torch.bfloat16).to(dev)
+    c.kv_append([0], [100], kv, kv.clone())
+    c.kv_evict([0])
+    retained = c.retained(0).tolist()
+    pages_before, blocks_before = c.page_list(0)
+    dead = next(x for x in range(100) if (x >> 4) not in set(int(b) for b in blocks_before))
+    c.indexed_enable()
+    good = torch.tensor(retained[:6], dtype=torch.int32)
+    for badval in (dead, 100, -1):
+        pos = good.repeat(2, 4, 1).contiguous()
+        pos[1, 1, 5] = badval
+        if badval == -1:
+            pos[1, 1] = torch.tensor([-1] + retained[:5], dtype=torch.int32)
+        cnt = torch.full((2, 4), 6, dtype=torch.int32, device=dev)
+        with pytest.raises(MurmurError) as e:
+            c.kv_evict_indexed(0, pos.to(dev), cnt)
+        assert e.value.status == 1
+    assert c.retained(0).tolist() == retained and c.last_error() == 0
+    assert list(c.page_list(0)[0]) == list(pages_before)
+    kg, vg = c.gather(0, retained, 0, 2)
+    assert torch.equal(kg.cpu(), kv[:, retained].cpu())
+    q = torch.randn(2, 1, 28, 128, generator=g).to(torch.bfloat16).to(dev)
+    c.decode_attn([0], q)  # still a positional sequence
     c.close()
