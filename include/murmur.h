@@ -219,7 +219,9 @@ MURMUR_API murmur_status_t murmur_decode_step(murmur_cache_t* cache, const int32
  * sequence, advances the lengths and runs the eviction - and must come first; calls with layer_begin > 0 only
  * write their layers' rows and attend (MURMUR_ERR_STATE unless the step is open for every listed sequence;
  * rows of a token the open step's eviction already freed are dropped).  Layer ranges may be issued in any
- * order and size after the opening one; murmur_decode_step == one call with [0, n_layers).
+ * order and size after the opening one, each layer ONCE: the step closes when every layer has been issued, and a
+ * range that touches a layer already issued in this step, or comes after a murmur_kv_append / murmur_kv_evict of
+ * the sequence, is MURMUR_ERR_STATE.  murmur_decode_step == one call with [0, n_layers).
  *   k_new, v_new : DEVICE bf16 [layer_end-layer_begin][n_seqs][n_kv_heads][head_dim]
  *   q, out       : DEVICE bf16 [layer_end-layer_begin][n_seqs][n_q_heads][head_dim];  lse likewise or NULL */
 MURMUR_API murmur_status_t murmur_decode_step_layers(murmur_cache_t* cache, const int32_t* seq_ids, int32_t n_seqs,
@@ -255,7 +257,10 @@ MURMUR_API murmur_status_t murmur_decode_step_host(murmur_cache_t* cache, const 
  * replay once per decode step.  Replays bypass the host-side validation (the kernels keep the device error word: page
  * exhaustion or max_blocks_per_seq raise it and the step does nothing) and the host mirror of lengths and free pages.
  * Call murmur_mirror_sync (synchronises `stream`) before the next non-replayed call on the handle; it re-reads lengths
- * and the free-stack height from the device.  Sequences may not begin or end inside a replayed stretch. */
+ * and the free-stack height from the device.  This is enforced: once a call has been recorded into a graph, every
+ * state-dependent call made outside a capture (sequence begin / end, append, evict, attention, step, prefill, the
+ * indexed calls) returns MURMUR_ERR_STATE until murmur_mirror_sync has run; introspection, options and statistics
+ * stay available.  Sequences may not begin or end inside a replayed stretch. */
 MURMUR_API murmur_status_t murmur_mirror_sync(murmur_cache_t* cache, void* stream);
 
 /* ---- chunking (host only) ------------------------------------------------------------------ */

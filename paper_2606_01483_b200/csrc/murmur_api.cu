@@ -42,6 +42,12 @@ struct HostSeq {
   bool indexed = false;      // indexed mode (kv_indexed.cu): the positional fields above are frozen
   int32_t idx_blocks = 0;    // blocks mapped in indexed mode
   int32_t idx_max_len = 0;   // rows of the longest slab
+  // Open decode step (murmur_decode_step_layers): the length the opening call left the sequence at, and the layers
+  // whose range has not been issued yet (bit l).  open_len == -1: no step is open.
+  // (Fixed-size bitmap: layers >= 256 are counted but a repeated issue of one of them is not detected.)
+  int32_t open_len = -1;
+  int32_t open_left = 0;  // layers not issued yet
+  uint64_t open_todo[4] = {0, 0, 0, 0};
 };
 
 constexpr size_t kAlign = 256;
@@ -124,6 +130,10 @@ struct murmur_cache {
   uint32_t step_done = 0;       // value kCtrlStepDone reaches once every step launch counted so far is through its keepers
   IdxView idx{nullptr, nullptr, 0};        // indexed-mode tables (murmur_indexed_enable)
   unsigned long long* idx_moved = nullptr;  // device counter of rows moved by the last index-set eviction
+  // A call was recorded into a CUDA graph: the host mirror (lengths, free pages, open steps) was advanced although
+  // nothing ran, and replays will advance the device without the mirror.  Until murmur_mirror_sync has re-read the
+  // device state, every state-dependent call outside a capture returns MURMUR_ERR_STATE.
+  bool mirror_stale = false;
 };
 
 namespace {
@@ -164,6 +174,46 @@ float l2_keep_fraction(murmur_cache* c, const int32_t* seq_ids, int32_t n_seqs) 
   if (bytes <= 0 || bytes > kL2KeepMaxWorkingSet * (double)c->l2_bytes) return 0.f;
   const double f = kL2KeepShare * (double)c->l2_bytes / bytes;
   return (float)(f > 1.0 ? 1.0 : f);
+}
+
+// First line of every call that reads or advances the host mirror.  While `stream` is being captured the call is
+// let through and the handle is marked; afterwards calls are refused until murmur_mirror_sync has run.
+murmur_status_t mirror_guard(murmur_cache* c, void* stream) {
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing((cudaStream_t)stream, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone) {
+    c->mirror_stale = true;
+    return MURMUR_OK;
+  }
+  return c->mirror_stale ? MURMUR_ERR_STATE : MURMUR_OK;
+}
+#define MM_GUARD(c, stream)                                   \
+  do {                                                        \
+    if ((c) != nullptr) {                                     \
+      murmur_status_t g__ = mirror_guard((c), (stream));      \
+      if (g__ != MURMUR_OK) return g__;                       \
+    }                                                         \
+  } while (0)
+
+// ---- open-step bookkeeping (murmur_decode_step_layers) ----
+void open_step_mark(murmur_cache* c, HostSeq& hs, int32_t layer_begin, int32_t layer_end, bool opens) {
+  const int L = c->desc.n_layers;
+  if (opens) {
+    hs.open_len = hs.sp.len;
+    hs.open_left = L;
+    for (int w = 0; w < 4; ++w) hs.open_todo[w] = 0;
+    for (int l = 0; l < L && l < 256; ++l) hs.open_todo[l >> 6] |= 1ull << (l & 63);
+  }
+  for (int l = layer_begin; l < layer_end; ++l) {
+    if (l < 256) hs.open_todo[l >> 6] &= ~(1ull << (l & 63));
+    hs.open_left -= 1;
+  }
+  if (hs.open_left <= 0) hs.open_len = -1;  // every layer issued: the step is closed
+}
+bool open_step_has(const HostSeq& hs, int32_t layer_begin, int32_t layer_end) {
+  if (hs.open_len < 1 || hs.open_len != hs.sp.len || hs.evict_len != hs.sp.len) return false;
+  for (int l = layer_begin; l < layer_end && l < 256; ++l)
+    if (!((hs.open_todo[l >> 6] >> (l & 63)) & 1ull)) return false;
+  return true;
 }
 
 murmur_status_t check_ids(murmur_cache* c, const int32_t* ids, int32_t n, int want_indexed = 0) {
@@ -266,6 +316,7 @@ murmur_status_t murmur_cache_destroy(murmur_cache_t* c) {
 murmur_status_t murmur_seq_begin(murmur_cache_t* c, int32_t seq, int32_t n_prefix, int32_t n_speech, int32_t n_mid,
                                  const murmur_policy_t* pol, void* stream) {
   if (!c || !pol) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   if (seq < 0 || seq >= c->desc.max_seqs) return MURMUR_ERR_INVALID_ARG;
   if (n_prefix < 0 || n_speech < 0 || n_mid < 0) return MURMUR_ERR_INVALID_ARG;
   if (pol->w_speech < 0 || pol->delay < 0 || pol->n_sink_speech < 0 || pol->w_out < 0 || pol->n_sink_out < 0)
@@ -289,6 +340,7 @@ murmur_status_t murmur_seq_begin(murmur_cache_t* c, int32_t seq, int32_t n_prefi
 
 murmur_status_t murmur_seq_end(murmur_cache_t* c, int32_t seq, void* stream) {
   if (!c) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   if (seq < 0 || seq >= c->desc.max_seqs) return MURMUR_ERR_INVALID_ARG;
   HostSeq& hs = c->seqs[seq];
   if (!hs.active) return MURMUR_ERR_STATE;
@@ -328,6 +380,7 @@ static murmur_status_t append_impl(murmur_cache_t* c, const int32_t* seq_ids, co
                                    const void* k_new, const void* v_new, int32_t layer_begin, int32_t layer_end,
                                    bool fuse_evict, void* stream) {
   if (!c || !n_tokens) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   murmur_status_t st = check_ids(c, seq_ids, n_seqs);
   if (st != MURMUR_OK) return st;
   if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
@@ -402,6 +455,7 @@ murmur_status_t murmur_kv_append(murmur_cache_t* c, const int32_t* seq_ids, cons
 
 murmur_status_t murmur_kv_evict(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, void* stream) {
   if (!c) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   murmur_status_t st = check_ids(c, seq_ids, n_seqs);
   if (st != MURMUR_OK) return st;
   for (int base = 0; base < n_seqs; base += kMaxSeqsPerLaunch) {
@@ -422,6 +476,7 @@ static murmur_status_t attn_impl(murmur_cache_t* c, const int32_t* seq_ids, int3
                                  float* lse, int32_t layer_begin, int32_t layer_end, float sm_scale,
                                  const murmur_policy_t* window, void* stream) {
   if (!c) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   murmur_status_t st = check_ids(c, seq_ids, n_seqs);
   if (st != MURMUR_OK) return st;
   if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
@@ -511,6 +566,7 @@ static murmur_status_t step_layers_impl(murmur_cache_t* c, const int32_t* seq_id
   if (!c || !k_new || !v_new || !q || !out) return MURMUR_ERR_INVALID_ARG;
   if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
   if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   const bool opens = (layer_begin == 0);
   murmur_status_t st;
   if (opens) {
@@ -520,10 +576,10 @@ static murmur_status_t step_layers_impl(murmur_cache_t* c, const int32_t* seq_id
     if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch) return MURMUR_ERR_INVALID_ARG;
     st = check_ids(c, seq_ids, n_seqs);
     if (st != MURMUR_OK) return st;
-    for (int i = 0; i < n_seqs; ++i) {  // the step must have been opened: token reserved, eviction run
-      const HostSeq& hs = c->seqs[seq_ids[i]];
-      if (hs.sp.len < 1 || hs.evict_len != hs.sp.len) return MURMUR_ERR_STATE;
-    }
+    // the step must be open for every listed sequence (token reserved, eviction run by a layer_begin == 0 call, no
+    // append or evict since) and none of these layers issued yet: a second write would overwrite the token's rows
+    for (int i = 0; i < n_seqs; ++i)
+      if (!open_step_has(c->seqs[seq_ids[i]], layer_begin, layer_end)) return MURMUR_ERR_STATE;
   }
   int32_t ones[kMaxSeqsPerLaunch];
   for (int i = 0; i < n_seqs; ++i) ones[i] = 1;
@@ -558,6 +614,7 @@ static murmur_status_t step_layers_impl(murmur_cache_t* c, const int32_t* seq_id
       mirror_evict(c, seq_ids, n_seqs);  // ... and of the eviction
       c->stats.append_calls += 1;
     }
+    for (int i = 0; i < n_seqs; ++i) open_step_mark(c, c->seqs[seq_ids[i]], layer_begin, layer_end, opens);
     c->stats.attn_calls += 1;
     c->stats.attn_grid = li.grid;
     c->stats.attn_smem_bytes = li.smem;
@@ -571,6 +628,7 @@ static murmur_status_t step_layers_impl(murmur_cache_t* c, const int32_t* seq_id
     st = murmur_kv_evict(c, seq_ids, n_seqs, stream);
     if (st != MURMUR_OK) return st;
   }
+  for (int i = 0; i < n_seqs; ++i) open_step_mark(c, c->seqs[seq_ids[i]], layer_begin, layer_end, opens);
   return murmur_decode_attn(c, seq_ids, n_seqs, q, out, lse, layer_begin, layer_end, sm_scale, stream);
 }
 
@@ -612,6 +670,7 @@ murmur_status_t murmur_decode_step_host(murmur_cache_t* c, const int32_t* seq_id
                                         const void* k_new_host, const void* v_new_host, const void* q_host,
                                         void* out_host, float sm_scale, void* stream) {
   if (!c || !k_new_host || !v_new_host || !q_host || !out_host) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
   if (n_seqs < 1 || n_seqs > c->cv.stage_seqs) return MURMUR_ERR_INVALID_ARG;
   // validate before any copy so that a failing call leaves everything untouched
@@ -671,6 +730,7 @@ murmur_status_t murmur_prefill_attn(murmur_cache_t* c, int32_t seq, int32_t pos_
                                     void* stream) {
   murmur_status_t st = check_seq(c, seq);
   if (st != MURMUR_OK) return st;
+  MM_GUARD(c, stream);
   if (!q || !out) return MURMUR_ERR_INVALID_ARG;
   if (layer_begin < 0 || layer_end > c->desc.n_layers || layer_begin >= layer_end) return MURMUR_ERR_INVALID_ARG;
   if (!(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
@@ -829,6 +889,7 @@ murmur_status_t murmur_kv_evict_indexed(murmur_cache_t* c, int32_t seq, const in
                                         int32_t cap, int64_t* bytes_moved_out, void* stream) {
   murmur_status_t st = check_seq(c, seq);
   if (st != MURMUR_OK) return st;
+  MM_GUARD(c, stream);
   if (!sel_pos || !sel_cnt || cap < 1) return MURMUR_ERR_INVALID_ARG;
   if (!c->idx.pos) return MURMUR_ERR_STATE;  // murmur_indexed_enable first
   HostSeq& hs = c->seqs[seq];
@@ -878,6 +939,7 @@ murmur_status_t murmur_kv_evict_indexed(murmur_cache_t* c, int32_t seq, const in
 murmur_status_t murmur_kv_append_indexed(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* k_new,
                                          const void* v_new, void* stream) {
   if (!c || !k_new || !v_new) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch) return MURMUR_ERR_INVALID_ARG;
   murmur_status_t st = check_ids(c, seq_ids, n_seqs, 1);
   if (st != MURMUR_OK) return st;
@@ -909,6 +971,7 @@ murmur_status_t murmur_kv_append_indexed(murmur_cache_t* c, const int32_t* seq_i
 murmur_status_t murmur_decode_attn_indexed(murmur_cache_t* c, const int32_t* seq_ids, int32_t n_seqs, const void* q,
                                            void* out, float* lse, float sm_scale, void* stream) {
   if (!c || !q || !out) return MURMUR_ERR_INVALID_ARG;
+  MM_GUARD(c, stream);
   if (n_seqs < 1 || n_seqs > kMaxSeqsPerLaunch || !(sm_scale > 0.f)) return MURMUR_ERR_INVALID_ARG;
   murmur_status_t st = check_ids(c, seq_ids, n_seqs, 1);
   if (st != MURMUR_OK) return st;
@@ -1109,6 +1172,8 @@ murmur_status_t murmur_mirror_sync(murmur_cache_t* c, void* stream) {
   MM_CUDA(c, cudaMemcpy(&done, c->view.ctrl + kCtrlStepDone, 4, cudaMemcpyDeviceToHost));
   c->step_done = (uint32_t)done;
   c->chain_ok = false;
+  for (HostSeq& hs : c->seqs) hs.open_len = -1;  // replayed steps are whole steps: nothing is left open
+  c->mirror_stale = false;
   return MURMUR_OK;
 }
 

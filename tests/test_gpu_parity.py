@@ -697,6 +697,25 @@ def test_decode_step_layers_rejects_a_range_of_an_unopened_step(dev):
     assert c.seq_state(0)["length"] == 31
     c.decode_step_layers([0], k1, k1.clone(), q1, torch.empty_like(q1), 2, 3)
     assert c.seq_state(0)["length"] == 31 and c.last_error() == 0
+
+    def refused(lb, le):
+        n = le - lb
+        k, q = k1.expand(n, 1, 4, 128).contiguous(), q1.expand(n, 1, 28, 128).contiguous()
+        with pytest.raises(MurmurError) as e:
+            c.decode_step_layers([0], k, k.clone(), q, torch.empty_like(q), lb, le)
+        assert e.value.status == 2
+        assert c.seq_state(0)["length"] == 31
+
+    refused(2, 3)  # layer 2 was already issued in this step: a second write would overwrite the token's rows
+    refused(1, 3)  # ... also as part of a larger range
+    c.decode_step_layers([0], k1, k1.clone(), q1, torch.empty_like(q1), 1, 2)  # the last open layer: the step closes
+    refused(1, 2)  # every layer issued: no step is open any more
+    # a plain append + evict leaves evict_len == len as an opening call would, but opens no step
+    c.kv_append([0], [1], kv[:, :1].contiguous(), kv[:, :1].contiguous())
+    c.kv_evict([0])
+    with pytest.raises(MurmurError) as e:
+        c.decode_step_layers([0], k1, k1.clone(), q1, torch.empty_like(q1), 1, 2)
+    assert e.value.status == 2 and c.seq_state(0)["length"] == 32 and c.last_error() == 0
     c.close()
 
 
@@ -818,6 +837,12 @@ def test_decode_step_cuda_graph_replay(dev, layered):
         torch.cuda.synchronize()
         if step % 4 == 0 or step >= 36:
             a.check_attention(ids, q_buf, out_buf)
+    # the host mirror has not seen the replays: ordinary calls are refused until murmur_mirror_sync has run
+    from paper_2606_01483_b200 import MurmurError
+    for call in (lambda: a.gpu.kv_evict(ids), lambda: a.gpu.decode_step(ids, k_buf, v_buf, q_buf, out_buf, None, a.scale)):
+        with pytest.raises(MurmurError) as e:
+            call()
+        assert e.value.status == 2
     a.gpu.mirror_sync()
     a.check_integer_state(ids)
     # and on through the ordinary calls
