@@ -1,5 +1,6 @@
 """murmur_chunk_plan (host logic) against oracle/chunker.py, plus the properties that
-define a greedy merge.  No GPU needed: the function does no device work."""
+define a greedy merge.  No GPU needed: the function does no device work.  The oracle's own pins live in
+tests/test_oracle_chunker.py, which does not load the product."""
 import numpy as np
 import pytest
 
@@ -15,14 +16,6 @@ def _segments(rng, n, max_seg=120.0, max_gap=20.0):
         out.append((float(np.float32(t)), float(np.float32(t + d))))
         t = out[-1][1]
     return out
-
-
-def test_oracle_by_hand():
-    # spans: [0,100] + [110,290] = 290 <= 300 -> merged; [295,400] would make 400 -> new chunk; 350 s segment alone
-    seg = [(0, 100), (110, 290), (295, 400), (410, 760), (761, 800)]
-    assert o_chunk.greedy_chunks(seg, 300.0) == [[0, 1], [2], [3], [4]]
-    assert o_chunk.greedy_chunks([], 300.0) == []
-    assert o_chunk.greedy_chunks([(5, 6)], 300.0) == [[0]]
 
 
 @pytest.mark.parametrize("seed", range(20))
