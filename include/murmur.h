@@ -274,6 +274,29 @@ MURMUR_API murmur_status_t murmur_chunk_plan(const float* seg_start, const float
                                              float max_len, int32_t* chunk_first_seg, int32_t cap,
                                              int32_t* n_chunks_out);
 
+/* Batch formation ("Chunks are submitted as a batch to an inference engine"; "a batch size of
+ * 16 chunks" and the maximum-new-tokens rule).  For the chunks murmur_chunk_plan produced (same segment arrays,
+ * chunk_first_seg HOST int32[n_chunks], n_chunks <= n_segments), entry j describes chunk j:
+ *   batch, slot  chunks stay in time order and fill consecutive batches of batch_size: j / batch_size, j % batch_size
+ *                (slot = the sequence id to use in that batch's handle)
+ *   n_speech     S = ceil(tokens_per_s * d), d = the chunk's span in seconds (first segment's start to last one's end);
+ *                BASELINE.json's rate is 7.5 (300 s -> 2250 tokens)
+ *   max_new      T = floor(max_new_nominal * d / d_nominal) for d < d_nominal, else max_new_nominal; at least 1
+ *                (the paper: 32768 and 3600 s)
+ *   max_blocks   ceil((n_prefix + S + n_mid + T) / page_size): what murmur_cache_desc_t.max_blocks_per_seq must cover
+ * so that murmur_seq_begin(cache_of(batch), slot, n_prefix, n_speech, n_mid, policy) can follow directly.
+ *   entries        : HOST murmur_batch_entry_t[n_chunks] out;  *n_batches_out = ceil(n_chunks / batch_size)
+ * Decisions are taken in IEEE double.  MURMUR_ERR_INVALID_ARG on NULL / non-positive parameters, a chunk table that is
+ * not strictly ascending from 0, or a geometry that does not fit int32.  No GPU work, no handle. */
+typedef struct {
+  int32_t chunk, batch, slot, n_speech, max_new, max_blocks;
+} murmur_batch_entry_t;
+MURMUR_API murmur_status_t murmur_batch_plan(const float* seg_start, const float* seg_end, int32_t n_segments,
+                                             const int32_t* chunk_first_seg, int32_t n_chunks, int32_t batch_size,
+                                             double tokens_per_s, int32_t max_new_nominal, double d_nominal,
+                                             int32_t n_prefix, int32_t n_mid, int32_t page_size,
+                                             murmur_batch_entry_t* entries, int32_t* n_batches_out);
+
 /* ---- prefill ------------------------------------------------------------------------------- */
 /* Causal self-attention of prefill tokens: for the positions x in
  * [pos_begin, pos_end) of `seq`, out[l][x - pos_begin][h] = Eq. 1 of query q_x over

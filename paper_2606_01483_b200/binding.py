@@ -38,7 +38,7 @@ EXPORTED_SYMBOLS = [
     "murmur_decode_step", "murmur_decode_step_layers", "murmur_decode_step_chunked", "murmur_decode_step_host", "murmur_mirror_sync", "murmur_seq_get_state", "murmur_kv_get_retained", "murmur_kv_get_page_list",
     "murmur_kv_get_runs", "murmur_kv_get_free_stack", "murmur_kv_gather", "murmur_get_last_error",
     "murmur_profile_scratch_bytes", "murmur_attn_profile", "murmur_attn_profile_noalloc",
-    "murmur_decode_attn_windowed", "murmur_prefill_attn", "murmur_chunk_plan",
+    "murmur_decode_attn_windowed", "murmur_prefill_attn", "murmur_chunk_plan", "murmur_batch_plan",
     "murmur_indexed_bytes", "murmur_indexed_enable", "murmur_select_scratch_bytes", "murmur_select_mass_sets",
     "murmur_kv_evict_indexed", "murmur_kv_append_indexed", "murmur_decode_attn_indexed", "murmur_kv_get_indexed",
     "murmur_kv_gather_indexed",
@@ -113,6 +113,7 @@ def lib() -> C.CDLL:
         L.murmur_debug_step_trace.argtypes = [vp, vp, vp]
     L.murmur_decode_attn_windowed.argtypes = [vp, vp, i32, vp, vp, vp, i32, i32, C.c_float, vp, vp]
     L.murmur_chunk_plan.argtypes = [vp, vp, i32, C.c_float, vp, i32, vp]
+    L.murmur_batch_plan.argtypes = [vp, vp, i32, vp, i32, i32, C.c_double, i32, C.c_double, i32, i32, i32, vp, vp]
     L.murmur_prefill_attn.argtypes = [vp, i32, i32, i32, vp, vp, vp, i32, i32, C.c_float, vp]
     L.murmur_profile_scratch_bytes.argtypes = [vp, vp, i32, i32, i32]
     L.murmur_profile_scratch_bytes.restype = C.c_size_t
@@ -523,6 +524,27 @@ def chunk_plan(segments, max_len: float = 300.0):
         raise MurmurError(st, "murmur_chunk_plan")
     cuts = list(first[: n.value]) + [len(seg)]
     return [list(range(cuts[j], cuts[j + 1])) for j in range(n.value)]
+
+
+def batch_plan(segments, chunks, batch_size: int = 16, tokens_per_s: float = 7.5, max_new_nominal: int = 32768,
+               d_nominal: float = 3600.0, n_prefix: int = 0, n_mid: int = 0, page_size: int = 64):
+    """murmur_batch_plan: chunks (lists of segment indices, as chunk_plan returns them) -> list of batches, each a list
+    of dicts {chunk, slot, n_speech, max_new, max_blocks}."""
+    seg = np.ascontiguousarray(np.asarray(segments, dtype=np.float32).reshape(-1, 2))
+    a, b = np.ascontiguousarray(seg[:, 0]), np.ascontiguousarray(seg[:, 1])
+    first = np.ascontiguousarray(np.asarray([ch[0] for ch in chunks], dtype=np.int32))
+    ent = np.zeros((max(1, len(first)), 6), dtype=np.int32)
+    nb = C.c_int32(0)
+    st = lib().murmur_batch_plan(a.ctypes.data, b.ctypes.data, len(seg), first.ctypes.data, len(first), batch_size,
+                                 C.c_double(tokens_per_s), max_new_nominal, C.c_double(d_nominal), n_prefix, n_mid,
+                                 page_size, ent.ctypes.data, C.byref(nb))
+    if st != 0:
+        raise MurmurError(st, "murmur_batch_plan")
+    batches = [[] for _ in range(nb.value)]
+    for j in range(len(first)):
+        ch, bt, slot, S, T, mb = (int(x) for x in ent[j])
+        batches[bt].append({"chunk": ch, "slot": slot, "n_speech": S, "max_new": T, "max_blocks": mb})
+    return batches
 
 
 def version() -> str:
