@@ -31,12 +31,36 @@ class COracle:
         self._lib = lib
         lib.murmur_oracle_retained.restype = ctypes.c_int
         lib.murmur_oracle_retained.argtypes = [ctypes.c_int] * 10 + [ctypes.c_void_p, ctypes.c_int]
+        lib.murmur_oracle_prefill.restype = ctypes.c_int
+        lib.murmur_oracle_prefill.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_double,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
+        ]
         lib.murmur_oracle_attend.restype = ctypes.c_int
         lib.murmur_oracle_attend.argtypes = [
             ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
             ctypes.c_int64, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_double,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
         ]
+
+    def prefill(self, q_bits: np.ndarray, k_bits: np.ndarray, v_bits: np.ndarray, pos_begin: int, scale: float,
+                n_threads: int = 0) -> Tuple[np.ndarray, np.ndarray, int]:
+        """Causal prefill attention, several layers at once: q [L, n_tok, n_q, d], k/v [L, n_pos, n_kv, d] uint16 ->
+        (out [L, n_tok, n_q, d] f64, lse [L, n_tok, n_q] f64, threads)."""
+        q_bits = np.ascontiguousarray(q_bits, dtype=np.uint16)
+        k_bits = np.ascontiguousarray(k_bits, dtype=np.uint16)
+        v_bits = np.ascontiguousarray(v_bits, dtype=np.uint16)
+        L, n_tok, n_q, d = q_bits.shape
+        _, n_pos, n_kv, _ = k_bits.shape
+        out = np.empty((L, n_tok, n_q, d), dtype=np.float64)
+        lse = np.empty((L, n_tok, n_q), dtype=np.float64)
+        used = self._lib.murmur_oracle_prefill(
+            L, n_q, n_kv, d, k_bits.ctypes.data, v_bits.ctypes.data, n_pos, int(pos_begin), n_tok,
+            q_bits.ctypes.data, float(scale), out.ctypes.data, lse.ctypes.data, int(n_threads))
+        if used < 0:
+            raise RuntimeError("murmur_oracle_prefill failed")
+        return out, lse, used
 
     def retained(self, P: int, S: int, M: int, t: int, pol, length: Optional[int] = None) -> np.ndarray:
         total = P + S + M + t

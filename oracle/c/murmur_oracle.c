@@ -113,3 +113,76 @@ int murmur_oracle_attend(int n_layers, int n_q, int n_kv, int d, const uint16_t*
   }
   return failed ? -1 : used;
 }
+
+/* Causal self-attention of prefill tokens, Eq. 1 of every query position over the cache positions
+ * y <= x (the model is a decoder) - the plain-C twin of oracle/prefill.py::causal_attention, several
+ * layers at once.  One query row at a time, written out: scores, maximum, exponentials, sum, weighted V sum; no
+ * blocking, no running maximum.  OpenMP over (layer, query head) only.
+ * k, v : [n_layers][n_pos][n_kv][d] bf16 bits by absolute position, n_pos >= pos_begin + n_tok
+ * q    : [n_layers][n_tok][n_q][d]  bf16 bits, row i = position pos_begin + i
+ * out  : [n_layers][n_tok][n_q][d]  fp64;   lse: [n_layers][n_tok][n_q] fp64 or NULL
+ * Returns the number of threads used, or -1 on error. */
+int murmur_oracle_prefill(int n_layers, int n_q, int n_kv, int d, const uint16_t* k, const uint16_t* v,
+                          int64_t n_pos, int pos_begin, int n_tok, const uint16_t* q, double scale, double* out,
+                          double* lse, int n_threads) {
+  if (n_tok <= 0 || pos_begin < 0 || n_q % n_kv != 0 || (int64_t)pos_begin + n_tok > n_pos) return -1;
+  const int G = n_q / n_kv;
+  int used = 1;
+#ifdef _OPENMP
+  if (n_threads > 0) omp_set_num_threads(n_threads);
+  used = omp_get_max_threads();
+#else
+  (void)n_threads;
+#endif
+  int failed = 0;
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+  for (int layer = 0; layer < n_layers; ++layer) {
+    for (int h = 0; h < n_q; ++h) {
+      const int g = h / G;
+      const int64_t n_max = (int64_t)pos_begin + n_tok;
+      double* s = (double*)malloc((size_t)n_max * sizeof(double));
+      double* kf = (double*)malloc((size_t)n_max * d * sizeof(double)); /* this head's K and V rows as fp64 */
+      double* vf = (double*)malloc((size_t)n_max * d * sizeof(double));
+      double* qf = (double*)malloc((size_t)d * sizeof(double));
+      if (!s || !kf || !vf || !qf) {
+        failed = 1;
+        free(s); free(kf); free(vf); free(qf);
+        continue;
+      }
+      for (int64_t y = 0; y < n_max; ++y) {
+        const uint16_t* krow = k + (((size_t)layer * n_pos + y) * n_kv + g) * d;
+        const uint16_t* vrow = v + (((size_t)layer * n_pos + y) * n_kv + g) * d;
+        for (int c = 0; c < d; ++c) {
+          kf[y * d + c] = bf16_to_f64(krow[c]);
+          vf[y * d + c] = bf16_to_f64(vrow[c]);
+        }
+      }
+      for (int i = 0; i < n_tok; ++i) {
+        const int64_t x = (int64_t)pos_begin + i; /* attends y = 0 .. x */
+        const uint16_t* qrow = q + (((size_t)layer * n_tok + i) * n_q + h) * d;
+        for (int c = 0; c < d; ++c) qf[c] = bf16_to_f64(qrow[c]);
+        double m = -INFINITY;
+        for (int64_t y = 0; y <= x; ++y) { /* s_y = q . k_y * scale */
+          double acc = 0.0;
+          for (int c = 0; c < d; ++c) acc += qf[c] * kf[y * d + c];
+          s[y] = acc * scale;
+          if (s[y] > m) m = s[y];
+        }
+        double denom = 0.0;
+        for (int64_t y = 0; y <= x; ++y) { /* e_y = exp(s_y - m) */
+          s[y] = exp(s[y] - m);
+          denom += s[y];
+        }
+        double* o = out + (((size_t)layer * n_tok + i) * n_q + h) * d;
+        for (int c = 0; c < d; ++c) o[c] = 0.0;
+        for (int64_t y = 0; y <= x; ++y) { /* o = sum alpha_y v_y */
+          const double a = s[y] / denom;
+          for (int c = 0; c < d; ++c) o[c] += a * vf[y * d + c];
+        }
+        if (lse) lse[((size_t)layer * n_tok + i) * n_q + h] = m + log(denom);
+      }
+      free(s); free(kf); free(vf); free(qf);
+    }
+  }
+  return failed ? -1 : used;
+}

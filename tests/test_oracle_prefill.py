@@ -60,3 +60,56 @@ def test_brute_force_pure_python():
             z = sum(math.exp(t) for t in s)
             want = [sum(math.exp(s[y]) / z * vf[y][0][e] for y in range(x + 1)) for e in range(4)]
             assert np.allclose(o[i, h], want, atol=1e-12)
+
+
+# ---- the plain-C twin (oracle/c: murmur_oracle_prefill), used for the full-size every-row comparisons --------
+def _rand_layers(seed, L, n_pos, n_tok, n_q=28, n_kv=4, d=128):
+    rng = np.random.default_rng(seed)
+    return (_bits(rng.standard_normal((L, n_tok, n_q, d))), _bits(rng.standard_normal((L, n_pos, n_kv, d))),
+            _bits(rng.standard_normal((L, n_pos, n_kv, d))))
+
+
+def test_c_twin_matches_the_numpy_oracle_to_1e_12():
+    from oracle import c as oracle_c
+
+    co = oracle_c.load()
+    for seed, (L, n_pos, n_tok, pos_begin) in enumerate([(2, 90, 90, 0), (1, 150, 40, 110), (3, 33, 1, 32)]):
+        q, k, v = _rand_layers(10 + seed, L, n_pos, n_tok)
+        o_c, lse_c, used = co.prefill(q, k, v, pos_begin, 1.0 / math.sqrt(128), n_threads=1 + seed)
+        assert used >= 1
+        for layer in range(L):
+            o, lse = o_pre.causal_attention(q[layer], k[layer], v[layer], pos_begin, 1.0 / math.sqrt(128))
+            assert np.max(np.abs(o_c[layer] - o)) < 1e-12 and np.max(np.abs(lse_c[layer] - lse)) < 1e-12
+
+
+def test_c_twin_matches_library_causal_sdpa_fp64_and_the_decode_twin():
+    from oracle import c as oracle_c
+
+    co = oracle_c.load()
+    n = 70
+    q, k, v = _rand_layers(20, 1, n, n, n_q=4, n_kv=2, d=16)
+    o_c, lse_c, _ = co.prefill(q, k, v, 0, 0.25)
+    qt = torch.tensor(o_attn.bf16_bits_to_f64(q[0])).permute(1, 0, 2)
+    kt = torch.tensor(o_attn.bf16_bits_to_f64(k[0])).permute(1, 0, 2).repeat_interleave(2, dim=0)
+    vt = torch.tensor(o_attn.bf16_bits_to_f64(v[0])).permute(1, 0, 2).repeat_interleave(2, dim=0)
+    ref = torch.nn.functional.scaled_dot_product_attention(qt, kt, vt, is_causal=True, scale=0.25)
+    assert np.allclose(o_c[0], ref.permute(1, 0, 2).numpy(), atol=1e-12)
+    # row i is the decode twin (murmur_oracle_attend) over the retained set [0, i]
+    for i in (0, 13, 69):
+        o_d, lse_d, _ = co.attend(q[:, i], k, v, list(range(i + 1)), 0.25)
+        assert np.allclose(o_c[:, i], o_d, atol=1e-13) and np.allclose(lse_c[:, i], lse_d, atol=1e-12)
+    # a wrong causal boundary (y < x instead of y <= x) would make row 0 empty / change every row: row 0 must return v_0
+    assert np.allclose(o_c[0, 0, 0], o_attn.bf16_bits_to_f64(v)[0, 0, 0])
+
+
+def test_c_twin_rejects_bad_sizes():
+    from oracle import c as oracle_c
+
+    co = oracle_c.load()
+    q, k, v = _rand_layers(30, 1, 10, 5, n_q=4, n_kv=2, d=16)
+    try:
+        co.prefill(q, k, v, 6, 0.25)  # positions 6..10 need 11 cache rows
+    except RuntimeError:
+        pass
+    else:
+        raise AssertionError("pos_begin + n_tok > n_pos must be refused")
