@@ -55,6 +55,31 @@ def _check(out, lse, q, k, v, pos_begin, rows, scale):
     assert e.max() <= 2e-2 and e.mean() <= 2e-3, (e.max(), e.mean())
 
 
+def _check_every_row_c(out, lse, q, k, v, layers, q_heads, scale):
+    """EVERY row of the given layers and query heads against the plain-C fp64 twin of oracle/prefill.py
+    (oracle/c: murmur_oracle_prefill); q_heads must cover whole GQA groups.  Returns (max, mean) abs error."""
+    from oracle import c as oracle_c
+
+    co = oracle_c.load()
+    layers, q_heads = list(layers), list(q_heads)
+    G = q.shape[2] // k.shape[2]
+    kv_heads = sorted(set(h // G for h in q_heads))
+    assert q_heads == [g * G + j for g in kv_heads for j in range(G)]
+    li = torch.tensor(layers, device=q.device)
+    hi = torch.tensor(q_heads, device=q.device)
+    gi = torch.tensor(kv_heads, device=q.device)
+    qb = workloads.to_bits(q[li][:, :, hi])
+    kb, vb = workloads.to_bits(k[li][:, :, gi]), workloads.to_bits(v[li][:, :, gi])
+    o_ref, lse_ref, _ = co.prefill(qb, kb, vb, 0, scale)
+    got = out[li][:, :, hi].float().cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    e = np.abs(got - o_ref)
+    assert e.max() <= 2e-2 and e.mean() <= 2e-3, (e.max(), e.mean())
+    if lse is not None:
+        assert np.max(np.abs(lse[li][:, :, hi].cpu().numpy() - lse_ref)) < 2e-3
+    return float(e.max()), float(e.mean())
+
+
 @pytest.mark.parametrize("page,n_tok", [(16, 200), (32, 130), (64, 257), (64, 64), (16, 1)])
 def test_prefill_every_row_small(dev, page, n_tok):
     L = 2
@@ -112,7 +137,8 @@ def test_prefill_moving_row_maximum(dev, page):
 def test_prefill_many_single_tile_items_per_cta(dev):
     """100 positions x 28 layers: 448 work items of ONE 128-key tile each, three per persistent CTA back to back, every
     one with rows past the sequence length in its last (only) tile - the hand-overs between softmax, epilogue, producer
-    and issuer that a multi-tile item spaces out all fall on top of each other.  Repeated, bit-identical every time."""
+    and issuer that a multi-tile item spaces out all fall on top of each other.  The first run is compared with the oracle
+    on every row of every layer and head; then repeated, bit-identical every time."""
     L, n_tok = 28, 100
     c = _cache(dev, L, n_tok, 16)
     k, v = _rand((L, n_tok, 4, 128), 31, dev), _rand((L, n_tok, 4, 128), 32, dev)
@@ -120,7 +146,7 @@ def test_prefill_many_single_tile_items_per_cta(dev):
     c.kv_append([0], [n_tok], k, v)
     lse = torch.empty(L, n_tok, 28, dtype=torch.float32, device=dev)
     out = c.prefill_attn(0, 0, n_tok, q, lse=lse)
-    _check(out, lse, q, k, v, 0, [0, 1, 31, 64, 98, 99], 1 / math.sqrt(128))
+    _check_every_row_c(out, lse, q, k, v, range(L), range(28), 1 / math.sqrt(128))  # every row, layer and head
     for _ in range(50):
         again = c.prefill_attn(0, 0, n_tok, q)
         assert torch.equal(again, out)
@@ -141,6 +167,31 @@ def test_prefill_config2_size_sampled_rows(dev):
     out = c.prefill_attn(0, 0, n_tok, q, lse=lse)
     torch.cuda.synchronize()
     _check(out, lse, q, k, v, 0, [0, 1, 15, 16, 63, 64, 65, 127, 128, 1000, 2047, 2048, n_tok - 2, n_tok - 1], 1 / math.sqrt(128))
+    c.close()
+
+
+def test_prefill_config2_size_every_row(dev):
+    """The launch bench.py times - one 300 s chunk (64 prefix + 2250 speech tokens), all 28 layers in ONE launch whose
+    148 persistent CTAs walk ~7 500 work items - compared with the fp64 oracle on EVERY row: all 28 query heads of
+    layers 0, 9, 18 and 27 (early, middle and late items of the persistent schedule), and all 28 layers on the two
+    middle KV heads (query heads 7 .. 20).  Output and log-sum-exp, tolerance as everywhere (2e-2 / 2e-3)."""
+    cfg = workloads.config2()
+    d = workloads.SeqData(cfg, 0, device=dev)
+    k, v = d.prefill_kv()
+    k, v = k.contiguous(), v.contiguous()
+    L, n_tok = k.shape[0], k.shape[1]
+    assert (L, n_tok) == (28, 2314)
+    c = _cache(dev, L, n_tok, 64, P=64)
+    c.kv_append([0], [n_tok], k, v)
+    q = _rand((L, n_tok, 28, 128), 17, dev)
+    lse = torch.empty(L, n_tok, 28, dtype=torch.float32, device=dev)
+    out = c.prefill_attn(0, 0, n_tok, q, lse=lse)
+    torch.cuda.synchronize()
+    scale = 1 / math.sqrt(128)
+    _check_every_row_c(out, lse, q, k, v, [0, 9, 18, 27], range(28), scale)
+    for half in (range(0, 14), range(14, 28)):
+        _check_every_row_c(out, lse, q, k, v, half, range(7, 21), scale)
+    assert c.last_error() == 0
     c.close()
 
 
